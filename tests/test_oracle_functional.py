@@ -1,0 +1,283 @@
+"""Pins of the oracle's functionals, decomposition, L-BFGS and outer loop.
+
+Expected values come from: finite differences (definition of a gradient), the closed-form
+optimal-interpolation minimiser when the model is the identity, the paper's identities
+eq (12), (14), (19), (70) and Table 3, numpy's dense solver, and a pure-Python Jacobi
+iteration of per-point weighted means (the consensus fixed point when Phi = identity).
+"""
+import numpy as np
+import pytest
+
+from oracle import Oracle, lbfgs_minimize
+from paper_2205_06649_b200 import synth
+
+
+def make(w, **kw):
+    o = Oracle.from_workload(w, **kw)
+    prob = synth.make_problem(w, o.forecast)
+    o.set_background(prob.xb, prob.sigma_b)
+    o.set_observations(prob.obs)
+    return o, prob
+
+
+@pytest.fixture(scope="module")
+def c0():
+    return make(synth.CONFIGS[0])
+
+
+# ------------------------------------------------------------------ O4: global J
+def test_global_cost_is_zero_at_background_without_observations():
+    w = synth.CONFIGS[0]
+    o = Oracle.from_workload(w)
+    t0 = synth.truth_initial(w); sb, _ = synth.sigmas(t0)
+    o.set_background(t0, sb)
+    J, g, _ = o.eval_global(t0)
+    assert J == 0.0 and np.all(g == 0.0)
+
+
+def fd_check(fun, x, g, scale, seeds, h=1e-5, tol=2e-7):
+    """|fd - g.d| <= tol |g.d| + rounding floors: 8 eps |J| / h for the difference of two costs and
+    1e-8 ||g o scale|| for the rounding of x + h d itself (x ~ 1e4, h d ~ 1e-4)."""
+    J0 = abs(fun(x)); gn = np.linalg.norm(g * scale)
+    for sd in seeds:
+        d = synth.random_fields(x.shape, sd) * scale
+        fd = (fun(x + h * d) - fun(x - h * d)) / (2 * h)
+        an = np.vdot(g, d)
+        assert abs(fd - an) <= tol * abs(an) + 8 * 2.2e-16 * J0 / h + 1e-8 * gn, (sd, fd, an, gn)
+
+
+def test_global_gradient_vs_centred_finite_differences(c0):
+    o, prob = c0
+    sb = prob.sigma_b[:, None, None]
+    x = prob.xb + 0.3 * sb * synth.random_fields(prob.xb.shape, 3)
+    J, g, _ = o.eval_global(x)
+    fd_check(lambda z: o.eval_global(z, want_grad=False)[0], x, g, sb, range(100, 110))
+
+
+def test_local_gradient_vs_centred_finite_differences(c0):
+    o, prob = c0
+    for k in range(o.nsub):
+        s = o.subs[k]
+        sb = prob.sigma_b[:, None, None]
+        x = o.get_control(k) + 0.5 * sb * synth.random_fields(o.sub_shape(k), 7 + k)
+        parts, g, _ = o.eval_local(k, x)
+        assert parts[0] == pytest.approx(parts[1:].sum(), rel=1e-14)
+        assert parts[3] > 0                                  # spatial overlap term active
+        assert (parts[4] > 0) == (s["jw"] > 0) and (parts[5] > 0) == (s["jw"] < 1)
+        fd_check(lambda z: o.eval_local(k, z, want_grad=False)[0][0], x, g, sb, range(200, 204))
+
+
+def identity_model(w, **kw):
+    """dt = 0 and kappa = 0 make Phi the identity."""
+    args = dict(nlon=w.nlon, nlat=w.nlat, dt=0.0, nsteps=w.nsteps, diffusion=0.0)
+    args.update(kw)
+    return Oracle(**args)
+
+
+def test_identity_model_minimiser_is_optimal_interpolation():
+    """x* = (x_b/sb^2 + lam sum_k y_k/so^2) / (1/sb^2 + lam n_k/so^2) per point (3D-Var/OI)."""
+    w = synth.CONFIGS[0]
+    o = identity_model(w, lam=0.7, n_inner=40)
+    t0 = synth.truth_initial(w); sb, so = synth.sigmas(t0); so = 4 * so
+    xb = synth.background(w, t0, sb)
+    obs = synth.make_observations(w, np.repeat(t0[None], synth.obs_levels(w).size, 0), so)
+    o.set_background(xb, sb); o.set_observations(obs)
+    num = xb.reshape(-1) / np.repeat(sb ** 2, w.nlon * w.nlat)
+    den = 1.0 / np.repeat(sb ** 2, w.nlon * w.nlat)
+    fld = obs.index // (w.nlon * w.nlat)
+    np.add.at(num, obs.index, 0.7 * obs.value / so[fld] ** 2)
+    np.add.at(den, obs.index, 0.7 / so[fld] ** 2)
+    xstar = (num / den).reshape(xb.shape)
+    J, g, _ = o.eval_global(xstar)
+    assert np.abs(g * sb[:, None, None]).max() < 1e-9 * J    # stationary point of the oracle's J
+    an, hist = o.global_4dvar(1)
+    assert np.all(np.diff(hist) <= 0)
+    for f in range(3):
+        assert np.abs(an[f] - xstar[f]).max() < 1e-8 * sb[f]
+
+
+# ------------------------------------------------------------------ O5, O6: geometry
+LAYOUTS = [(1, 1, 1, 0), (2, 2, 2, 1), (3, 2, 4, 2), (4, 3, 1, 1), (1, 2, 2, 2), (5, 4, 3, 1)]
+
+
+@pytest.mark.parametrize("lay", LAYOUTS)
+def test_tile_extents_and_weights_sum_to_one(lay):
+    a, b, q, ov = lay
+    o = Oracle(40, 21, 100.0, 13, p_lon=a, p_lat=b, q_time=q, overlap=ov)
+    assert o.nsub == a * b * q
+    for k, s in enumerate(o.subs):
+        # eq (70): n/p + 2 o (truncated at the pole walls, none when p = 1)
+        assert s["ex"] == (s["oi1"] - s["oi0"]) + (2 * ov if a > 1 else 0)
+        assert s["ey"] == (s["oj1"] - s["oj0"]) + ov * ((s["oj0"] > 0) + (s["oj1"] < 21))
+        assert s["oi0"] == (s["a"] * 40) // a and s["oj1"] == ((s["b"] + 1) * 21) // b
+        assert s["s"] == (s["jw"] * 13) // q and s["e"] == ((s["jw"] + 1) * 13) // q
+    # eq (12): u = sum EO[RO_ji u] at every space-time point <=> weights sum to 1
+    rng = np.random.default_rng(1)
+    for level in range(14):
+        tot = np.zeros((21, 40)); u = rng.standard_normal((21, 40)); rec = np.zeros((21, 40))
+        for k, s in enumerate(o.subs):
+            wt = o.sub_weight(k, level)
+            jj = s["ej0"] + np.arange(s["ey"]); ii = (s["ei0"] + np.arange(s["ex"])) % 40
+            np.add.at(tot, (jj[:, None], ii[None, :]), wt)
+            np.add.at(rec, (jj[:, None], ii[None, :]), wt * u[jj[:, None], ii[None, :]])
+        assert np.allclose(tot, 1.0, rtol=0, atol=1e-15)
+        assert np.allclose(rec, u, rtol=0, atol=1e-14)       # eq (14) round trip
+
+
+def test_restriction_weights_reduce_to_the_papers_halves_and_quarters():
+    """Def 4 PAPER.md:170 for Omega in R (1-D space: a single latitude band): 1, 1/2, 1/2, 1/4."""
+    o = Oracle(40, 6, 100.0, 12, p_lon=4, p_lat=1, q_time=3, overlap=2)
+    s = o.subs[1]
+    w_in = o.sub_weight(1, 2); w_tb = o.sub_weight(1, 4)     # level 4 is shared with window 1
+    assert set(np.unique(w_in)) == {0.5, 1.0} and set(np.unique(w_tb)) == {0.25, 0.5}
+    assert np.all(w_in[:, :4] == 0.5) and np.all(w_in[:, 4:-4] == 1.0)
+
+
+def test_table3_problem_sizes():
+    """Table 3: problem size = QP * 3 * 32^2."""
+    printed = {2: 6.1e3, 4: 1.2e4, 8: 2.4e4, 16: 4.9e4, 32: 9.8e4, 64: 1.9e5}
+    for qp, val in printed.items():
+        assert qp * 3 * 32 ** 2 == pytest.approx(val, rel=0.04)
+
+
+def test_decomposition_that_does_not_fit_is_rejected():
+    with pytest.raises(ValueError):
+        Oracle(36, 18, 600.0, 4, q_time=5)                   # more windows than steps
+    with pytest.raises(ValueError):
+        Oracle(36, 18, 600.0, 4, p_lat=9, overlap=1)         # ghost ring leaves the owner band
+
+
+# ------------------------------------------------------------------ O7: local functional
+@pytest.mark.parametrize("lay", [(1, 1, 1, 0), (2, 2, 2, 1), (3, 2, 4, 2), (1, 3, 2, 1), (2, 1, 1, 2)])
+def test_sum_of_local_functionals_at_background_is_global(lay):
+    """eq (19) PAPER.md:288 at u^b (overlap terms vanish, weights split the observation term)."""
+    a, b, q, ov = lay
+    o, prob = make(synth.CONFIGS[0].with_layout(a, b, q, ov))
+    Jg, _, _ = o.eval_global(prob.xb, want_grad=False)
+    parts = np.array([o.eval_local(k, o.get_control(k), want_grad=False)[0] for k in range(o.nsub)])
+    assert np.all(parts[:, 1] == 0) and np.all(parts[:, 3:] == 0)
+    assert parts[:, 0].sum() == pytest.approx(Jg, rel=1e-13)
+
+
+def test_local_sweep_with_exact_ghost_data_reproduces_global_trajectory(c0):
+    o, prob = c0
+    w = prob.w
+    ub = o.forecast(prob.xb, np.arange(w.nsteps + 1))
+    for k, s in enumerate(o.subs):
+        _, _, tr = o.eval_local(k, o.get_control(k), want_grad=False, want_traj=True)
+        jj = s["ej0"] + np.arange(s["ey"]); ii = (s["ei0"] + np.arange(s["ex"])) % w.nlon
+        ref = ub[s["s"]:s["e"] + 1][:, :, jj[:, None], ii[None, :]]
+        assert np.array_equal(tr, ref)                       # bit for bit: same operation order
+
+
+def test_undecomposed_layout_equals_plain_global_4dvar(c0):
+    _, prob = c0
+    o, _ = make(prob.w.with_layout(1, 1, 1, 0))
+    an_g, hist_g = o.global_4dvar(4)
+    an_d, hist_d = o.run(4)
+    assert np.allclose(hist_d[:, 0], hist_g, rtol=1e-12)
+    assert np.allclose(hist_d[1:, 1], hist_g[1:], rtol=1e-12)
+    for f in range(3):
+        assert np.linalg.norm(an_d[f] - an_g[f]) <= 1e-12 * np.linalg.norm(an_g[f])
+    assert hist_g[-1] < 0.2 * hist_g[0]
+
+
+# ------------------------------------------------------------------ O8: L-BFGS
+def test_lbfgs_solves_spd_quadratic_like_dense_solver():
+    rng = np.random.default_rng(5)
+    Q = rng.standard_normal((20, 20)); A = Q @ Q.T + 20 * np.eye(20); b = rng.standard_normal(20)
+    fun = lambda w: (0.5 * w @ A @ w - b @ w, A @ w - b)
+    w, J = lbfgs_minimize(fun, np.zeros(20), m=25, n_iter=60)
+    xs = np.linalg.solve(A, b)
+    # an Armijo test on J resolves the minimiser to ~sqrt(eps) relative, the cost to ~eps
+    assert np.abs(w - xs).max() < 1e-7 * np.abs(xs).max()
+    assert J == pytest.approx(fun(xs)[0], rel=1e-13)
+
+
+def test_lbfgs_cost_is_monotone_and_handles_zero_gradient():
+    rng = np.random.default_rng(6)
+    A = np.diag(np.logspace(0, 3, 12)); b = rng.standard_normal(12)
+    seen = []
+
+    def fun(w):
+        J = 0.5 * w @ A @ w - b @ w + 0.25 * np.sum(w ** 4)
+        return J, A @ w - b + w ** 3
+    for it in range(1, 8):
+        _, J = lbfgs_minimize(fun, np.zeros(12), m=3, n_iter=it)
+        seen.append(J)
+    assert np.all(np.diff(seen) <= 1e-15)
+    w, J = lbfgs_minimize(lambda w: (0.0, np.zeros_like(w)), np.ones(4), n_iter=3)
+    assert np.array_equal(w, np.ones(4))
+
+
+# ------------------------------------------------------------------ O9: outer loop
+def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity():
+    """Phi = identity decouples the grid points: each local solve is a per-point weighted mean
+    of background, observations and the neighbours' frozen values (eq (25)); iterate that
+    Jacobi map in NumPy and compare every outer iteration's gathered analysis."""
+    w = synth.CONFIGS[0]
+    nlon, nlat, N, ov, mu, lam = 12, 8, 4, 1, 0.8, 1.3
+    o = Oracle(nlon, nlat, 0.0, N, p_lon=2, p_lat=2, q_time=2, overlap=ov, mu=mu, lam=lam,
+               diffusion=0.0, n_inner=60, lbfgs_m=10)
+    rng = np.random.default_rng(9)
+    xb = rng.standard_normal((3, nlat, nlon)); sb = np.array([1.0, 2.0, 0.5]); so = np.array([0.7, 0.9, 1.1])
+    levels = np.array([0, 2, 4], dtype=np.int32)
+    cells = np.sort(rng.choice(nlon * nlat, 40, replace=False))
+    idx1 = np.concatenate([cells + f * nlon * nlat for f in range(3)]).astype(np.int32)
+    obs = synth.Observations(levels, np.arange(4, dtype=np.int64) * idx1.size, np.tile(idx1, 3),
+                             rng.standard_normal(3 * idx1.size), so)
+    o.set_background(xb, sb); o.set_observations(obs)
+    # independent NumPy model of the iteration, on global arrays per (window, tile)
+    subs = o.subs
+    cover = [np.zeros((nlat, nlon), bool) for _ in subs]
+    for k, s in enumerate(subs):
+        jj = s["ej0"] + np.arange(s["ey"]); ii = (s["ei0"] + np.arange(s["ex"])) % nlon
+        cover[k][jj[:, None], ii[None, :]] = True
+    mult = sum(c.astype(int) for c in cover[:4])
+    X = [xb.copy() for _ in subs]                            # controls (identity: = trajectories)
+    yv = obs.value.reshape(3, 3, -1)                         # [time][field][cell]
+    for it in range(1, 4):
+        Xn = []
+        for k, s in enumerate(subs):
+            num = np.zeros_like(xb); den = np.zeros_like(xb)
+            for f in range(3):
+                num[f] += xb[f] / mult / sb[f] ** 2; den[f] += 1.0 / mult / sb[f] ** 2
+                for t, lev in enumerate(levels):
+                    if s["s"] <= lev <= s["e"]:
+                        wt = 1.0 / mult.reshape(-1)[cells] / (2.0 if lev == 2 else 1.0)
+                        np.add.at(num[f].reshape(-1), cells, lam * wt * yv[t, f] / so[f] ** 2)
+                        np.add.at(den[f].reshape(-1), cells, lam * wt / so[f] ** 2)
+                for k2, s2 in enumerate(subs):
+                    if k2 == k:
+                        continue
+                    if s2["jw"] == s["jw"]:                  # spatial neighbours, case 1
+                        m = cover[k2]
+                    elif (s2["a"], s2["b"]) == (s["a"], s["b"]):   # same tile, other window
+                        m = np.ones((nlat, nlon), bool)
+                    else:
+                        continue
+                    num[f] += mu * m * X[k2][f] / sb[f] ** 2; den[f] += mu * m / sb[f] ** 2
+            Xn.append(np.where(cover[k][None], num / den, xb))
+        X = Xn
+        an_ref = sum(np.where(cover[k][None], X[k], 0.0) for k in range(4)) / mult
+        o2 = Oracle(nlon, nlat, 0.0, N, p_lon=2, p_lat=2, q_time=2, overlap=ov, mu=mu, lam=lam,
+                    diffusion=0.0, n_inner=60, lbfgs_m=10)
+        o2.set_background(xb, sb); o2.set_observations(obs)
+        an, hist = o2.run(it)
+        assert np.abs(an - an_ref).max() < 1e-8, it
+    assert hist[-1, 2] < hist[1, 2]                          # delta_l shrinks
+
+
+def test_config0_run_history_behaviour(c0):
+    """Reported behaviour (no guarantee in the paper beyond Theorem 1's convex case): on config 0
+    J(gathered analysis), sum J_ji and delta_l all fall; the analysis beats the background."""
+    _, prob = c0
+    o, _ = make(prob.w)
+    an, hist = o.run(6)
+    assert hist[0, 0] == pytest.approx(hist[0, 1], rel=1e-13)
+    assert np.all(np.diff(hist[:, 0]) < 0) and np.all(np.diff(hist[1:, 1]) < 0)
+    assert np.all(np.diff(hist[1:, 2]) < 0)
+    for f in range(3):
+        assert np.linalg.norm(an[f] - prob.truth0[f]) < 0.6 * np.linalg.norm(prob.xb[f] - prob.truth0[f])
+    tr = o.get_trajectory(0)
+    assert np.allclose(tr, an, rtol=0, atol=1e-12 * np.abs(an).max())
