@@ -1,0 +1,166 @@
+/*
+ * dd4dvar.h -- C-ABI of the B200-native space-time decomposed 4D-Var (DD-4DVar) library.
+ *
+ * Method: arXiv 2205.06649 (text: /root/reference/PAPER.md; "l.N" below = PAPER.md line N).
+ * The library evaluates, on every overlapping space-time subdomain Delta_j x Omega_i at once,
+ * the regularised local functional J_ji (Def 13 eq (23)-(25), l.326-344) and its gradient by a
+ * forward sweep of the discretised shallow-water model (eq (60)-(62) l.945-954, discretisation
+ * l.971-989) and an adjoint backward sweep (eq (3)-(4) l.91-98), and drives a batched
+ * per-subdomain L-BFGS (Remark 3 l.595; l.941) inside the outer loop of Algorithm 1 (l.443-472).
+ * The readings of the paper that fix every constant and convention are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every `d_*` pointer is DEVICE memory owned by the caller (e.g. a torch tensor's data_ptr());
+ *     every `h_*` pointer is HOST memory owned by the caller.  The library keeps no pointer to
+ *     caller memory after a call returns, except the workspaces handed over with
+ *     dd4dvar_set_workspace / dd4dvar_set_observations, which must outlive the handle.
+ *   - Fields are ordered (h, u, v).  A global state is fp64 [3][nlat][nlon], longitude fastest;
+ *     row j is the cell-centred latitude theta_j = -pi/2 + (j + 1/2) pi/nlat.
+ *   - A subdomain's control / gradient is fp64 [3][ey][ex] on its extended tile (owned range
+ *     plus `overlap` cells on every interior side, periodic in longitude, cut at the pole
+ *     walls).  "All subdomains" arrays are the concatenation of these in subdomain order
+ *     k = (window * p_lat + tile_row) * p_lon + tile_col; offsets from dd4dvar_subdomain_info.
+ *   - All work is queued on the CUDA stream given to dd4dvar_create; calls that return host
+ *     values synchronise that stream before returning.
+ *   - Return value: 0 on success, otherwise
+ *       -1 invalid argument            -2 decomposition does not fit the grid / window
+ *       -3 called out of order         -4 CUDA error          -5 non-finite cost
+ *     Nothing is thrown across the ABI; dd4dvar_last_error gives the text of the last failure.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns -4.
+ */
+#ifndef DD4DVAR_H
+#define DD4DVAR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dd4dvar_s* dd4dvar_t; /* opaque, library-owned */
+
+/* Grid and model constants: eq (60)-(62) l.945-954 (a, Omega, g), index ranges eq (67) l.976-980.
+ * cos_clamp: lower bound of the cos(theta) metric factor (R3); diffusion: the
+ * dimensionless index-space diffusion kappa of stage A (R3). */
+typedef struct {
+    int nlon, nlat;
+    double radius, omega, gravity;
+    double cos_clamp;
+    double diffusion;
+} dd4dvar_grid;
+
+/* Uniform space-time decomposition, Def 3 l.128-154 and Def 16 l.755-763: p_lon x p_lat tiles
+ * times q_time windows; `overlap` cells are added on each interior side (eq (70) l.1024).
+ * mu = weight of the overlap term (25c) l.344; lambda = weight of the observation term eq (6)
+ * l.111. */
+typedef struct {
+    int p_lon, p_lat, q_time;
+    int overlap;
+    double mu, lambda;
+} dd4dvar_decomp;
+
+/* Assimilation window: nsteps model steps of dt seconds, time levels 0..nsteps (Def 1 l.78-87). */
+typedef struct {
+    double dt;
+    int nsteps;
+} dd4dvar_window;
+
+/* Local minimiser (L-BFGS, R10): history length, iterations per outer iteration,
+ * maximum number of step halvings, Armijo constant.
+ * path: 0 = choose automatically, 1 = force the generic (per-step, global-memory) kernels,
+ *       2 = force the fused persistent kernels (create fails with -2 if a tile does not fit). */
+typedef struct {
+    int lbfgs_m, n_inner, max_backtrack;
+    double armijo_c1;
+    int path;
+} dd4dvar_opts;
+
+/* Build the handle: row tables, decomposition, device descriptors.  `cuda_stream` is a
+ * cudaStream_t (NULL = the legacy default stream).  Fails with -2 if a tile is narrower than its
+ * ghost ring allows, a window has no step, or overlap regions would cover a cell more than 4x4
+ * times. */
+int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp,
+                   const dd4dvar_window* window, const dd4dvar_opts* opts, void* cuda_stream,
+                   dd4dvar_t* out);
+
+/* Device memory the library needs besides the observations; the caller allocates it (256-byte
+ * aligned) and hands it over before set_background. */
+size_t dd4dvar_workspace_bytes(dd4dvar_t h);
+int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes);
+
+/* Background u_0^b and B = diag(sigma_b^2 per field) (Def 1 l.82, eq (6) l.111).  Runs the model
+ * from d_xb over the whole window (Alg 1 l.452: u^b = M(u_0^b)), sets every local control to
+ * the restricted background (l.455) and all frozen neighbour data to the background trajectory. */
+int dd4dvar_set_background(dd4dvar_t h, const double* d_xb, const double h_sigma_b[3]);
+
+/* Observations v_k, H = selection of grid values, R = diag(sigma_o^2 per field) (Def 1 l.83-85;
+ * DESIGN.md R20).  h_levels: n_times strictly ascending time levels in [0, nsteps];
+ * h_offsets[n_times+1]: start of each level's block in d_index / d_value; d_index: flat index
+ * into [3][nlat][nlon], strictly ascending inside a level; d_value: observed values.
+ * The restriction of H to each subdomain (Def 8 l.239) is built here.  d_obs_ws: device
+ * workspace of at least dd4dvar_obs_workspace_bytes(h, total) bytes, total = h_offsets[n_times]. */
+size_t dd4dvar_obs_workspace_bytes(dd4dvar_t h, long long n_obs_total);
+int dd4dvar_set_observations(dd4dvar_t h, int n_times, const int* h_levels,
+                             const long long* h_offsets, const int* d_index,
+                             const double* d_value, const double h_sigma_o[3], void* d_obs_ws,
+                             size_t obs_ws_bytes);
+
+/* Algorithm 1 l.443-472: `outer_iters` additive (Jacobi) outer iterations, each = n_inner
+ * L-BFGS iterations on every subdomain at once followed by the exchange of overlap / boundary
+ * data (l.465).  Continues from the current local controls (fresh after set_background).
+ * d_analysis [3][nlat][nlon]: gathered analysis at t_0 (eq (12)-(13) l.194-201).
+ * h_history [(outer_iters+1)][3]: row l = J(gathered analysis after iteration l) by eq (6),
+ * sum_ji J_ji at the end of iteration l (row 0: at the start of iteration 1),
+ * delta_l = max_ji ||u_ji^l - u_ji^(l-1)||_inf (l.466; row 0: 0). */
+int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_history);
+
+/* eq (6) l.111 and its gradient by one forward + one adjoint sweep over the whole grid.
+ * d_x0 [3][nlat][nlon]; h_cost[1]; d_grad [3][nlat][nlon] or NULL. */
+int dd4dvar_eval_global(dd4dvar_t h, const double* d_x0, double* h_cost, double* d_grad);
+
+/* The hot path: J_ji (eq (25) l.338-344) and dJ_ji/dx of EVERY subdomain at the given controls,
+ * with the current frozen neighbour data: forward sweep + trajectory store, misfit / background /
+ * overlap terms, adjoint sweep.  d_controls, d_grads: "all subdomains" arrays (physical units);
+ * d_grads may be NULL (forward sweep and costs only).  h_costs[nsub]; h_parts[nsub][5] or NULL =
+ * background (25a), observation (25b), spatial-overlap, predecessor and successor terms (25c). */
+int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, double* h_parts,
+                       double* d_grads);
+
+/* Same evaluation, queued on the stream without host synchronisation or host output, at the
+ * library's own current controls: used for timing the gradient sweep (bench.py). */
+int dd4dvar_sweep_async(dd4dvar_t h, int with_adjoint);
+
+/* Copy the current local controls of all subdomains ("all subdomains" array, physical units). */
+int dd4dvar_get_controls(dd4dvar_t h, double* d_controls);
+
+/* Gathered state at a time level from the stored local trajectories: weighted extension-sum
+ * with weights 1/multiplicity (Def 4 l.164-170, eq (12) l.196).  d_out [3][nlat][nlon]. */
+int dd4dvar_get_trajectory(dd4dvar_t h, int level, double* d_out);
+
+/* Local trajectory of subdomain `sub` as stored by the last sweep: d_out [(W+1)][3][ey][ex]. */
+int dd4dvar_get_local_trajectory(dd4dvar_t h, int sub, double* d_out);
+
+/* Model only: run the forecast from d_x0 and return the states at the given ascending levels,
+ * d_out [n_levels][3][nlat][nlon] (used to generate twin-experiment observations, l.993-995). */
+int dd4dvar_forecast(dd4dvar_t h, const double* d_x0, int n_levels, const int* h_levels,
+                     double* d_out);
+
+int dd4dvar_num_subdomains(dd4dvar_t h);
+/* out[16] = tile_col, tile_row, window, owned i0,i1,j0,j1, ext i0 (may be < 0: wraps), ext j0,
+ * ex, ey, ghost width lon, ghost south, ghost north, first level s, last level e. */
+int dd4dvar_subdomain_info(dd4dvar_t h, int sub, int out[16]);
+/* offset (in doubles) of subdomain `sub` inside an "all subdomains" array; sub = nsub gives the
+ * total length. */
+long long dd4dvar_control_offset(dd4dvar_t h, int sub);
+/* which kernels serve the local sweeps: 1 generic, 2 fused persistent */
+int dd4dvar_active_path(dd4dvar_t h);
+/* number of kernel launches issued by this handle so far (bench.py's gpu_launches) */
+long long dd4dvar_launch_count(dd4dvar_t h);
+
+const char* dd4dvar_last_error(dd4dvar_t h);
+void dd4dvar_destroy(dd4dvar_t h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DD4DVAR_H */

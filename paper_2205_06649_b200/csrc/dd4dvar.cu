@@ -1,0 +1,746 @@
+// dd4dvar.cu -- host side of the DD-4DVar library: geometry, workspace plan, the outer driver of
+// Algorithm 1 and the C-ABI of include/dd4dvar.h.  All arithmetic of the
+// hot path runs in the kernels of generic_kernels.cuh / fused_kernels.cuh / lbfgs_kernels.cuh /
+// exchange_kernels.cuh; there is no CPU fallback.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <string>
+#include <vector>
+
+#include "../../include/dd4dvar.h"
+#include "common.cuh"
+#include "exchange_kernels.cuh"
+#include "fused_kernels.cuh"
+#include "generic_kernels.cuh"
+#include "lbfgs_kernels.cuh"
+
+namespace {
+
+constexpr int NT_GK = 256;     // generic kernels: threads per block
+constexpr int NT_RED = 256;    // cost reduction
+constexpr int NT_LB = 512;     // L-BFGS CTA
+
+struct Arena {
+    char* base = nullptr;
+    size_t off = 0, cap = 0;
+    template <class T> T* take(size_t n)
+    {
+        off = (off + 255) & ~size_t(255);
+        T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+void* ar_take_bytes(void* arena, size_t bytes) { return static_cast<Arena*>(arena)->take<char>(bytes); }
+
+struct Layout {
+    int p1 = 1, p2 = 1, q = 1, o = 0, nsub = 0;
+    bool lbfgs = false;
+    int path = 1;                       // 1 generic, 2 fused
+    std::vector<Sub> hs;
+    std::vector<int> colown, rowown, ncolcov, colcov, nrowcov, rowcov, tc_ei0, tc_ex, tr_ej0, tr_ey, wb;
+    long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0;
+    int maxnpad = 0, maxncell = 0, maxnring = 0, Wmax = 0, CB = 1, maxcov = 1;
+    // device
+    Sub* dsubs = nullptr;
+    GeoP geo{};
+    int* itab = nullptr;
+    double *x = nullptr, *xbs = nullptr, *xfrozen = nullptr, *pred_end = nullptr, *gx = nullptr;
+    double *traj = nullptr, *ghost = nullptr;
+    double *Zp = nullptr, *Za = nullptr, *lamA = nullptr, *lamB = nullptr, *A = nullptr;
+    double *H1 = nullptr, *HB = nullptr, *P = nullptr, *UB = nullptr;
+    double *partial = nullptr, *parts = nullptr, *Jev = nullptr, *dmax = nullptr;
+    double *w = nullptr, *wt = nullptr, *g = nullptr, *gn = nullptr, *d = nullptr, *S = nullptr, *Y = nullptr;
+    LbfgsState st{};
+    int* okmask = nullptr;
+    // observations binned per (subdomain, local level)
+    bool have_obs = false;
+    long long* obs_start = nullptr;
+    int* obs_idx = nullptr;
+    double *obs_y = nullptr, *obs_c = nullptr;
+    FusedPlan fp{};
+};
+
+}  // namespace
+
+struct dd4dvar_s {
+    dd4dvar_grid grid;
+    dd4dvar_decomp dec;
+    dd4dvar_window win;
+    dd4dvar_opts opt;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    long long launches = 0;
+    // model tables
+    std::vector<double> h_tab;          // 6 x nlat
+    double* d_tab = nullptr;
+    ModelP mp{};
+    CostP cp{};
+    double sig_o[3] = { 1, 1, 1 };
+    Layout G, L;
+    bool have_ws = false, have_bg = false;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    int* h_pin = nullptr;               // pinned scratch for small read-backs
+    std::vector<double> h_tmp;
+};
+
+namespace {
+
+int fail(dd4dvar_t h, int code, const std::string& msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+#define CU(call)                                                                         \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess)                                                           \
+            return fail(h, -4, std::string(#call) + ": " + cudaGetErrorString(e_));      \
+    } while (0)
+#define LAUNCH(kern, grid, block, ...)                        \
+    do {                                                      \
+        kern<<<grid, block, 0, h->stream>>>(__VA_ARGS__);     \
+        ++h->launches;                                        \
+    } while (0)
+
+int imod(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }
+
+// ---- geometry: Def 3 l.128-154, Def 16 l.755-763, eq (70) l.1024; ragged split DESIGN.md R9
+int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, int o)
+{
+    L.p1 = p1; L.p2 = p2; L.q = q; L.o = o;
+    if (p1 < 1 || p2 < 1 || q < 1 || o < 0 || q > N) return -2;
+    if ((long long)p1 * p2 * q > 65535) return -2;
+    L.nsub = p1 * p2 * q;
+    L.wb.resize(q + 1);
+    for (int j = 0; j <= q; ++j) L.wb[j] = (int)(((long long)j * N) / q);
+    L.tc_ei0.resize(p1); L.tc_ex.resize(p1); L.tr_ej0.resize(p2); L.tr_ey.resize(p2);
+    std::vector<int> oi0(p1), oi1(p1), oj0(p2), oj1(p2), gys(p2), gyn(p2);
+    for (int a = 0; a < p1; ++a) {
+        oi0[a] = (int)(((long long)a * nlon) / p1); oi1[a] = (int)(((long long)(a + 1) * nlon) / p1);
+        if (oi1[a] <= oi0[a]) return -2;
+        if (p1 == 1) { L.tc_ei0[a] = 0; L.tc_ex[a] = nlon; }
+        else { L.tc_ei0[a] = oi0[a] - o; L.tc_ex[a] = oi1[a] - oi0[a] + 2 * o; }
+        if (L.tc_ex[a] > nlon) return -2;
+    }
+    for (int b = 0; b < p2; ++b) {
+        oj0[b] = (int)(((long long)b * nlat) / p2); oj1[b] = (int)(((long long)(b + 1) * nlat) / p2);
+        if (oj1[b] <= oj0[b]) return -2;
+        int j0 = std::max(oj0[b] - o, 0), j1 = std::min(oj1[b] + o, nlat);
+        L.tr_ej0[b] = j0; L.tr_ey[b] = j1 - j0;
+        gys[b] = j0 == 0 ? 0 : DD_GHOST; gyn[b] = j1 == nlat ? 0 : DD_GHOST;
+        if (j0 - gys[b] < 0 || j1 + gyn[b] > nlat) return -2;        // ghost ring off the grid
+    }
+    L.colown.assign(nlon, 0); L.rowown.assign(nlat, 0);
+    L.ncolcov.assign(nlon, 0); L.colcov.assign(4 * nlon, 0);
+    L.nrowcov.assign(nlat, 0); L.rowcov.assign(4 * nlat, 0);
+    for (int a = 0; a < p1; ++a) {
+        for (int i = oi0[a]; i < oi1[a]; ++i) L.colown[i] = a;
+        for (int li = 0; li < L.tc_ex[a]; ++li) {
+            int gi = imod(L.tc_ei0[a] + li, nlon);
+            if (L.ncolcov[gi] >= 4) return -2;
+            L.colcov[4 * gi + L.ncolcov[gi]++] = a;
+        }
+    }
+    for (int b = 0; b < p2; ++b) {
+        for (int j = oj0[b]; j < oj1[b]; ++j) L.rowown[j] = b;
+        for (int lj = 0; lj < L.tr_ey[b]; ++lj) {
+            int gj = L.tr_ej0[b] + lj;
+            if (L.nrowcov[gj] >= 4) return -2;
+            L.rowcov[4 * gj + L.nrowcov[gj]++] = b;
+        }
+    }
+    int mc = 1, mr = 1;
+    for (int v : L.ncolcov) mc = std::max(mc, v);
+    for (int v : L.nrowcov) mr = std::max(mr, v);
+    L.maxcov = mc * mr;
+    L.hs.resize(L.nsub);
+    L.ctot = L.ttot = L.gtot = L.ptot1 = L.otot = 0;
+    L.maxnpad = L.maxncell = L.maxnring = L.Wmax = 0;
+    for (int jw = 0; jw < q; ++jw)
+        for (int b = 0; b < p2; ++b)
+            for (int a = 0; a < p1; ++a) {
+                Sub& s = L.hs[(jw * p2 + b) * p1 + a];
+                s.a = a; s.b = b; s.jw = jw;
+                s.oi0 = oi0[a]; s.oi1 = oi1[a]; s.oj0 = oj0[b]; s.oj1 = oj1[b];
+                s.ei0 = L.tc_ei0[a]; s.ej0 = L.tr_ej0[b]; s.ex = L.tc_ex[a]; s.ey = L.tr_ey[b];
+                s.gx = p1 == 1 ? 0 : DD_GHOST; s.gys = gys[b]; s.gyn = gyn[b];
+                s.px = s.ex + 2 * s.gx; s.py = s.ey + s.gys + s.gyn;
+                s.s = L.wb[jw]; s.W = L.wb[jw + 1] - L.wb[jw];
+                if (s.W < 1) return -2;
+                s.ncell = s.ex * s.ey; s.npad = s.px * s.py; s.nring = s.npad - s.ncell;
+                s.coff = L.ctot; s.toff = L.ttot; s.goff = L.gtot; s.poff = 3 * L.ptot1; s.ooff = L.otot;
+                // keep every plane 16-byte aligned relative to 256-byte aligned array bases
+                L.ctot += 3LL * s.ncell; L.ctot = (L.ctot + 1) & ~1LL;
+                L.ttot += (long long)(s.W + 1) * 3 * s.ncell; L.ttot = (L.ttot + 1) & ~1LL;
+                L.gtot += (long long)s.W * 3 * s.nring; L.gtot = (L.gtot + 1) & ~1LL;
+                L.ptot1 += s.npad;
+                L.otot += s.W + 2;
+                L.maxnpad = std::max(L.maxnpad, s.npad); L.maxncell = std::max(L.maxncell, s.ncell);
+                L.maxnring = std::max(L.maxnring, s.nring); L.Wmax = std::max(L.Wmax, s.W);
+            }
+    L.CB = std::min(64, std::max(1, (3 * L.maxncell + NT_RED * 32 - 1) / (NT_RED * 32)));
+    return 0;
+}
+
+// device arrays of one layout, taken from the arena in a fixed order (dry run = size query)
+void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
+{
+    L.dsubs = ar.take<Sub>(L.nsub);
+    const size_t nit = (size_t)nlon * 6 + (size_t)nlat * 6 + 2 * L.p1 + 2 * L.p2 + L.q + 1;
+    L.itab = ar.take<int>(nit);
+    L.x = ar.take<double>(L.ctot); L.xbs = ar.take<double>(L.ctot); L.gx = ar.take<double>(L.ctot);
+    L.xfrozen = ar.take<double>(L.ctot); L.pred_end = ar.take<double>(L.ctot);
+    L.traj = ar.take<double>(L.ttot);
+    L.ghost = ar.take<double>(std::max<long long>(L.gtot, 2));
+    L.Zp = ar.take<double>(3 * L.ptot1); L.Za = ar.take<double>(3 * L.ptot1);
+    L.lamA = ar.take<double>(3 * L.ptot1); L.lamB = ar.take<double>(3 * L.ptot1);
+    L.A = ar.take<double>(3 * L.ptot1);
+    L.H1 = ar.take<double>(L.ptot1); L.HB = ar.take<double>(L.ptot1);
+    L.P = ar.take<double>(L.ptot1); L.UB = ar.take<double>(L.ptot1);
+    L.partial = ar.take<double>((size_t)L.nsub * L.CB * 5);
+    L.parts = ar.take<double>((size_t)L.nsub * 5);
+    L.Jev = ar.take<double>(L.nsub);
+    L.dmax = ar.take<double>(L.nsub);
+    L.okmask = ar.take<int>(L.nsub);
+    if (L.lbfgs) {
+        L.w = ar.take<double>(L.ctot); L.wt = ar.take<double>(L.ctot); L.g = ar.take<double>(L.ctot);
+        L.gn = ar.take<double>(L.ctot); L.d = ar.take<double>(L.ctot);
+        L.S = ar.take<double>((size_t)std::max(m, 1) * L.ctot); L.Y = ar.take<double>((size_t)std::max(m, 1) * L.ctot);
+        L.st.J = ar.take<double>(L.nsub); L.st.Jt = ar.take<double>(L.nsub); L.st.t = ar.take<double>(L.nsub);
+        L.st.gd = ar.take<double>(L.nsub);
+        L.st.nh = ar.take<int>(L.nsub); L.st.head = ar.take<int>(L.nsub); L.st.active = ar.take<int>(L.nsub);
+        L.st.ok = ar.take<int>(L.nsub); L.st.done = ar.take<int>(L.nsub); L.st.trial = ar.take<int>(L.nsub);
+        L.st.rho = ar.take<double>((size_t)L.nsub * std::max(m, 1));
+        L.st.gam = ar.take<double>((size_t)L.nsub * std::max(m, 1));
+        L.st.nactive = ar.take<int>(4);
+    }
+    fused_plan_arrays(L.fp, ar_take_bytes, &ar);
+}
+
+int upload_layout(dd4dvar_t h, Layout& L)
+{
+    const int nlon = h->grid.nlon, nlat = h->grid.nlat;
+    CU(cudaMemcpyAsync(L.dsubs, L.hs.data(), sizeof(Sub) * L.nsub, cudaMemcpyHostToDevice, h->stream));
+    std::vector<int> t;
+    auto put = [&](const std::vector<int>& v) { size_t o = t.size(); t.insert(t.end(), v.begin(), v.end()); return o; };
+    const size_t o_colown = put(L.colown), o_ncolcov = put(L.ncolcov), o_colcov = put(L.colcov);
+    const size_t o_rowown = put(L.rowown), o_nrowcov = put(L.nrowcov), o_rowcov = put(L.rowcov);
+    const size_t o_ei0 = put(L.tc_ei0), o_ex = put(L.tc_ex), o_ej0 = put(L.tr_ej0), o_ey = put(L.tr_ey);
+    const size_t o_wb = put(L.wb);
+    CU(cudaMemcpyAsync(L.itab, t.data(), sizeof(int) * t.size(), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    GeoP& g = L.geo;
+    g.nlon = nlon; g.nlat = nlat; g.p1 = L.p1; g.p2 = L.p2; g.q = L.q;
+    g.colown = L.itab + o_colown; g.ncolcov = L.itab + o_ncolcov; g.colcov = L.itab + o_colcov;
+    g.rowown = L.itab + o_rowown; g.nrowcov = L.itab + o_nrowcov; g.rowcov = L.itab + o_rowcov;
+    g.tc_ei0 = L.itab + o_ei0; g.tc_ex = L.itab + o_ex; g.tr_ej0 = L.itab + o_ej0; g.tr_ey = L.itab + o_ey;
+    g.wb = L.itab + o_wb;
+    // adjoint buffers: the ghost ring must be (and stays) zero
+    CU(cudaMemsetAsync(L.lamA, 0, sizeof(double) * 3 * L.ptot1, h->stream));
+    CU(cudaMemsetAsync(L.lamB, 0, sizeof(double) * 3 * L.ptot1, h->stream));
+    CU(cudaMemsetAsync(L.xfrozen, 0, sizeof(double) * L.ctot, h->stream));
+    CU(cudaMemsetAsync(L.pred_end, 0, sizeof(double) * L.ctot, h->stream));
+    CU(cudaMemsetAsync(L.x, 0, sizeof(double) * L.ctot, h->stream));
+    CU(cudaMemsetAsync(L.xbs, 0, sizeof(double) * L.ctot, h->stream));
+    if (L.lbfgs) {
+        CU(cudaMemsetAsync(L.w, 0, sizeof(double) * L.ctot, h->stream));
+        CU(cudaMemsetAsync(L.st.nh, 0, sizeof(int) * L.nsub, h->stream));
+        CU(cudaMemsetAsync(L.st.head, 0, sizeof(int) * L.nsub, h->stream));
+        CU(cudaMemsetAsync(L.st.done, 0, sizeof(int) * L.nsub, h->stream));
+    }
+    return 0;
+}
+
+// ---- sweeps (generic path) -------------------------------------------------------------
+dim3 pad_grid(const Layout& L) { return dim3((L.maxnpad + NT_GK - 1) / NT_GK, L.nsub); }
+dim3 cell_grid(const Layout& L) { return dim3((L.maxncell + NT_GK - 1) / NT_GK, L.nsub); }
+
+void forward_generic(dd4dvar_t h, Layout& L, const int* mask)
+{
+    // level 0 of the store = the control
+    LAUNCH(gk_store_control, cell_grid(L), NT_GK, L.dsubs, mask, L.x, L.traj);
+    for (int n = 0; n < L.Wmax; ++n) {
+        LAUNCH(gk_fill_pad, pad_grid(L), NT_GK, L.dsubs, mask, n, L.traj, L.ghost, L.Zp);
+        LAUNCH(gk_stageA, pad_grid(L), NT_GK, L.dsubs, mask, n, h->mp, L.Zp, L.Za);
+        LAUNCH(gk_stageH, pad_grid(L), NT_GK, L.dsubs, mask, n, h->mp, L.Za, L.H1);
+        LAUNCH(gk_stageUV, pad_grid(L), NT_GK, L.dsubs, mask, n, h->mp, L.Za, L.H1, L.traj);
+    }
+}
+void cost_generic(dd4dvar_t h, Layout& L, const int* mask, double* Jout)
+{
+    LAUNCH(gk_cost_partial<NT_RED>, dim3(L.CB, L.nsub), NT_RED, L.dsubs, mask, L.geo, h->cp, L.x, L.xbs,
+           L.xfrozen, L.pred_end, L.traj, L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c,
+           L.partial);
+    LAUNCH(gk_cost_final, (L.nsub + 127) / 128, 128, L.nsub, mask, L.CB, L.partial, L.parts, Jout);
+}
+void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
+{
+    double* buf[2] = { L.lamA, L.lamB };
+    LAUNCH(gk_adj_init, cell_grid(L), NT_GK, L.dsubs, mask, L.Wmax, L.q, L.p1 * L.p2, h->cp, L.traj,
+           L.xfrozen, L.lamA, L.lamB);
+    for (int n = L.Wmax; n >= 0; --n) {
+        double* cur = buf[(L.Wmax - n) & 1];
+        double* nxt = buf[(L.Wmax - n + 1) & 1];
+        if (L.have_obs)
+            LAUNCH(gk_obs_force, dim3(4, L.nsub), NT_GK, L.dsubs, mask, n, L.obs_start, L.obs_idx, L.obs_y,
+                   L.obs_c, L.traj, cur);
+        if (n > 0) {
+            LAUNCH(gk_fill_pad, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, L.traj, L.ghost, L.Zp);
+            LAUNCH(gk_stageA, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Zp, L.Za);
+            LAUNCH(gk_adjHB, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Za, cur, L.traj, L.HB, L.P, L.UB);
+            LAUNCH(gk_adjA, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Za, cur, L.HB, L.P, L.UB, L.A);
+            LAUNCH(gk_adjL0, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Zp, L.A, nxt);
+        }
+    }
+    LAUNCH(gk_grad_final, cell_grid(L), NT_GK, L.dsubs, mask, L.geo, h->cp, L.x, L.xbs, L.xfrozen,
+           L.pred_end, buf[L.Wmax & 1], L.gx, gw);
+}
+
+// one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
+void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
+{
+    if (L.path == 2) {
+        fused_sweep(h->stream, &h->launches, L.fp, L.dsubs, L.nsub, mask, h->mp, h->cp, L.geo, L.x, L.xbs,
+                    L.xfrozen, L.pred_end, L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx,
+                    L.obs_y, L.obs_c, L.parts, Jout, with_adjoint, L.gx, gw);
+        return;
+    }
+    forward_generic(h, L, mask);
+    cost_generic(h, L, mask, Jout);
+    if (with_adjoint) adjoint_generic(h, L, mask, gw);
+}
+void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
+{
+    if (L.path == 2) {
+        fused_adjoint(h->stream, &h->launches, L.fp, L.dsubs, L.nsub, mask, h->mp, h->cp, L.geo, L.x, L.xbs,
+                      L.xfrozen, L.pred_end, L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx,
+                      L.obs_y, L.obs_c, L.gx, gw);
+        return;
+    }
+    adjoint_generic(h, L, mask, gw);
+}
+
+// Alg 1 l.465: this iteration's results become the next one's frozen data
+void exchange(dd4dvar_t h, Layout& L)
+{
+    LAUNCH(xk_freeze<NT_RED>, L.nsub, NT_RED, L.dsubs, L.geo, L.traj, L.x, L.xfrozen, L.pred_end, L.dmax);
+    if (L.maxnring > 0)
+        LAUNCH(xk_ghost_fill, dim3((L.maxnring + 127) / 128, L.nsub, std::min(L.Wmax, 8)), 128, L.dsubs, L.geo,
+               L.traj, L.ghost);
+}
+
+int sync_check(dd4dvar_t h)
+{
+    CU(cudaStreamSynchronize(h->stream));
+    CU(cudaGetLastError());
+    return 0;
+}
+
+// J of eq (6) at a global state already in G.x
+int global_cost(dd4dvar_t h, double* out)
+{
+    sweep(h, h->G, false, nullptr, h->G.Jev, nullptr);
+    CU(cudaMemcpyAsync(out, h->G.Jev, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    return sync_check(h);
+}
+
+size_t plan_all(dd4dvar_t h, char* base)
+{
+    Arena ar; ar.base = base;
+    h->d_tab = ar.take<double>(6 * (size_t)h->grid.nlat);
+    plan_layout(h->G, ar, h->grid.nlon, h->grid.nlat, h->opt.lbfgs_m);
+    plan_layout(h->L, ar, h->grid.nlon, h->grid.nlat, h->opt.lbfgs_m);
+    return ar.off + 256;
+}
+
+}  // namespace
+
+// =============================================================================== C-ABI ====
+extern "C" {
+
+int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const dd4dvar_window* window,
+                   const dd4dvar_opts* opts, void* cuda_stream, dd4dvar_t* out)
+{
+    if (!grid || !decomp || !window || !out) return -1;
+    *out = nullptr;
+    if (grid->nlon < 3 || grid->nlat < 2 || window->nsteps < 1 || !(grid->radius > 0)) return -1;
+    dd4dvar_s* h = new dd4dvar_s();
+    h->grid = *grid; h->dec = *decomp; h->win = *window;
+    if (opts) h->opt = *opts;
+    else { h->opt.lbfgs_m = 5; h->opt.n_inner = 5; h->opt.max_backtrack = 20; h->opt.armijo_c1 = 1e-4; h->opt.path = 0; }
+    if (h->opt.lbfgs_m < 0 || h->opt.lbfgs_m > 32 || h->opt.n_inner < 0 || h->opt.max_backtrack < 0) { delete h; return -1; }
+    h->stream = (cudaStream_t)cuda_stream;
+    const int nlon = grid->nlon, nlat = grid->nlat;
+    // O1 row tables (eq (60)-(62) l.945-954; cell-centred rows R2; clamped metric R3), dt folded in
+    const double PI = 3.14159265358979323846;
+    const double dlam = 2.0 * PI / nlon, dth = PI / nlat, dt = window->dt, a = grid->radius;
+    std::vector<double> mc(nlat);
+    h->h_tab.assign(6 * (size_t)nlat, 0.0);
+    double* dtcz = &h->h_tab[0]; double* gdtcz = &h->h_tab[nlat]; double* dtf = &h->h_tab[2 * nlat];
+    double* dtt = &h->h_tab[3 * nlat]; double* rp = &h->h_tab[4 * nlat]; double* rm = &h->h_tab[5 * nlat];
+    for (int j = 0; j < nlat; ++j) {
+        const double th = -0.5 * PI + (j + 0.5) * dth, c = cos(th);
+        mc[j] = c > grid->cos_clamp ? c : grid->cos_clamp;
+        const double cz = 1.0 / (2.0 * a * dlam * mc[j]);
+        dtcz[j] = dt * cz; gdtcz[j] = grid->gravity * dt * cz;
+        dtf[j] = dt * 2.0 * grid->omega * sin(th);
+        dtt[j] = dt * sin(th) / (a * mc[j]);
+    }
+    for (int j = 0; j < nlat; ++j) {
+        rp[j] = (j + 1 < nlat ? mc[j + 1] : mc[j]) / mc[j];
+        rm[j] = (j > 0 ? mc[j - 1] : mc[j]) / mc[j];
+    }
+    const double cm = 1.0 / (2.0 * a * dth);
+    h->mp.nlon = nlon; h->mp.nlat = nlat; h->mp.kap = grid->diffusion;
+    h->mp.dtcm = dt * cm; h->mp.gdtcm = grid->gravity * dt * cm;
+    h->cp.mu = decomp->mu; h->cp.lambda = decomp->lambda;
+    for (int f = 0; f < 3; ++f) { h->cp.ib[f] = 1.0; h->cp.sb[f] = 1.0; }
+    int rc = build_layout(h->G, nlon, nlat, window->nsteps, 1, 1, 1, 0);
+    if (!rc) rc = build_layout(h->L, nlon, nlat, window->nsteps, decomp->p_lon, decomp->p_lat, decomp->q_time,
+                               decomp->overlap);
+    if (rc) { delete h; return rc; }
+    h->G.lbfgs = false; h->L.lbfgs = true;
+    h->G.path = 1;
+    const bool fits = fused_fits(h->L.hs.data(), h->L.nsub);
+    if (h->opt.path == 2 && !fits) { delete h; return -2; }
+    h->L.path = (h->opt.path == 1 || !fits) ? 1 : 2;
+    fused_plan_init(h->G.fp, nullptr, 0, h->opt.lbfgs_m);
+    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, h->opt.lbfgs_m);
+    h->ws_bytes = plan_all(h, nullptr);
+    *out = h;
+    return 0;
+}
+
+size_t dd4dvar_workspace_bytes(dd4dvar_t h) { return h ? h->ws_bytes : 0; }
+
+int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
+{
+    if (!h || !d_buf) return fail(h, -1, "set_workspace: null argument");
+    if (bytes < h->ws_bytes) return fail(h, -1, "set_workspace: buffer smaller than dd4dvar_workspace_bytes");
+    if (((uintptr_t)d_buf & 255) != 0) return fail(h, -1, "set_workspace: buffer not 256-byte aligned");
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    h->ws = d_buf;
+    plan_all(h, (char*)d_buf);
+    const int nlat = h->grid.nlat;
+    CU(cudaMemcpyAsync(h->d_tab, h->h_tab.data(), sizeof(double) * 6 * nlat, cudaMemcpyHostToDevice, h->stream));
+    h->mp.dtcz = h->d_tab; h->mp.gdtcz = h->d_tab + nlat; h->mp.dtf = h->d_tab + 2 * nlat;
+    h->mp.dtt = h->d_tab + 3 * nlat; h->mp.rp = h->d_tab + 4 * nlat; h->mp.rm = h->d_tab + 5 * nlat;
+    int rc = upload_layout(h, h->G);
+    if (rc) return rc;
+    rc = upload_layout(h, h->L);
+    if (rc) return rc;
+    rc = fused_setup(h->stream, h->L.fp, h->L.dsubs);
+    if (rc) return fail(h, -4, "fused kernel setup failed (shared-memory opt-in)");
+    h->have_ws = true; h->have_bg = false; h->G.have_obs = h->L.have_obs = false;
+    return sync_check(h);
+}
+
+int dd4dvar_set_background(dd4dvar_t h, const double* d_xb, const double h_sigma_b[3])
+{
+    if (!h || !d_xb || !h_sigma_b) return fail(h, -1, "set_background: null argument");
+    if (!h->have_ws) return fail(h, -3, "set_background before set_workspace");
+    for (int f = 0; f < 3; ++f) {
+        if (!(h_sigma_b[f] > 0)) return fail(h, -1, "set_background: sigma_b must be positive");
+        h->cp.sb[f] = h_sigma_b[f]; h->cp.ib[f] = 1.0 / (h_sigma_b[f] * h_sigma_b[f]);
+    }
+    Layout& G = h->G; Layout& L = h->L;
+    const size_t n3 = 3 * (size_t)h->grid.nlon * h->grid.nlat;
+    CU(cudaMemcpyAsync(G.xbs, d_xb, sizeof(double) * n3, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaMemcpyAsync(G.x, d_xb, sizeof(double) * n3, cudaMemcpyDeviceToDevice, h->stream));
+    // Alg 1 l.452: u^b = M(u_0^b)
+    forward_generic(h, G, nullptr);
+    // l.455: u_ji^0 = u_ji^b; local stores = restricted background trajectory
+    for (int lev = 0; lev <= h->win.nsteps; ++lev)
+        LAUNCH(xk_restrict_level, cell_grid(L), NT_GK, L.dsubs, h->grid.nlon, h->grid.nlat, lev,
+               G.traj + (size_t)lev * n3, L.traj, L.xbs, L.x);
+    CU(cudaMemsetAsync(L.w, 0, sizeof(double) * L.ctot, h->stream));
+    exchange(h, L);
+    h->have_bg = true;
+    return sync_check(h);
+}
+
+size_t dd4dvar_obs_workspace_bytes(dd4dvar_t h, long long n_obs_total)
+{
+    if (!h || n_obs_total < 0) return 0;
+    const size_t per = 4 + 8 + 8;
+    size_t nb = (size_t)n_obs_total * (1 + 2 * (size_t)h->L.maxcov);
+    return nb * per + (size_t)(h->G.otot + h->L.otot + 8) * 8 + 4096;
+}
+
+static int bin_observations(dd4dvar_t h, Layout& L, int n_times, const int* levels, const long long* offs,
+                            const int* idx, const double* val, Arena& ar, bool weights)
+{
+    const int nlon = h->grid.nlon, nlat = h->grid.nlat;
+    const long long n1 = (long long)nlon * nlat;
+    std::vector<long long> start(L.otot + 1, 0);
+    // Def 8 l.239: restriction of H^(k) to Delta_j x Omega_i = the observations inside it
+    auto visit = [&](auto&& fn) {
+        for (int t = 0; t < n_times; ++t) {
+            const int lev = levels[t];
+            for (long long qq = offs[t]; qq < offs[t + 1]; ++qq) {
+                const int f = (int)(idx[qq] / n1); const long long c = idx[qq] % n1;
+                const int gj = (int)(c / nlon), gi = (int)(c % nlon);
+                int ntime = 0;
+                for (int jw = 0; jw < L.q; ++jw) if (lev >= L.wb[jw] && lev <= L.wb[jw + 1]) ++ntime;
+                for (int jw = 0; jw < L.q; ++jw) {
+                    if (lev < L.wb[jw] || lev > L.wb[jw + 1]) continue;
+                    for (int cb = 0; cb < L.nrowcov[gj]; ++cb)
+                        for (int ca = 0; ca < L.ncolcov[gi]; ++ca) {
+                            const int k = (jw * L.p2 + L.rowcov[4 * gj + cb]) * L.p1 + L.colcov[4 * gi + ca];
+                            const Sub& s = L.hs[k];
+                            const int li = imod(gi - s.ei0, nlon), lj = gj - s.ej0;
+                            const double wt = weights ? 1.0 / (double)(L.ncolcov[gi] * L.nrowcov[gj]) / (double)ntime : 1.0;
+                            fn(s.ooff + (lev - s.s), f * s.ncell + lj * s.ex + li, val[qq], wt, f);
+                        }
+                }
+            }
+        }
+    };
+    visit([&](long long bin, int, double, double, int) { ++start[bin + 1]; });
+    for (long long b = 0; b < L.otot; ++b) start[b + 1] += start[b];
+    const long long nb = start[L.otot];
+    std::vector<long long> fill(start.begin(), start.end() - 1);
+    std::vector<int> oi(nb + 1); std::vector<double> oy(nb + 1), oc(nb + 1);
+    visit([&](long long bin, int lidx, double y, double wt, int f) {
+        const long long p = fill[bin]++;
+        oi[p] = lidx; oy[p] = y; oc[p] = h->cp.lambda * wt / (h->sig_o[f] * h->sig_o[f]);
+    });
+    L.obs_start = ar.take<long long>(L.otot + 1);
+    L.obs_idx = ar.take<int>(nb + 1); L.obs_y = ar.take<double>(nb + 1); L.obs_c = ar.take<double>(nb + 1);
+    if (ar.off > ar.cap) return fail(h, -1, "set_observations: observation workspace too small");
+    CU(cudaMemcpyAsync(L.obs_start, start.data(), sizeof(long long) * (L.otot + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(L.obs_idx, oi.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(L.obs_y, oy.data(), sizeof(double) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(L.obs_c, oc.data(), sizeof(double) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    L.have_obs = true;
+    return 0;
+}
+
+int dd4dvar_set_observations(dd4dvar_t h, int n_times, const int* h_levels, const long long* h_offsets,
+                             const int* d_index, const double* d_value, const double h_sigma_o[3],
+                             void* d_obs_ws, size_t obs_ws_bytes)
+{
+    if (!h || n_times < 0 || !h_sigma_o) return fail(h, -1, "set_observations: bad argument");
+    if (!h->have_ws) return fail(h, -3, "set_observations before set_workspace");
+    if (n_times > 0 && (!h_levels || !h_offsets || !d_index || !d_value || !d_obs_ws))
+        return fail(h, -1, "set_observations: null argument");
+    for (int f = 0; f < 3; ++f) {
+        if (!(h_sigma_o[f] > 0)) return fail(h, -1, "set_observations: sigma_o must be positive");
+        h->sig_o[f] = h_sigma_o[f];
+    }
+    const long long tot = n_times ? h_offsets[n_times] : 0;
+    if (n_times && obs_ws_bytes < dd4dvar_obs_workspace_bytes(h, tot))
+        return fail(h, -1, "set_observations: observation workspace too small");
+    std::vector<int> idx(tot + 1); std::vector<double> val(tot + 1);
+    if (tot) {
+        CU(cudaMemcpyAsync(idx.data(), d_index, sizeof(int) * tot, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(val.data(), d_value, sizeof(double) * tot, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    const long long n3 = 3LL * h->grid.nlon * h->grid.nlat;
+    for (int t = 0; t < n_times; ++t) {
+        if (h_levels[t] < 0 || h_levels[t] > h->win.nsteps || (t && h_levels[t] <= h_levels[t - 1]))
+            return fail(h, -1, "set_observations: levels must be strictly ascending inside [0, nsteps]");
+        if (h_offsets[t + 1] < h_offsets[t]) return fail(h, -1, "set_observations: offsets must ascend");
+        for (long long q = h_offsets[t]; q < h_offsets[t + 1]; ++q) {
+            if (idx[q] < 0 || idx[q] >= n3) return fail(h, -1, "set_observations: index out of range");
+            if (q > h_offsets[t] && idx[q] <= idx[q - 1])
+                return fail(h, -1, "set_observations: indices must be strictly ascending inside a level");
+        }
+    }
+    Arena ar; ar.base = (char*)d_obs_ws; ar.cap = obs_ws_bytes;
+    int rc = 0;
+    if (n_times == 0) { h->G.have_obs = h->L.have_obs = false; return 0; }
+    rc = bin_observations(h, h->G, n_times, h_levels, h_offsets, idx.data(), val.data(), ar, false);
+    if (!rc) rc = bin_observations(h, h->L, n_times, h_levels, h_offsets, idx.data(), val.data(), ar, true);
+    return rc;
+}
+
+int dd4dvar_eval_global(dd4dvar_t h, const double* d_x0, double* h_cost, double* d_grad)
+{
+    if (!h || !d_x0 || !h_cost) return fail(h, -1, "eval_global: null argument");
+    if (!h->have_bg) return fail(h, -3, "eval_global before set_background");
+    Layout& G = h->G;
+    const size_t n3 = 3 * (size_t)h->grid.nlon * h->grid.nlat;
+    CU(cudaMemcpyAsync(G.x, d_x0, sizeof(double) * n3, cudaMemcpyDeviceToDevice, h->stream));
+    sweep(h, G, d_grad != nullptr, nullptr, G.Jev, nullptr);
+    CU(cudaMemcpyAsync(h_cost, G.Jev, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    if (d_grad) CU(cudaMemcpyAsync(d_grad, G.gx, sizeof(double) * n3, cudaMemcpyDeviceToDevice, h->stream));
+    int rc = sync_check(h);
+    if (rc) return rc;
+    if (!isfinite(*h_cost)) return fail(h, -5, "eval_global: non-finite cost");
+    return 0;
+}
+
+int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, double* h_parts, double* d_grads)
+{
+    if (!h || !d_controls || !h_costs) return fail(h, -1, "eval_local: null argument");
+    if (!h->have_bg) return fail(h, -3, "eval_local before set_background");
+    Layout& L = h->L;
+    CU(cudaMemcpyAsync(L.x, d_controls, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
+    sweep(h, L, d_grads != nullptr, nullptr, L.Jev, nullptr);
+    CU(cudaMemcpyAsync(h_costs, L.Jev, sizeof(double) * L.nsub, cudaMemcpyDeviceToHost, h->stream));
+    if (h_parts) CU(cudaMemcpyAsync(h_parts, L.parts, sizeof(double) * 5 * L.nsub, cudaMemcpyDeviceToHost, h->stream));
+    if (d_grads) CU(cudaMemcpyAsync(d_grads, L.gx, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
+    int rc = sync_check(h);
+    if (rc) return rc;
+    for (int k = 0; k < L.nsub; ++k)
+        if (!isfinite(h_costs[k])) return fail(h, -5, "eval_local: non-finite cost");
+    return 0;
+}
+
+int dd4dvar_sweep_async(dd4dvar_t h, int with_adjoint)
+{
+    if (!h) return -1;
+    if (!h->have_bg) return fail(h, -3, "sweep_async before set_background");
+    sweep(h, h->L, with_adjoint != 0, nullptr, h->L.Jev, nullptr);
+    return 0;
+}
+
+int dd4dvar_get_controls(dd4dvar_t h, double* d_controls)
+{
+    if (!h || !d_controls) return fail(h, -1, "get_controls: null argument");
+    if (!h->have_bg) return fail(h, -3, "get_controls before set_background");
+    CU(cudaMemcpyAsync(d_controls, h->L.xfrozen, sizeof(double) * h->L.ctot, cudaMemcpyDeviceToDevice, h->stream));
+    return sync_check(h);
+}
+
+int dd4dvar_get_trajectory(dd4dvar_t h, int level, double* d_out)
+{
+    if (!h || !d_out || level < 0 || level > h->win.nsteps) return fail(h, -1, "get_trajectory: bad argument");
+    if (!h->have_bg) return fail(h, -3, "get_trajectory before set_background");
+    const int n1 = h->grid.nlon * h->grid.nlat;
+    LAUNCH(xk_gather, (n1 + 255) / 256, 256, h->L.dsubs, h->L.geo, 0, level, h->L.traj, d_out);
+    return sync_check(h);
+}
+
+int dd4dvar_get_local_trajectory(dd4dvar_t h, int sub, double* d_out)
+{
+    if (!h || !d_out || sub < 0 || sub >= h->L.nsub) return fail(h, -1, "get_local_trajectory: bad argument");
+    if (!h->have_bg) return fail(h, -3, "get_local_trajectory before set_background");
+    const Sub& s = h->L.hs[sub];
+    CU(cudaMemcpyAsync(d_out, h->L.traj + s.toff, sizeof(double) * (size_t)(s.W + 1) * 3 * s.ncell,
+                       cudaMemcpyDeviceToDevice, h->stream));
+    return sync_check(h);
+}
+
+int dd4dvar_forecast(dd4dvar_t h, const double* d_x0, int n_levels, const int* h_levels, double* d_out)
+{
+    if (!h || !d_x0 || n_levels < 0 || (n_levels && (!h_levels || !d_out))) return fail(h, -1, "forecast: bad argument");
+    if (!h->have_ws) return fail(h, -3, "forecast before set_workspace");
+    Layout& G = h->G;
+    const size_t n3 = 3 * (size_t)h->grid.nlon * h->grid.nlat;
+    for (int q = 0; q < n_levels; ++q)
+        if (h_levels[q] < 0 || h_levels[q] > h->win.nsteps || (q && h_levels[q] < h_levels[q - 1]))
+            return fail(h, -1, "forecast: levels must ascend inside [0, nsteps]");
+    CU(cudaMemcpyAsync(G.x, d_x0, sizeof(double) * n3, cudaMemcpyDeviceToDevice, h->stream));
+    forward_generic(h, G, nullptr);
+    for (int q = 0; q < n_levels; ++q)
+        CU(cudaMemcpyAsync(d_out + (size_t)q * n3, G.traj + (size_t)h_levels[q] * n3, sizeof(double) * n3,
+                           cudaMemcpyDeviceToDevice, h->stream));
+    return sync_check(h);
+}
+
+// Algorithm 1 l.443-472 (additive outer iteration R16, fixed iteration count R17)
+int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_history)
+{
+    if (!h || outer_iters < 0 || !d_analysis || !h_history) return fail(h, -1, "run: bad argument");
+    if (!h->have_bg) return fail(h, -3, "run before set_background");
+    Layout& L = h->L; Layout& G = h->G;
+    const int n1 = h->grid.nlon * h->grid.nlat;
+    const int nsub = L.nsub;
+    LbfgsP lp; lp.m = h->opt.lbfgs_m; lp.max_bt = h->opt.max_backtrack; lp.c1 = h->opt.armijo_c1; lp.ctot = L.ctot;
+    h->h_tmp.resize(std::max(nsub, 8));
+    int rc;
+    auto sumJ = [&](const double* dJ, double* out) -> int {
+        CU(cudaMemcpyAsync(h->h_tmp.data(), dJ, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
+        int r = sync_check(h); if (r) return r;
+        long double sacc = 0; for (int k = 0; k < nsub; ++k) sacc += h->h_tmp[k];
+        *out = (double)sacc; return 0;
+    };
+    auto gather_and_cost = [&](double* out) -> int {
+        LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, G.x);
+        return global_cost(h, out);
+    };
+    if ((rc = gather_and_cost(&h_history[0]))) return rc;
+    h_history[1] = 0.0; h_history[2] = 0.0;
+    const dim3 vgrid(std::min(64, (3 * L.maxncell + 255) / 256), nsub);
+    if (outer_iters == 0) {
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+               (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        sweep(h, L, false, nullptr, L.st.J, nullptr);
+        if ((rc = sumJ(L.st.J, &h_history[1]))) return rc;
+    }
+    for (int l = 1; l <= outer_iters; ++l) {
+        // local functional changed: clear the history (R10), evaluate J_ji and its gradient at w
+        CU(cudaMemsetAsync(L.st.nh, 0, sizeof(int) * nsub, h->stream));
+        CU(cudaMemsetAsync(L.st.head, 0, sizeof(int) * nsub, h->stream));
+        CU(cudaMemsetAsync(L.st.done, 0, sizeof(int) * nsub, h->stream));
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+               (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        sweep(h, L, true, nullptr, L.st.J, L.g);
+        if (l == 1 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
+        for (int it = 0; it < h->opt.n_inner; ++it) {
+            LAUNCH(lk_direction<NT_LB>, nsub, NT_LB, L.dsubs, lp, L.st, L.g, L.S, L.Y, L.d);
+            for (int b = 0; b <= lp.max_bt; ++b) {
+                CU(cudaMemsetAsync(L.st.nactive, 0, sizeof(int), h->stream));
+                LAUNCH(lk_trial, vgrid, 256, L.dsubs, L.st.active, h->cp, L.st.t, L.w, L.d, L.xbs, L.wt, L.x);
+                sweep(h, L, false, L.st.active, L.st.Jt, nullptr);
+                LAUNCH(lk_lscheck, (nsub + 127) / 128, 128, nsub, lp, L.st);
+                int nact = 0;
+                CU(cudaMemcpyAsync(&nact, L.st.nactive, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                if ((rc = sync_check(h))) return rc;
+                if (nact == 0) break;
+            }
+            // gradient at the accepted points (their trajectories are still in the store)
+            adjoint_only(h, L, L.st.ok, L.gn);
+            LAUNCH(lk_update<NT_LB>, nsub, NT_LB, L.dsubs, lp, L.st, L.w, L.wt, L.g, L.gn, L.S, L.Y);
+        }
+        // one more forward sweep so that the stored trajectory belongs to the accepted iterate
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+               (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        sweep(h, L, false, nullptr, L.Jev, nullptr);
+        if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
+        exchange(h, L);
+        CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
+        if ((rc = sync_check(h))) return rc;
+        double dl = 0; for (int k = 0; k < nsub; ++k) dl = std::max(dl, h->h_tmp[k]);
+        h_history[3 * l + 2] = dl;
+        if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
+        if (!isfinite(h_history[3 * l]) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run: non-finite cost");
+    }
+    LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
+    return sync_check(h);
+}
+
+int dd4dvar_num_subdomains(dd4dvar_t h) { return h ? h->L.nsub : -1; }
+
+int dd4dvar_subdomain_info(dd4dvar_t h, int sub, int out[16])
+{
+    if (!h || !out || sub < 0 || sub >= h->L.nsub) return fail(h, -1, "subdomain_info: bad argument");
+    const Sub& s = h->L.hs[sub];
+    const int v[16] = { s.a, s.b, s.jw, s.oi0, s.oi1, s.oj0, s.oj1, s.ei0, s.ej0, s.ex, s.ey, s.gx, s.gys, s.gyn, s.s, s.s + s.W };
+    memcpy(out, v, sizeof(v));
+    return 0;
+}
+
+long long dd4dvar_control_offset(dd4dvar_t h, int sub)
+{
+    if (!h || sub < 0 || sub > h->L.nsub) return -1;
+    return sub == h->L.nsub ? h->L.ctot : h->L.hs[sub].coff;
+}
+
+int dd4dvar_active_path(dd4dvar_t h) { return h ? h->L.path : -1; }
+long long dd4dvar_launch_count(dd4dvar_t h) { return h ? h->launches : -1; }
+const char* dd4dvar_last_error(dd4dvar_t h) { return h ? h->err.c_str() : "null handle"; }
+void dd4dvar_destroy(dd4dvar_t h) { delete h; }
+
+}  // extern "C"

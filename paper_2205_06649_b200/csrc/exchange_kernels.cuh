@@ -1,0 +1,122 @@
+// exchange_kernels.cuh -- Algorithm 1 l.465 "Exchange u_ji between adjacent subdomains" and
+// l.470 "Gather", all inside device memory: refresh of the frozen ghost-ring trajectories,
+// predecessor end states and frozen controls, the step norm (l.466), the restriction of a
+// global state to the tiles (Def 4 l.164-170) and the weighted extension-sum (eq (12)-(13)
+// l.194-201).
+#pragma once
+#include "common.cuh"
+
+// ghost[k][n][f][r] <- traj[owner][n][f][cell]: every ghost cell takes the value of the tile
+// that OWNS it, same window, all levels that start a step (R14).
+__global__ void xk_ghost_fill(const Sub* __restrict__ subs, GeoP geo, const double* __restrict__ traj,
+                              double* __restrict__ ghost)
+{
+    const int k = blockIdx.y;
+    const Sub s = subs[k];
+    const int rr = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rr >= s.nring) return;
+    // ring index -> padded coordinates (inverse of the enumeration in gk_fill_pad)
+    int i, j;
+    const int nsouth = s.gys * s.px, nns = (s.gys + s.gyn) * s.px;
+    if (rr < nsouth) { j = rr / s.px; i = rr - j * s.px; }
+    else if (rr < nns) { const int q = rr - nsouth; j = s.gys + s.ey + q / s.px; i = q % s.px; }
+    else {
+        const int q = rr - nns, w2 = 2 * s.gx;
+        const int lj = q / w2, t = q - lj * w2;
+        j = s.gys + lj; i = t < s.gx ? t : t + s.ex;
+    }
+    const int gi = imodd(s.ei0 - s.gx + i, geo.nlon), gj = s.ej0 - s.gys + j;
+    const Sub& so = subs[(s.jw * geo.p2 + geo.rowown[gj]) * geo.p1 + geo.colown[gi]];
+    const int li = imodd(gi - so.ei0, geo.nlon), lj = gj - so.ej0;
+    const long long c = (long long)lj * so.ex + li;
+    for (int n = blockIdx.z; n < s.W; n += gridDim.z) {
+        const double* t = traj + so.toff + (long long)n * DD_NF * so.ncell;
+        double* g = ghost + s.goff + (long long)n * DD_NF * s.nring;
+#pragma unroll
+        for (int f = 0; f < DD_NF; ++f) g[(long long)f * s.nring + rr] = t[(long long)f * so.ncell + c];
+    }
+}
+
+// pred_end[k] <- final state of the predecessor window on the same tile (eq (25c) case 2);
+// delta_k = ||x_k - xfrozen_k||_inf (l.466, l.704); xfrozen[k] <- x[k].
+template <int NT>
+__global__ void xk_freeze(const Sub* __restrict__ subs, GeoP geo, const double* __restrict__ traj,
+                          const double* __restrict__ x, double* __restrict__ xfrozen,
+                          double* __restrict__ pred_end, double* __restrict__ dmax)
+{
+    __shared__ double sh[32];
+    const int k = blockIdx.x;
+    const Sub s = subs[k];
+    const int n3 = DD_NF * s.ncell;
+    double mx = 0.0;
+    const double* tp = nullptr;
+    if (s.jw > 0) {
+        const Sub& sp = subs[k - geo.p1 * geo.p2];
+        tp = traj + sp.toff + (long long)sp.W * DD_NF * sp.ncell;
+    }
+    for (int q = threadIdx.x; q < n3; q += NT) {
+        const double xn = x[s.coff + q];
+        mx = fmax(mx, fabs(xn - xfrozen[s.coff + q]));
+        xfrozen[s.coff + q] = xn;
+        if (tp) pred_end[s.coff + q] = tp[q];
+    }
+    mx = block_max<NT>(mx, sh);
+    if (threadIdx.x == 0) dmax[k] = mx;
+}
+
+// traj[k][n] <- restriction of global level s_k + n (source = the undecomposed layout's store)
+__global__ void xk_restrict_level(const Sub* __restrict__ subs, int nlon, int nlat, int level,
+                                  const double* __restrict__ gstate, double* __restrict__ traj,
+                                  double* __restrict__ xbs, double* __restrict__ x)
+{
+    const int k = blockIdx.y;
+    const Sub s = subs[k];
+    if (level < s.s || level > s.s + s.W) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= s.ncell) return;
+    const int lj = c / s.ex, li = c - lj * s.ex;
+    const int gi = imodd(s.ei0 + li, nlon), gj = s.ej0 + lj;
+    double* t = traj + s.toff + (long long)(level - s.s) * DD_NF * s.ncell;
+#pragma unroll
+    for (int f = 0; f < DD_NF; ++f) {
+        const double v = gstate[((long long)f * nlat + gj) * nlon + gi];
+        t[(long long)f * s.ncell + c] = v;
+        if (level == s.s) { xbs[s.coff + (long long)f * s.ncell + c] = v; x[s.coff + (long long)f * s.ncell + c] = v; }
+    }
+}
+
+// out[f][gj][gi] = sum over the subdomains that hold (level, cell) of weight * value, in
+// ascending subdomain order; weight = 1/multiplicity (Def 4 generalised, R6).
+// mode 0: from the trajectory store at `level`; mode 1: analysis = window-0 frozen controls.
+__global__ void xk_gather(const Sub* __restrict__ subs, GeoP geo, int mode, int level,
+                          const double* __restrict__ src, double* __restrict__ out)
+{
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= geo.nlon * geo.nlat) return;
+    const int gj = g / geo.nlon, gi = g - gj * geo.nlon;
+    const int nc = geo.ncolcov[gi], nr = geo.nrowcov[gj];
+    int jw0 = 0, jw1 = 0, tm = 1;
+    if (mode == 0) {
+        jw0 = -1;
+        for (int jw = 0; jw < geo.q; ++jw)
+            if (level >= geo.wb[jw] && level <= geo.wb[jw + 1]) { if (jw0 < 0) jw0 = jw; jw1 = jw; }
+        tm = jw1 - jw0 + 1;
+    }
+    const double wt = 1.0 / (double)(nc * nr) / (double)tm;
+    const double wsp = 1.0 / (double)(nc * nr);
+    double acc[3] = { 0.0, 0.0, 0.0 };
+    for (int jw = jw0; jw <= jw1; ++jw)
+        for (int cb = 0; cb < nr; ++cb)
+            for (int ca = 0; ca < nc; ++ca) {
+                const Sub& s = subs[(jw * geo.p2 + geo.rowcov[4 * gj + cb]) * geo.p1 + geo.colcov[4 * gi + ca]];
+                const int li = imodd(gi - s.ei0, geo.nlon), lj = gj - s.ej0;
+                const long long c = (long long)lj * s.ex + li;
+                const double* p = mode == 0 ? src + s.toff + (long long)(level - s.s) * DD_NF * s.ncell
+                                            : src + s.coff;
+#pragma unroll
+                for (int f = 0; f < DD_NF; ++f)
+                    acc[f] += (mode == 0 ? wt : wsp) * p[(long long)f * s.ncell + c];
+            }
+#pragma unroll
+    for (int f = 0; f < DD_NF; ++f) out[((long long)f * geo.nlat + gj) * geo.nlon + gi] = acc[f];
+}

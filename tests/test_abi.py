@@ -1,0 +1,91 @@
+"""The C-ABI library loads and exports every symbol include/dd4dvar.h declares (no compute)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2205_06649_b200 import build
+    return ctypes.CDLL(build.build())
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "dd4dvar.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(dd4dvar_[a-z_]+)\s*\(", src)))
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = declared_symbols()
+    for n in ("dd4dvar_create", "dd4dvar_set_background", "dd4dvar_set_observations", "dd4dvar_run",
+              "dd4dvar_eval_local", "dd4dvar_eval_global"):
+        assert n in names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for n in declared_symbols():
+        assert hasattr(lib, n), n
+
+
+def test_binding_lists_the_same_symbols(lib):
+    from paper_2205_06649_b200 import binding
+    assert sorted(binding.EXPORTS) == declared_symbols()
+
+
+def test_create_rejects_bad_arguments_without_a_gpu(lib):
+    from paper_2205_06649_b200.binding import Grid, Decomp, Window, Opts
+    lib.dd4dvar_create.argtypes = [ctypes.c_void_p] * 6
+    h = ctypes.c_void_p()
+    g = Grid(36, 18, 6.371e6, 7.292e-5, 9.806, 0.64, 0.02)
+    w = Window(600.0, 16)
+    o = Opts(5, 5, 20, 1e-4, 0)
+    # more windows than steps, tile rows without room for the ghost ring: -2 (does not fit)
+    for d in (Decomp(2, 2, 17, 1, 1.0, 1.0), Decomp(2, 9, 2, 1, 1.0, 1.0)):
+        rc = lib.dd4dvar_create(ctypes.byref(g), ctypes.byref(d), ctypes.byref(w), ctypes.byref(o), None, ctypes.byref(h))
+        assert rc == -2 and not h.value
+    bad = Grid(2, 18, 6.371e6, 7.292e-5, 9.806, 0.64, 0.02)
+    d = Decomp(1, 1, 1, 0, 1.0, 1.0)
+    assert lib.dd4dvar_create(ctypes.byref(bad), ctypes.byref(d), ctypes.byref(w), ctypes.byref(o), None, ctypes.byref(h)) == -1
+    # a valid layout builds its geometry on the host and reports sizes without touching a device
+    d = Decomp(2, 2, 2, 1, 1.0, 1.0)
+    assert lib.dd4dvar_create(ctypes.byref(g), ctypes.byref(d), ctypes.byref(w), ctypes.byref(o), None, ctypes.byref(h)) == 0
+    lib.dd4dvar_num_subdomains.argtypes = [ctypes.c_void_p]
+    lib.dd4dvar_workspace_bytes.argtypes = [ctypes.c_void_p]
+    lib.dd4dvar_workspace_bytes.restype = ctypes.c_size_t
+    assert lib.dd4dvar_num_subdomains(h) == 8
+    assert lib.dd4dvar_workspace_bytes(h) > 0
+    out = (ctypes.c_int * 16)()
+    lib.dd4dvar_subdomain_info.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+    assert lib.dd4dvar_subdomain_info(h, 3, out) == 0
+    # tile (1,1) of window 0: owned 18..36 x 9..18, extended by 1 cell on interior sides (eq (70))
+    assert list(out)[:11] == [1, 1, 0, 18, 36, 9, 18, 17, 8, 20, 10]
+    lib.dd4dvar_destroy.argtypes = [ctypes.c_void_p]
+    lib.dd4dvar_destroy(h)
+
+
+def test_geometry_matches_oracle_on_ragged_layouts(lib):
+    from oracle import Oracle
+    from paper_2205_06649_b200.binding import Grid, Decomp, Window, Opts
+    lib.dd4dvar_create.argtypes = [ctypes.c_void_p] * 6
+    lib.dd4dvar_subdomain_info.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
+    lib.dd4dvar_num_subdomains.argtypes = [ctypes.c_void_p]
+    lib.dd4dvar_destroy.argtypes = [ctypes.c_void_p]
+    for (nlon, nlat, N, p1, p2, q, o) in [(36, 18, 16, 2, 2, 2, 1), (40, 23, 17, 3, 2, 3, 2), (36, 18, 16, 1, 1, 1, 0),
+                                          (48, 30, 10, 1, 3, 2, 2), (720, 360, 128, 16, 16, 8, 2)]:
+        h = ctypes.c_void_p()
+        g = Grid(nlon, nlat, 6.371e6, 7.292e-5, 9.806, 0.64, 0.02)
+        d = Decomp(p1, p2, q, o, 1.0, 1.0); w = Window(100.0, N); op = Opts(5, 5, 20, 1e-4, 0)
+        assert lib.dd4dvar_create(ctypes.byref(g), ctypes.byref(d), ctypes.byref(w), ctypes.byref(op), None, ctypes.byref(h)) == 0
+        orc = Oracle(nlon, nlat, 100.0, N, p1, p2, q, o)
+        assert lib.dd4dvar_num_subdomains(h) == orc.nsub
+        for k in range(orc.nsub):
+            out = (ctypes.c_int * 16)()
+            lib.dd4dvar_subdomain_info(h, k, out)
+            assert list(out) == [orc.subs[k][f] for f in ("a", "b", "jw", "oi0", "oi1", "oj0", "oj1", "ei0", "ej0",
+                                                           "ex", "ey", "gx", "gys", "gyn", "s", "e")], k
+        lib.dd4dvar_destroy(h)
