@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point.steps/s of the fused forward+adjoint gradient sweep (BASELINE.json metric).
+
+A "step" = one pass of the whole hot path (forward sweep + trajectory
+store, misfit / background / overlap terms, adjoint sweep) over every subdomain of the workload.
+Default workload: BASELINE.json configs[3], the 0.25 deg 1440x720 grid, 256 steps, 16x16x8
+decomposition, overlap 2 (the config the roofline target is quoted on).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+`--impl reference` times the CPU oracle (oracle/), as it stands, on the host cores on a bounded
+sample of the same workload.  N > 1: one process per GPU (torchrun), each rank runs an independent
+replica of the workload ("replicas only"): weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2205_06649_b200 import synth  # noqa: E402
+
+METRIC = "grid-point.steps/s of fused forward+adjoint gradient sweep"
+UNIT = "grid-point.steps/s"
+
+
+def peaks():
+    """Measured HBM copy bandwidth (GB/s) from MEASURED_PEAKS.json, else the guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes(subs, q_time, nobs_binned, with_gw=False):
+    """per sweep, forward and adjoint kernels separately.
+    subs: list of dicts from subdomain_info; nobs_binned: total binned observations."""
+    fwd = adj = 0
+    pts = 0
+    for s in subs:
+        nc = s["ex"] * s["ey"]
+        px = s["ex"] + 2 * s["gx"]; py = s["ey"] + s["gys"] + s["gyn"]
+        nring = px * py - nc
+        W = s["e"] - s["s"]
+        pts += nc * W
+        fixed_f = 24 * nc * 2            # control, u^b(s_j)
+        if s["jw"] > 0:
+            fixed_f += 24 * nc           # predecessor end state
+        if s["jw"] < q_time - 1:
+            fixed_f += 24 * nc           # successor control
+        fwd += fixed_f + 24 * W * nring + 24 * W * nc          # ghost read, trajectory write
+        fixed_a = 24 * nc * 3            # level W (end forcing), control + u^b (gradient terms)
+        if s["jw"] > 0:
+            fixed_a += 24 * nc
+        if s["jw"] < q_time - 1:
+            fixed_a += 24 * nc
+        adj += fixed_a + 24 * W * nring + 24 * W * nc + 24 * nc * (2 if with_gw else 1)
+    fwd += 20 * nobs_binned
+    adj += 20 * nobs_binned
+    return fwd, adj, pts
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill(); out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(cfg):
+    if cfg in synth.CONFIGS:
+        return synth.CONFIGS[cfg]
+    raise SystemExit(f"unknown config {cfg}")
+
+
+def oracle_sweep_sample(w, budget_pts=1.5e8):
+    """The oracle's gradient sweep on the first subdomains of the SAME workload (bounded sample)."""
+    from oracle import Oracle
+    o = Oracle.from_workload(w)
+    prob = synth.make_problem(w, o.forecast)
+    o.set_background(prob.xb, prob.sigma_b)
+    o.set_observations(prob.obs)
+    k1 = 0; pts = 0
+    while k1 < o.nsub and pts < budget_pts:
+        s = o.subs[k1]; pts += s["ex"] * s["ey"] * (s["e"] - s["s"]); k1 += 1
+    tot = sum(s["ex"] * s["ey"] * (s["e"] - s["s"]) for s in o.subs)
+    o.useful_ratio = w.nlon * w.nlat * w.nsteps / tot      # useful / processed point-steps
+    return o, k1
+
+
+def cpu_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    o, k1 = oracle_sweep_sample(w)
+    for _ in range(max(args.warmup, 0) and 1):
+        o.sweep_range(0, k1)
+    t0 = time.perf_counter(); pts = 0.0
+    for _ in range(args.steps):
+        p, _ = o.sweep_range(0, k1); pts += p
+    dt = time.perf_counter() - t0
+    val = o.useful_ratio * pts / dt
+    sample = (f"subdomains 0..{k1 - 1} of {o.nsub} ({int(pts / args.steps)} processed point-steps per step; "
+              f"value scaled by the workload's useful/processed ratio {o.useful_ratio:.4f})")
+    line = {"metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": w.name, "counted": "useful = nlon*nlat*nsteps per sweep"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic kernels, 2 fused kernels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    w = workload(args.config)
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2205_06649_b200.binding import DD4DVar
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the library has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- build the replica of the workload on this rank (seeded synthetic inputs)
+    g = DD4DVar.from_workload(w, path=args.path, device=f"cuda:{local_rank}")
+    prob = synth.make_problem(w, g.forecast)          # truth trajectory from the library's own model
+    g.set_background(prob.xb, prob.sigma_b)
+    g.set_observations(prob.obs)
+    nobs_binned = 0
+    lv = set(int(x) for x in prob.obs.levels)
+    n_per_level = int(prob.obs.offsets[1] - prob.obs.offsets[0]) if len(prob.obs.levels) else 0
+    # binned observation count: every observation lands in every (window, tile) that holds it
+    cell = prob.obs.index[:n_per_level] % (w.nlon * w.nlat)
+    gi = cell % w.nlon; gj = cell // w.nlon
+    colmult = np.zeros(w.nlon, dtype=np.int64); rowmult = np.zeros(w.nlat, dtype=np.int64)
+    seen_a, seen_b = set(), set()
+    for s in g.subs:
+        if s["jw"] == 0 and s["b"] == 0:
+            colmult[(s["ei0"] + np.arange(s["ex"])) % w.nlon] += 1
+        if s["jw"] == 0 and s["a"] == 0:
+            rowmult[s["ej0"] + np.arange(s["ey"])] += 1
+    per_level = int(np.sum(colmult[gi] * rowmult[gj]))
+    wins = sorted(set((s["s"], s["e"]) for s in g.subs))
+    for lev in lv:
+        nobs_binned += per_level * sum(1 for (s0, e0) in wins if s0 <= lev <= e0)
+    fwd_b, adj_b, pts = algorithmic_bytes(g.subs, w.q_time, nobs_binned)
+    useful = w.nlon * w.nlat * w.nsteps
+
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing: K gradient sweeps (inputs far larger than L2, no flush needed)
+    for _ in range(args.warmup):
+        g.sweep_async(1)
+    barrier()
+    l0 = g.launch_count
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    barrier()
+    ev[0].record(stream)
+    for _ in range(args.steps):
+        g.sweep_async(1)
+    ev[1].record(stream)
+    barrier()
+    ms = ev[0].elapsed_time(ev[1])
+    launches = g.launch_count - l0
+    clocks = sampler.stop() if sampler else None
+    # per-kernel split (forward+cost vs adjoint), same stream, same events
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t_f = t_a = 0.0
+    nsplit = max(3, min(args.steps, 10))
+    for _ in range(nsplit):
+        evs[0].record(stream); g.sweep_async(0); evs[1].record(stream); g.sweep_async(2); evs[2].record(stream)
+        torch.cuda.synchronize(dev)
+        t_f += evs[0].elapsed_time(evs[1]); t_a += evs[1].elapsed_time(evs[2])
+    t_f /= nsplit; t_a /= nsplit
+
+    # ---- end to end through the C-ABI with host buffers (pinned), copies inside the timed region
+    h_ctrl = g.get_controls().cpu().pin_memory()
+    h_grad = torch.empty_like(h_ctrl).pin_memory()
+    h_cost = np.zeros(g.nsub)
+    e2e_steps = max(3, min(args.steps, 5))
+    g.eval_local_host(h_ctrl, h_cost, h_grad)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        g.eval_local_host(h_ctrl, h_cost, h_grad)
+    torch.cuda.synchronize(dev)
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+
+    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms, e2e_s = float(tmax[0]), float(tmax[1])
+
+    if rank == 0:
+        ms_step = ms / args.steps
+        peak, peak_src = peaks()
+        fused = g.active_path == 2
+        if fused:
+            kern, kb, kt = "fk_adjoint (fused adjoint sweep, one launch per gradient sweep)", adj_b, t_a
+        else:
+            kern, kb, kt = "gradient sweep, all per-stage launches of the generic path", fwd_b + adj_b, ms_step
+        achieved = kb / (kt * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": world * useful / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "counted": "useful = nlon*nlat*nsteps per sweep",
+                       "processed_point_steps_per_sweep": pts, "processed_value": world * pts / (ms_step * 1e-3),
+                       "subdomains": g.nsub, "path": "fused" if fused else "generic",
+                       "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
+                       "parallelism": "replicas" if world > 1 else "single GPU"},
+            "clocks": clocks,
+            "e2e": {"value": world * useful / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.ctot * 8),
+                    "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": kern, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": kb, "kernel_ms": kt,
+                         "sweep_algorithmic_GBps": (fwd_b + adj_b) / (ms_step * 1e-3) / 1e9,
+                         "forward_ms": t_f, "adjoint_ms": t_a,
+                         "bytes_per_processed_point_step": (fwd_b + adj_b) / pts},
+        }
+        if not args.no_cpu_baseline and world >= 1:
+            t0 = time.perf_counter()
+            o, k1 = oracle_sweep_sample(w)
+            t1 = time.perf_counter()
+            p, _ = o.sweep_range(0, k1)
+            t2 = time.perf_counter()
+            line["cpu_baseline"] = {"value": o.useful_ratio * p / (t2 - t1), "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
+                                    "sample": f"gradient sweep of subdomains 0..{k1 - 1} of {o.nsub} "
+                                              f"({int(p)} processed point-steps, {t2 - t1:.1f} s; oracle setup {t1 - t0:.1f} s not timed)"}
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -126,9 +126,16 @@ int dd4dvar_eval_global(dd4dvar_t h, const double* d_x0, double* h_cost, double*
 int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, double* h_parts,
                        double* d_grads);
 
+/* The same evaluation end to end with HOST buffers: h_controls is copied to the device, the
+ * gradient sweep runs, costs and (if h_grads != NULL) gradients are copied back.  Pinned host
+ * memory makes the copies asynchronous with respect to the host but they are inside the call. */
+int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_costs, double* h_grads);
+
 /* Same evaluation, queued on the stream without host synchronisation or host output, at the
- * library's own current controls: used for timing the gradient sweep (bench.py). */
-int dd4dvar_sweep_async(dd4dvar_t h, int with_adjoint);
+ * library's own current controls: used for timing the gradient sweep (bench.py).
+ * mode 0: forward sweep + trajectory store + cost terms (a1-a3); 1: the whole gradient sweep
+ * (a1-a4); 2: adjoint sweep only (a4), on the trajectories the last forward sweep stored. */
+int dd4dvar_sweep_async(dd4dvar_t h, int mode);
 
 /* Copy the current local controls of all subdomains ("all subdomains" array, physical units). */
 int dd4dvar_get_controls(dd4dvar_t h, double* d_controls);

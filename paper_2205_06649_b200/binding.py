@@ -48,7 +48,7 @@ _lib = None
 EXPORTS = [
     "dd4dvar_create", "dd4dvar_workspace_bytes", "dd4dvar_set_workspace", "dd4dvar_set_background",
     "dd4dvar_obs_workspace_bytes", "dd4dvar_set_observations", "dd4dvar_run", "dd4dvar_eval_global",
-    "dd4dvar_eval_local", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
+    "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
     "dd4dvar_last_error", "dd4dvar_destroy",
@@ -76,6 +76,7 @@ def load_library():
     lib.dd4dvar_run.argtypes = [vp, C.c_int, dp, hd]
     lib.dd4dvar_eval_global.argtypes = [vp, dp, hd, dp]
     lib.dd4dvar_eval_local.argtypes = [vp, dp, hd, hd, dp]
+    lib.dd4dvar_eval_local_host.argtypes = [vp, C.c_void_p, hd, C.c_void_p]
     lib.dd4dvar_sweep_async.argtypes = [vp, C.c_int]
     lib.dd4dvar_get_controls.argtypes = [vp, dp]
     lib.dd4dvar_get_trajectory.argtypes = [vp, C.c_int, dp]
@@ -237,6 +238,14 @@ class DD4DVar:
         self._check("dd4dvar_eval_local", rc)
         return costs, parts, grads
 
+    def eval_local_host(self, h_controls, h_costs, h_grads=None):
+        """End to end with host buffers (pinned torch CPU tensors or numpy arrays), copies inside."""
+        def ptr(a):
+            return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
+        rc = self.lib.dd4dvar_eval_local_host(self._h, ptr(h_controls), h_costs.ctypes.data_as(C.POINTER(C.c_double)),
+                                              ptr(h_grads) if h_grads is not None else None)
+        self._check("dd4dvar_eval_local_host", rc)
+
     def eval_global(self, x0, want_grad=True):
         torch = self.torch
         x0 = self._dev(x0)
@@ -246,8 +255,9 @@ class DD4DVar:
         self._check("dd4dvar_eval_global", rc)
         return float(J[0]), g
 
-    def sweep_async(self, with_adjoint=True):
-        self._check("dd4dvar_sweep_async", self.lib.dd4dvar_sweep_async(self._h, 1 if with_adjoint else 0))
+    def sweep_async(self, mode=1):
+        """0: forward + costs, 1: forward + costs + adjoint (the gradient sweep), 2: adjoint only."""
+        self._check("dd4dvar_sweep_async", self.lib.dd4dvar_sweep_async(self._h, int(mode)))
 
     def run(self, outer_iters):
         torch = self.torch

@@ -597,11 +597,28 @@ int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, d
     return 0;
 }
 
-int dd4dvar_sweep_async(dd4dvar_t h, int with_adjoint)
+int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_costs, double* h_grads)
 {
-    if (!h) return -1;
+    if (!h || !h_controls || !h_costs) return fail(h, -1, "eval_local_host: null argument");
+    if (!h->have_bg) return fail(h, -3, "eval_local_host before set_background");
+    Layout& L = h->L;
+    CU(cudaMemcpyAsync(L.x, h_controls, sizeof(double) * L.ctot, cudaMemcpyHostToDevice, h->stream));
+    sweep(h, L, h_grads != nullptr, nullptr, L.Jev, nullptr);
+    CU(cudaMemcpyAsync(h_costs, L.Jev, sizeof(double) * L.nsub, cudaMemcpyDeviceToHost, h->stream));
+    if (h_grads) CU(cudaMemcpyAsync(h_grads, L.gx, sizeof(double) * L.ctot, cudaMemcpyDeviceToHost, h->stream));
+    int rc = sync_check(h);
+    if (rc) return rc;
+    for (int k = 0; k < L.nsub; ++k)
+        if (!isfinite(h_costs[k])) return fail(h, -5, "eval_local_host: non-finite cost");
+    return 0;
+}
+
+int dd4dvar_sweep_async(dd4dvar_t h, int mode)
+{
+    if (!h || mode < 0 || mode > 2) return -1;
     if (!h->have_bg) return fail(h, -3, "sweep_async before set_background");
-    sweep(h, h->L, with_adjoint != 0, nullptr, h->L.Jev, nullptr);
+    if (mode == 2) adjoint_only(h, h->L, nullptr, nullptr);
+    else sweep(h, h->L, mode == 1, nullptr, h->L.Jev, nullptr);
     return 0;
 }
 
