@@ -303,27 +303,21 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 }
 
 // one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
-void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
-{
-    if (L.path == 2) {
-        fused_sweep(h->stream, &h->launches, L.fp, L.dsubs, L.nsub, mask, h->mp, h->cp, L.geo, L.x, L.xbs,
-                    L.xfrozen, L.pred_end, L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx,
-                    L.obs_y, L.obs_c, L.parts, Jout, with_adjoint, L.gx, gw);
-        return;
-    }
-    forward_generic(h, L, mask);
-    cost_generic(h, L, mask, Jout);
-    if (with_adjoint) adjoint_generic(h, L, mask, gw);
-}
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
     if (L.path == 2) {
-        fused_adjoint(h->stream, &h->launches, L.fp, L.dsubs, L.nsub, mask, h->mp, h->cp, L.geo, L.x, L.xbs,
-                      L.xfrozen, L.pred_end, L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx,
-                      L.obs_y, L.obs_c, L.gx, gw);
+        LAUNCH(fk_adjoint, L.nsub, FK_NT, L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end,
+               L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
         return;
     }
     adjoint_generic(h, L, mask, gw);
+}
+void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
+{
+    if (L.path == 2) LAUNCH(fk_forward, L.nsub, FK_NT, L.dsubs, mask, h->mp, L.x, L.traj, L.ghost);
+    else forward_generic(h, L, mask);
+    cost_generic(h, L, mask, Jout);
+    if (with_adjoint) adjoint_only(h, L, mask, gw);
 }
 
 // Alg 1 l.465: this iteration's results become the next one's frozen data
