@@ -4,6 +4,7 @@
 // exchange_kernels.cuh; there is no CPU fallback.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -306,16 +307,25 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
     if (L.path == 2) {
-        LAUNCH(fk_adjoint, L.nsub, FK_NT, L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end,
-               L.traj, L.ghost, L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
+        if (L.fp.lam_smem)
+            fk_adjoint<true><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
+                L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
+                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
+        else
+            fk_adjoint<false><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
+                L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
+                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
+        ++h->launches;
         return;
     }
     adjoint_generic(h, L, mask, gw);
 }
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
-    if (L.path == 2) LAUNCH(fk_forward, L.nsub, FK_NT, L.dsubs, mask, h->mp, L.x, L.traj, L.ghost);
-    else forward_generic(h, L, mask);
+    if (L.path == 2) {
+        fk_forward<<<L.nsub, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost);
+        ++h->launches;
+    } else forward_generic(h, L, mask);
     cost_generic(h, L, mask, Jout);
     if (with_adjoint) adjoint_only(h, L, mask, gw);
 }
@@ -404,8 +414,11 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     const bool fits = fused_fits(h->L.hs.data(), h->L.nsub);
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
     h->L.path = (h->opt.path == 1 || !fits) ? 1 : 2;
-    fused_plan_init(h->G.fp, nullptr, 0, h->opt.lbfgs_m);
-    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, h->opt.lbfgs_m);
+    fused_plan_init(h->G.fp, nullptr, 0, 0);
+    {
+        const char* e = getenv("DD4DVAR_LAM");      // tuning knob: 1 = adjoint variable in global memory, 2 = shared
+        fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, e ? atoi(e) : 0);
+    }
     h->ws_bytes = plan_all(h, nullptr);
     *out = h;
     return 0;

@@ -22,6 +22,9 @@
 
 struct FusedPlan {
     int enabled = 0;
+    int maxpy = 0, maxncell = 0;
+    int lam_smem = 0;                 // adjoint variable resident in shared memory
+    size_t smem_fwd = 0, smem_adj = 0;
 };
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
@@ -31,15 +34,20 @@ inline bool fused_fits(const Sub* subs, int nsub)
         if (subs[k].px > FK_NT || subs[k].py < 1) return false;
     return nsub > 0;
 }
-inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int) { fp.enabled = subs && nsub > 0; }
+inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mode);
 inline void fused_plan_arrays(FusedPlan&, fused_take_fn, void*) {}
 
-// geometry of the marching CTA, shared by both kernels
+// ------------------------------------------------------------------------------------------
+// Per-thread view of the marching CTA.  Row conditions are uniform over the CTA (plain branches);
+// column conditions are per-thread constants.  Values computed outside a stage's valid range are
+// finite and are never consumed by a valid cell, so only the adjoint
+// variable (zero outside the extended tile) and the global stores are predicated per thread.
 struct FkGeo {
     int px, py, ex, ey, gx, gys, gyn, joff, ncell, nring;
     bool perx, ws, wn;
     int i, li, iE, iW;
-    bool col_ok, cA, cH, cU;
+    bool col_ok, cU;
+    int jA0, jA1, jH0, jH1, jU0, jU1;     // row ranges of stage A / h1 / u1,v1 (half open)
 };
 __device__ __forceinline__ FkGeo fk_geo(const Sub& s)
 {
@@ -52,44 +60,66 @@ __device__ __forceinline__ FkGeo fk_geo(const Sub& s)
     g.iE = g.i + 1 < s.px ? g.i + 1 : (g.perx ? 0 : g.i);
     g.iW = g.i > 0 ? g.i - 1 : (g.perx ? s.px - 1 : 0);
     if (!g.col_ok) { g.iE = g.iW = g.i; }
-    g.cA = g.col_ok && (g.perx || (g.i >= 1 && g.i < s.px - 1));
-    g.cH = g.col_ok && (g.perx || (g.i >= 2 && g.i < s.px - 2));
     g.cU = g.col_ok && g.li >= 0 && g.li < s.ex;
+    g.jA0 = g.ws ? 0 : 1; g.jA1 = g.wn ? s.py : s.py - 1;
+    g.jH0 = g.ws ? 0 : 2; g.jH1 = g.wn ? s.py : s.py - 2;
+    g.jU0 = s.gys; g.jU1 = s.gys + s.ey;
     return g;
 }
-__device__ __forceinline__ bool fk_vA(const FkGeo& g, int j) { return j >= (g.ws ? 0 : 1) && j < (g.wn ? g.py : g.py - 1); }
-__device__ __forceinline__ bool fk_vH(const FkGeo& g, int j) { return j >= (g.ws ? 0 : 2) && j < (g.wn ? g.py : g.py - 2); }
-__device__ __forceinline__ bool fk_vU(const FkGeo& g, int j) { return j >= g.gys && j < g.gys + g.ey; }
 
-// value of padded row j, column of this thread, from the trajectory level (interior) or the frozen
-// ghost ring of that level
-__device__ __forceinline__ void fk_load_row(const FkGeo& g, int j, const double* tz, const double* gz, double z[3])
+// row tables of the tile in shared memory: entry r = padded row r-1 (rows -1 .. py, clamped)
+struct FkTab {
+    const double *dtcz, *gdtcz, *dtf, *dtt, *rp, *rm;
+};
+__device__ __forceinline__ FkTab fk_tables(const ModelP& m, const FkGeo& g, double* sm)
 {
-    z[0] = z[1] = z[2] = 0.0;
-    if (!g.col_ok || j < 0 || j >= g.py) return;
-    if (j >= g.gys && j < g.gys + g.ey) {
-        if (g.cU) {
-            const int c = (j - g.gys) * g.ex + g.li;
-#pragma unroll
-            for (int f = 0; f < 3; ++f) z[f] = tz[(long long)f * g.ncell + c];
-        } else {
-            const int rr = (g.gys + g.gyn) * g.px + (j - g.gys) * (2 * g.gx) + (g.i < g.gx ? g.i : g.i - g.ex);
-#pragma unroll
-            for (int f = 0; f < 3; ++f) z[f] = __ldg(gz + (long long)f * g.nring + rr);
-        }
-    } else {
-        const int rr = j < g.gys ? j * g.px + g.i : g.gys * g.px + (j - g.gys - g.ey) * g.px + g.i;
-#pragma unroll
-        for (int f = 0; f < 3; ++f) z[f] = __ldg(gz + (long long)f * g.nring + rr);
+    const int TP = g.py + 2;
+    for (int r = threadIdx.x; r < TP; r += FK_NT) {
+        int gj = g.joff + r - 1;
+        gj = gj < 0 ? 0 : (gj >= m.nlat ? m.nlat - 1 : gj);
+        sm[r] = m.dtcz[gj]; sm[TP + r] = m.gdtcz[gj]; sm[2 * TP + r] = m.dtf[gj];
+        sm[3 * TP + r] = m.dtt[gj]; sm[4 * TP + r] = m.rp[gj]; sm[5 * TP + r] = m.rm[gj];
     }
+    FkTab t;
+    t.dtcz = sm + 1; t.gdtcz = sm + TP + 1; t.dtf = sm + 2 * TP + 1; t.dtt = sm + 3 * TP + 1;
+    t.rp = sm + 4 * TP + 1; t.rm = sm + 5 * TP + 1;
+    return t;
+}
+
+// where this thread's column of the padded rows of one level lives: south ghost rows, tile rows
+// (trajectory store for tile columns, ghost strip otherwise), north ghost rows
+struct FkCol {
+    const double *pS, *pI, *pN;
+    int sI;
+    long long fI, fG;
+};
+__device__ __forceinline__ FkCol fk_col(const FkGeo& g, const double* tz, const double* gz)
+{
+    FkCol c;
+    const int i = g.col_ok ? g.i : 0;
+    c.fG = g.nring;
+    c.pS = gz + i;
+    c.pN = gz + g.gys * g.px + i;
+    if (g.cU || !g.col_ok) { c.pI = tz + (g.col_ok ? g.li : 0); c.sI = g.ex; c.fI = g.ncell; }
+    else { c.pI = gz + (g.gys + g.gyn) * g.px + (i < g.gx ? i : i - g.ex); c.sI = 2 * g.gx; c.fI = g.nring; }
+    return c;
+}
+__device__ __forceinline__ void fk_load_row(const FkGeo& g, const FkCol& c, int j, double z[3])
+{
+    const double* p; long long fs;
+    if (j < g.gys) { p = c.pS + j * g.px; fs = c.fG; }
+    else if (j < g.gys + g.ey) { p = c.pI + (j - g.gys) * c.sI; fs = c.fI; }
+    else { p = c.pN + (j - g.gys - g.ey) * g.px; fs = c.fG; }
+    z[0] = p[0]; z[1] = p[fs]; z[2] = p[2 * fs];
 }
 
 // ------------------------------------------------------------------------------------------
 // forward sweep of one window: Z^{n+1} = Phi(Z^n) for n = 0..W-1, every level to the store
 __global__ void __launch_bounds__(FK_NT) fk_forward(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                     ModelP m, const double* __restrict__ x, double* traj,
-                                                    const double* __restrict__ ghost)
+                                                    const double* ghost)
 {
+    extern __shared__ double dsm[];
     __shared__ double z0s[2][3][FK_NT];
     __shared__ double uas[2][FK_NT];
     __shared__ double h1s[2][FK_NT];
@@ -97,24 +127,26 @@ __global__ void __launch_bounds__(FK_NT) fk_forward(const Sub* __restrict__ subs
     if (mask && !mask[k]) return;
     const Sub s = subs[k];
     const FkGeo g = fk_geo(s);
+    const FkTab tb = fk_tables(m, g, dsm);
     const int i = g.i;
+    const double kap = m.kap, dtcm = m.dtcm, gdtcm = m.gdtcm;
     // level 0 of the store = the control
     for (int c = threadIdx.x; c < 3 * s.ncell; c += FK_NT) traj[s.toff + c] = x[s.coff + c];
     __syncthreads();
     for (int n = 0; n < s.W; ++n) {
         const double* tz = traj + s.toff + (long long)n * 3 * s.ncell;
-        double* tn = traj + s.toff + (long long)(n + 1) * 3 * s.ncell;
-        const double* gz = ghost + s.goff + (long long)n * 3 * s.nring;
-        double zm[3] = { 0, 0, 0 }, zc[3] = { 0, 0, 0 }, zp[3] = { 0, 0, 0 }, zn[3];
+        double* tn = traj + s.toff + (long long)(n + 1) * 3 * s.ncell + (g.cU ? g.li : 0);
+        const FkCol col = fk_col(g, tz, ghost + s.goff + (long long)n * 3 * s.nring);
+        double zm[3] = { 0, 0, 0 }, zc[3] = { 0, 0, 0 }, zp[3] = { 0, 0, 0 }, zn[3] = { 0, 0, 0 };
         double ha1 = 0, ha2 = 0, ua1 = 0, ua2 = 0, ua3 = 0, va1 = 0, va2 = 0, va3 = 0;
         double h1a = 0, h1b = 0, h1c = 0;
-        fk_load_row(g, 0, tz, gz, zn);
+        fk_load_row(g, col, 0, zn);
         for (int t = 0; t < s.py + 3; ++t) {
             // ---- S0: row t arrives (prefetched last tick), next row is requested
 #pragma unroll
             for (int f = 0; f < 3; ++f) { zm[f] = zc[f]; zc[f] = zp[f]; zp[f] = zn[f]; }
             if (t == s.py && g.wn) { zp[0] = zc[0]; zp[1] = zc[1]; zp[2] = -zc[2]; }   // mirrored pole row
-            fk_load_row(g, t + 1, tz, gz, zn);
+            if (t + 1 < s.py) fk_load_row(g, col, t + 1, zn);
             if (t < s.py) {
 #pragma unroll
                 for (int f = 0; f < 3; ++f) z0s[t & 1][f][i] = zp[f];
@@ -123,47 +155,46 @@ __global__ void __launch_bounds__(FK_NT) fk_forward(const Sub* __restrict__ subs
             {
                 const int j = t - 1;
                 double ha = 0, ua = 0, va = 0;
-                if (g.cA && fk_vA(g, j)) {
-                    const int gj = g.joff + j;
+                if (j >= g.jA0 && j < g.jA1) {
                     double sm0 = zm[0], sm1 = zm[1], sm2 = zm[2];
                     if (j == 0 && g.ws) { sm0 = zc[0]; sm1 = zc[1]; sm2 = -zc[2]; }
-                    const double cu = m.dtcz[gj] * zc[1], cv = m.dtcm * zc[2];
-                    ha = mm_stageA(zc[0], z0s[j & 1][0][g.iE], z0s[j & 1][0][g.iW], zp[0], sm0, cu, cv, m.kap);
-                    ua = mm_stageA(zc[1], z0s[j & 1][1][g.iE], z0s[j & 1][1][g.iW], zp[1], sm1, cu, cv, m.kap);
-                    va = mm_stageA(zc[2], z0s[j & 1][2][g.iE], z0s[j & 1][2][g.iW], zp[2], sm2, cu, cv, m.kap);
+                    const double cu = tb.dtcz[j] * zc[1], cv = dtcm * zc[2];
+                    const double* zE = &z0s[j & 1][0][g.iE];
+                    const double* zW = &z0s[j & 1][0][g.iW];
+                    ha = mm_stageA(zc[0], zE[0], zW[0], zp[0], sm0, cu, cv, kap);
+                    ua = mm_stageA(zc[1], zE[FK_NT], zW[FK_NT], zp[1], sm1, cu, cv, kap);
+                    va = mm_stageA(zc[2], zE[2 * FK_NT], zW[2 * FK_NT], zp[2], sm2, cu, cv, kap);
+                    uas[j & 1][i] = ua;
                 }
                 ha2 = ha1; ha1 = ha; ua3 = ua2; ua2 = ua1; ua1 = ua; va3 = va2; va2 = va1; va1 = va;
-                if (j >= 0) uas[j & 1][i] = ua;
             }
             // ---- S2: h1 on row j = t-2
             {
                 const int j = t - 2;
                 double h1 = 0;
-                if (g.cH && fk_vH(g, j)) {
-                    const int gj = g.joff + j;
+                if (j >= g.jH0 && j < g.jH1) {
                     const double vaN = (j == s.py - 1 && g.wn) ? -va2 : va1;
                     const double vaS = (j == 0 && g.ws) ? -va2 : va3;
-                    const double D = mm_div(uas[j & 1][g.iE], uas[j & 1][g.iW], vaN, vaS, m.dtcz[gj], m.dtcm,
-                                            m.rp[gj], m.rm[gj]);
+                    const double D = mm_div(uas[j & 1][g.iE], uas[j & 1][g.iW], vaN, vaS, tb.dtcz[j], dtcm,
+                                            tb.rp[j], tb.rm[j]);
                     h1 = mm_h1(ha2, D);
+                    h1s[j & 1][i] = h1;
                 }
                 h1c = h1b; h1b = h1a; h1a = h1;
-                if (j >= 0) h1s[j & 1][i] = h1;
             }
             // ---- S3: u1, v1 on row j = t-3 -> trajectory store
             {
                 const int j = t - 3;
-                if (g.cU && fk_vU(g, j)) {
-                    const int gj = g.joff + j;
-                    const double dtf = m.dtf[gj], dtt = m.dtt[gj];
+                if (j >= g.jU0 && j < g.jU1) {
+                    const double dtf = tb.dtf[j], dtt = tb.dtt[j];
                     const double h1N = (j == s.py - 1 && g.wn) ? h1b : h1a;
                     const double h1S = (j == 0 && g.ws) ? h1b : h1c;
-                    const double u1 = mm_u1(ua3, va3, h1s[j & 1][g.iE], h1s[j & 1][g.iW], m.gdtcz[gj], dtf, dtt);
-                    const double v1 = mm_v1(va3, u1, h1N, h1S, m.gdtcm, dtf, dtt);
-                    const int c = (j - s.gys) * s.ex + g.li;
-                    tn[c] = h1b;
-                    tn[s.ncell + c] = u1;
-                    tn[2 * s.ncell + c] = v1;
+                    const double u1 = mm_u1(ua3, va3, h1s[j & 1][g.iE], h1s[j & 1][g.iW], tb.gdtcz[j], dtf, dtt);
+                    const double v1 = mm_v1(va3, u1, h1N, h1S, gdtcm, dtf, dtt);
+                    if (g.cU) {
+                        double* o = tn + (j - s.gys) * s.ex;
+                        o[0] = h1b; o[s.ncell] = u1; o[2 * s.ncell] = v1;
+                    }
                 }
             }
             __syncthreads();
@@ -172,19 +203,22 @@ __global__ void __launch_bounds__(FK_NT) fk_forward(const Sub* __restrict__ subs
 }
 
 // ------------------------------------------------------------------------------------------
-// adjoint sweep of one window.  lam (= the gradient array of this subdomain, [3][ncell]) holds
-// the adjoint variable on the extended tile and is updated in place level by level.
+// adjoint sweep of one window.  The adjoint variable on the extended tile, [3][ncell], is updated
+// in place level by level; LSM = it lives in shared memory (tiles up to ~100 KB), otherwise in
+// the gradient array of the subdomain (L2-resident while its CTA runs).
+template <bool LSM>
 __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                     ModelP m, CostP cp, GeoP geo, const double* __restrict__ x,
                                                     const double* __restrict__ xbs,
                                                     const double* __restrict__ xfrozen,
                                                     const double* __restrict__ pred_end, const double* traj,
-                                                    const double* __restrict__ ghost,
+                                                    const double* ghost,
                                                     const long long* __restrict__ obs_start,
                                                     const int* __restrict__ obs_idx,
                                                     const double* __restrict__ obs_y,
                                                     const double* __restrict__ obs_c, double* gx, double* gw)
 {
+    extern __shared__ double dsm[];
     __shared__ double zr[FK_ZR][3][FK_NT];
     __shared__ double uas[4][FK_NT];
     __shared__ double ubs[2][FK_NT];
@@ -194,9 +228,11 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
     if (mask && !mask[k]) return;
     const Sub s = subs[k];
     const FkGeo g = fk_geo(s);
+    const FkTab tb = fk_tables(m, g, dsm);
     const int i = g.i;
-    double* lam = gx + s.coff;
-    const int n3 = 3 * s.ncell;
+    const int n3 = 3 * s.ncell, nc1 = s.ncell;
+    double* lam = LSM ? dsm + 6 * (s.py + 2) : gx + s.coff;
+    const double kap = m.kap, dtcm = m.dtcm, gdtcm = m.gdtcm, c0 = 1.0 - 4.0 * m.kap;
     // ---- adjoint variable at the window end: successor-window overlap forcing (25c), else zero
     {
         const bool succ = s.jw < geo.q - 1;
@@ -208,6 +244,7 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
         }
         __syncthreads();
     }
+    double* lcol = lam + (g.cU ? g.li : 0);                 // this thread's column of lam
     for (int n = s.W; n >= 0; --n) {
         // ---- H^T R^-1 (misfit) at level n (25b)
         if (obs_start) {
@@ -222,25 +259,22 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
         if (n == 0) break;
         // ---- lam <- M_{n-1}^T lam, marching over the rows
         const double* tz = traj + s.toff + (long long)(n - 1) * n3;
-        const double* tu = traj + s.toff + (long long)n * n3 + s.ncell;      // u^1 = u of level n
-        const double* gz = ghost + s.goff + (long long)(n - 1) * 3 * s.nring;
-        double zm[3] = { 0, 0, 0 }, zc[3] = { 0, 0, 0 }, zp[3] = { 0, 0, 0 }, zn[3];
+        const double* tu = traj + s.toff + (long long)n * n3 + s.ncell + (g.cU ? g.li : 0);   // u^1
+        const FkCol col = fk_col(g, tz, ghost + s.goff + (long long)(n - 1) * 3 * s.nring);
+        double zm[3] = { 0, 0, 0 }, zc[3] = { 0, 0, 0 }, zp[3] = { 0, 0, 0 }, zn[3] = { 0, 0, 0 };
         double ha1 = 0, ha2 = 0, ua1 = 0, ua2 = 0, ua3 = 0, va1 = 0, va2 = 0, va3 = 0, va4 = 0;
         double hb1 = 0, hb2 = 0, vb1 = 0, vb2 = 0, vb3 = 0, UB1 = 0, UB2 = 0, UB3 = 0;
         double HB2 = 0, HB3 = 0, P2 = 0, P3 = 0, P4 = 0;
         double A3[3] = { 0, 0, 0 }, A4[3] = { 0, 0, 0 }, A5[3] = { 0, 0, 0 };
-        double ln[4] = { 0, 0, 0, 0 };     // prefetched lam row (h,u,v) and u1
-        fk_load_row(g, 0, tz, gz, zn);
-        if (g.cU && fk_vU(g, 0)) {
-            const int c = (0 - s.gys) * s.ex + g.li;
-            ln[0] = lam[c]; ln[1] = lam[s.ncell + c]; ln[2] = lam[2 * s.ncell + c]; ln[3] = tu[c];
-        }
+        double l0 = 0, l1 = 0, l2 = 0, l3 = 0;     // prefetched lam row (h,u,v) and u1
+        fk_load_row(g, col, 0, zn);
+        if (g.jU0 == 0) { l0 = lcol[0]; l1 = lcol[nc1]; l2 = lcol[2 * nc1]; l3 = tu[0]; }
         for (int t = 0; t < s.py + 4; ++t) {
             // ---- S0: row t of Z0
 #pragma unroll
             for (int f = 0; f < 3; ++f) { zm[f] = zc[f]; zc[f] = zp[f]; zp[f] = zn[f]; }
             if (t == s.py && g.wn) { zp[0] = zc[0]; zp[1] = zc[1]; zp[2] = -zc[2]; }
-            fk_load_row(g, t + 1, tz, gz, zn);
+            if (t + 1 < s.py) fk_load_row(g, col, t + 1, zn);
             if (t < s.py) {
 #pragma unroll
                 for (int f = 0; f < 3; ++f) zr[t & (FK_ZR - 1)][f][i] = zp[f];
@@ -249,28 +283,27 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
             {
                 const int j = t - 1;
                 double ha = 0, ua = 0, va = 0;
-                if (g.cA && fk_vA(g, j)) {
-                    const int gj = g.joff + j, r = j & (FK_ZR - 1);
+                if (j >= g.jA0 && j < g.jA1) {
                     double sm0 = zm[0], sm1 = zm[1], sm2 = zm[2];
                     if (j == 0 && g.ws) { sm0 = zc[0]; sm1 = zc[1]; sm2 = -zc[2]; }
-                    const double cu = m.dtcz[gj] * zc[1], cv = m.dtcm * zc[2];
-                    ha = mm_stageA(zc[0], zr[r][0][g.iE], zr[r][0][g.iW], zp[0], sm0, cu, cv, m.kap);
-                    ua = mm_stageA(zc[1], zr[r][1][g.iE], zr[r][1][g.iW], zp[1], sm1, cu, cv, m.kap);
-                    va = mm_stageA(zc[2], zr[r][2][g.iE], zr[r][2][g.iW], zp[2], sm2, cu, cv, m.kap);
+                    const double cu = tb.dtcz[j] * zc[1], cv = dtcm * zc[2];
+                    const double* zE = &zr[j & (FK_ZR - 1)][0][g.iE];
+                    const double* zW = &zr[j & (FK_ZR - 1)][0][g.iW];
+                    ha = mm_stageA(zc[0], zE[0], zW[0], zp[0], sm0, cu, cv, kap);
+                    ua = mm_stageA(zc[1], zE[FK_NT], zW[FK_NT], zp[1], sm1, cu, cv, kap);
+                    va = mm_stageA(zc[2], zE[2 * FK_NT], zW[2 * FK_NT], zp[2], sm2, cu, cv, kap);
+                    uas[j & 3][i] = ua;
                 }
                 ha2 = ha1; ha1 = ha; ua3 = ua2; ua2 = ua1; ua1 = ua;
                 va4 = va3; va3 = va2; va2 = va1; va1 = va;
-                if (j >= 0) uas[j & 3][i] = ua;
-                // lam^{n} row j (prefetched) -> UB; next row requested
+                // lam row j (prefetched) -> UB; next row requested
                 double UB = 0, hb = 0, vb = 0;
-                if (g.cU && fk_vU(g, j)) {
-                    const int gj = g.joff + j;
-                    hb = ln[0]; vb = ln[2];
-                    UB = mm_UB(ln[1], ln[2], ln[3], m.dtf[gj], m.dtt[gj]);
+                if (j >= g.jU0 && j < g.jU1) {
+                    if (g.cU) { hb = l0; vb = l2; UB = mm_UB(l1, l2, l3, tb.dtf[j], tb.dtt[j]); }
                 }
-                if (g.cU && fk_vU(g, j + 1)) {
-                    const int c = (j + 1 - s.gys) * s.ex + g.li;
-                    ln[0] = lam[c]; ln[1] = lam[s.ncell + c]; ln[2] = lam[2 * s.ncell + c]; ln[3] = tu[c];
+                if (j + 1 >= g.jU0 && j + 1 < g.jU1) {
+                    const int o = (j + 1 - s.gys) * s.ex;
+                    l0 = lcol[o]; l1 = lcol[nc1 + o]; l2 = lcol[2 * nc1 + o]; l3 = tu[o];
                 }
                 hb2 = hb1; hb1 = hb; vb3 = vb2; vb2 = vb1; vb1 = vb; UB3 = UB2; UB2 = UB1; UB1 = UB;
                 if (j >= 0) ubs[j & 1][i] = UB;
@@ -279,11 +312,10 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
             {
                 const int j = t - 2;
                 double HB = 0, P = 0;
-                if (g.cA && fk_vA(g, j)) {
-                    const int gj = g.joff + j;
+                if (j >= g.jA0 && j < g.jA1) {
                     const double vbN = (j == s.py - 1 && g.wn) ? -vb2 : vb1;
                     const double vbS = (j == 0 && g.ws) ? -vb2 : vb3;
-                    HB = mm_HB(hb2, vbN, vbS, ubs[j & 1][g.iE], ubs[j & 1][g.iW], m.gdtcm, m.gdtcz[gj]);
+                    HB = mm_HB(hb2, vbN, vbS, ubs[j & 1][g.iE], ubs[j & 1][g.iW], gdtcm, tb.gdtcz[j]);
                     P = -ha2 * HB;
                 }
                 HB3 = HB2; HB2 = HB; P4 = P3; P3 = P2; P2 = P;
@@ -293,21 +325,20 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
             {
                 const int j = t - 3;
                 double a0 = 0, a1 = 0, a2 = 0;
-                if (g.cA && fk_vA(g, j)) {
-                    const int gj = g.joff + j;
-                    const double dtcz = m.dtcz[gj], dtf = m.dtf[gj], dtt = m.dtt[gj];
+                if (j >= g.jA0 && j < g.jA1) {
+                    const double dtcz = tb.dtcz[j], dtf = tb.dtf[j], dtt = tb.dtt[j];
                     const bool atN = (j == s.py - 1 && g.wn), atS = (j == 0 && g.ws);
-                    if (g.cH && fk_vH(g, j)) {
+                    if (j >= g.jH0 && j < g.jH1) {
                         const double vaN = atN ? -va3 : va2;
                         const double vaS = atS ? -va3 : va4;
-                        const double D = mm_div(uas[j & 3][g.iE], uas[j & 3][g.iW], vaN, vaS, dtcz, m.dtcm,
-                                                m.rp[gj], m.rm[gj]);
+                        const double D = mm_div(uas[j & 3][g.iE], uas[j & 3][g.iW], vaN, vaS, dtcz, dtcm,
+                                                tb.rp[j], tb.rm[j]);
                         a0 = mm_Ah(HB3, D);
                     }
-                    const double PSr = atS ? m.rm[gj] * P3 : m.rp[gj - 1] * P4;
-                    const double PNr = atN ? m.rp[gj] * P3 : m.rm[gj + 1] * P2;
+                    const double PSr = atS ? tb.rm[j] * P3 : tb.rp[j - 1] * P4;
+                    const double PNr = atN ? tb.rp[j] * P3 : tb.rm[j + 1] * P2;
                     a1 = mm_Au(UB3, va3, ps[j & 1][g.iW], ps[j & 1][g.iE], dtt, dtcz);
-                    a2 = mm_Av(vb3, UB3, ua3, PSr, PNr, dtf, dtt, m.dtcm);
+                    a2 = mm_Av(vb3, UB3, ua3, PSr, PNr, dtf, dtt, dtcm);
                 }
 #pragma unroll
                 for (int f = 0; f < 3; ++f) { A5[f] = A4[f]; A4[f] = A3[f]; }
@@ -317,36 +348,38 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
             // ---- S4: lam0 on row j = t-4 (extended tile) -> in place
             {
                 const int j = t - 4;
-                if (g.cU && fk_vU(g, j)) {
-                    const int gj = g.joff + j;
-                    const double dtcz = m.dtcz[gj], dtcm = m.dtcm;
+                if (j >= g.jU0 && j < g.jU1) {
+                    const double dtcz = tb.dtcz[j];
                     const bool atN = (j == s.py - 1 && g.wn), atS = (j == 0 && g.ws);
-                    const int r = j & (FK_ZR - 1), rN = (j + 1) & (FK_ZR - 1), rS = (j - 1) & (FK_ZR - 1);
+                    const double* zc_ = &zr[j & (FK_ZR - 1)][0][0];
+                    const double* zN_ = atN ? zc_ : &zr[(j + 1) & (FK_ZR - 1)][0][0];
+                    const double* zS_ = atS ? zc_ : &zr[(j - 1) & (FK_ZR - 1)][0][0];
                     double xE[3], xW[3], xN[3], xS[3];
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {
-                        xE[f] = zr[r][f][g.iE]; xW[f] = zr[r][f][g.iW];
-                        xN[f] = atN ? zr[r][f][i] : zr[rN][f][i];
-                        xS[f] = atS ? zr[r][f][i] : zr[rS][f][i];
+                        xE[f] = zc_[f * FK_NT + g.iE]; xW[f] = zc_[f * FK_NT + g.iW];
+                        xN[f] = zN_[f * FK_NT + i]; xS[f] = zS_[f * FK_NT + i];
                     }
                     if (atN) xN[2] = -xN[2];
                     if (atS) xS[2] = -xS[2];
-                    const double cuW = dtcz * xW[1], cuE = dtcz * xE[1];
-                    const double cvS = dtcm * xS[2], cvN = dtcm * xN[2];
+                    const double kW = kap - dtcz * xW[1], kE = kap + dtcz * xE[1];
+                    const double kS = kap - dtcm * xS[2], kN = kap + dtcm * xN[2];
+                    const double* aE = &as[j & 1][0][g.iE];
+                    const double* aW = &as[j & 1][0][g.iW];
                     double out[3], su = 0.0, sv = 0.0;
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {
                         const double sg = f == 2 ? -1.0 : 1.0;
                         const double aN = atN ? sg * A4[f] : A3[f];
                         const double aS = atS ? sg * A4[f] : A5[f];
-                        out[f] = mm_L0(A4[f], as[j & 1][f][g.iW], as[j & 1][f][g.iE], aS, aN, cuW, cuE, cvS, cvN, m.kap);
+                        out[f] = A4[f] * c0 + aW[f * FK_NT] * kW + aE[f * FK_NT] * kE + aS * kS + aN * kN;
                         su += (xE[f] - xW[f]) * A4[f];
                         sv += (xN[f] - xS[f]) * A4[f];
                     }
-                    const int c = (j - s.gys) * s.ex + g.li;
-                    lam[c] = out[0];
-                    lam[s.ncell + c] = out[1] - dtcz * su;
-                    lam[2 * s.ncell + c] = out[2] - dtcm * sv;
+                    if (g.cU) {
+                        double* o = lcol + (j - s.gys) * s.ex;
+                        o[0] = out[0]; o[nc1] = out[1] - dtcz * su; o[2 * nc1] = out[2] - dtcm * sv;
+                    }
                 }
             }
             __syncthreads();
@@ -364,7 +397,7 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
             for (int f = 0; f < 3; ++f) {
                 const long long o = s.coff + (long long)f * s.ncell + c;
                 const double xv = x[o];
-                double gg = gx[o];
+                double gg = lam[f * s.ncell + c];
                 gg += 2.0 * wsp * (xv - xbs[o]) * cp.ib[f];
                 if (nc * nr > 1)
                     for (int cb = 0; cb < nr; ++cb)
@@ -383,4 +416,40 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
     }
 }
 
-inline int fused_setup(cudaStream_t, FusedPlan&, const Sub*) { return 0; }
+// dynamic shared memory of the two kernels (row tables, and the adjoint variable when resident)
+inline size_t fused_smem_forward(int maxpy) { return sizeof(double) * 6 * (size_t)(maxpy + 2); }
+inline size_t fused_smem_adjoint(int maxpy, int maxncell, bool lsm)
+{
+    return sizeof(double) * (6 * (size_t)(maxpy + 2) + (lsm ? 3 * (size_t)maxncell : 0));
+}
+
+// lam_mode: 0 auto (shared memory when two CTAs per SM still fit), 1 global, 2 shared
+inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mode)
+{
+    fp = FusedPlan();
+    if (!subs || nsub <= 0) return;
+    fp.enabled = 1;
+    for (int k = 0; k < nsub; ++k) {
+        fp.maxpy = subs[k].py > fp.maxpy ? subs[k].py : fp.maxpy;
+        fp.maxncell = subs[k].ncell > fp.maxncell ? subs[k].ncell : fp.maxncell;
+    }
+    const size_t stat = sizeof(double) * FK_NT * (FK_ZR * 3 + 4 + 2 + 2 + 6);
+    const size_t with = fused_smem_adjoint(fp.maxpy, fp.maxncell, true) + stat;
+    const bool can = with <= 227 * 1024;
+    const bool two = with <= 113 * 1024;
+    fp.lam_smem = lam_mode == 2 ? (can ? 1 : 0) : (lam_mode == 1 ? 0 : (two ? 1 : 0));
+    fp.smem_fwd = fused_smem_forward(fp.maxpy);
+    fp.smem_adj = fused_smem_adjoint(fp.maxpy, fp.maxncell, fp.lam_smem != 0);
+}
+inline int fused_setup(cudaStream_t, FusedPlan& fp, const Sub*)
+{
+    if (!fp.enabled) return 0;
+    cudaError_t e = cudaFuncSetAttribute(fk_adjoint<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, true) <= 200 * 1024
+                                             ? (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, true) : 200 * 1024);
+    if (e != cudaSuccess) return -1;
+    e = cudaFuncSetAttribute(fk_adjoint<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, false));
+    if (e != cudaSuccess) return -1;
+    e = cudaFuncSetAttribute(fk_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fp.smem_fwd);
+    return e == cudaSuccess ? 0 : -1;
+}
