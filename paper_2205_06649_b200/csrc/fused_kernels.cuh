@@ -416,6 +416,8 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
     }
 }
 
+#include "fused_adjoint.cuh"
+
 // dynamic shared memory of the two kernels (row tables, and the adjoint variable when resident)
 inline size_t fused_smem_forward(int maxpy) { return sizeof(double) * 6 * (size_t)(maxpy + 2); }
 inline size_t fused_smem_adjoint(int maxpy, int maxncell, bool lsm)
@@ -449,6 +451,8 @@ inline int fused_setup(cudaStream_t, FusedPlan& fp, const Sub*)
                                              ? (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, true) : 200 * 1024);
     if (e != cudaSuccess) return -1;
     e = cudaFuncSetAttribute(fk_adjoint<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, false));
+    if (e != cudaSuccess) return -1;
+    e = cudaFuncSetAttribute(fk_adjoint2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, false));
     if (e != cudaSuccess) return -1;
     e = cudaFuncSetAttribute(fk_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fp.smem_fwd);
     return e == cudaSuccess ? 0 : -1;
