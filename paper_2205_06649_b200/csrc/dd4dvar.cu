@@ -311,10 +311,13 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
             fk_adjoint<true><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
-        else if (!getenv("DD4DVAR_ADJ1"))
-            fk_adjoint2<<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
+        else if (!getenv("DD4DVAR_ADJ1")) {
+            cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
+            fk_adjoint2<<<L.fp.nslots, FK_NT, L.fp.smem_adj, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
-                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
+                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
+                L.fp.slot_stride, L.fp.counter);
+        }
         else
             fk_adjoint<false><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,

@@ -171,23 +171,33 @@ __global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ 
                                                         const long long* __restrict__ obs_start,
                                                         const int* __restrict__ obs_idx,
                                                         const double* __restrict__ obs_y,
-                                                        const double* __restrict__ obs_c, double* gx, double* gw)
+                                                        const double* __restrict__ obs_c, double* gx, double* gw,
+                                                        int nsub, double* scratch, long long slot_stride,
+                                                        int* counter)
 {
     extern __shared__ double dsm[];
+    __shared__ int s_next;
     __shared__ double zr[FK_ZR * 3 * FK_NT];
     __shared__ double uas[4 * FK_NT];
     __shared__ double ubs[2 * FK_NT];
     __shared__ double ps[2 * FK_NT];
     __shared__ double as[2 * 3 * FK_NT];
-    const int k = blockIdx.x;
-    if (mask && !mask[k]) return;
+    // persistent CTA: subdomains are taken from a work counter; the adjoint variable lives in this
+    // CTA's slot of an L2-persistent scratch, not in HBM
+    for (;;) {
+    if (threadIdx.x == 0) s_next = atomicAdd(counter, 1);
+    __syncthreads();
+    const int k = s_next;
+    __syncthreads();
+    if (k >= nsub) break;
+    if (mask && !mask[k]) continue;
     const Sub s = subs[k];
     AdjCtx C;
     C.g = fk_geo(s);
     C.tb = fk_tables(m, C.g, dsm);
     const FkGeo& g = C.g;
     const int n3 = 3 * s.ncell;
-    double* lam = gx + s.coff;
+    double* lam = scratch + (long long)blockIdx.x * slot_stride;
     C.zr = zr; C.uas = uas; C.ubs = ubs; C.ps = ps; C.as = as;
     C.nc1 = s.ncell; C.gys = s.gys; C.ex = s.ex; C.py = s.py;
     C.kap = m.kap; C.dtcm = m.dtcm; C.gdtcm = m.gdtcm; C.c0 = 1.0 - 4.0 * m.kap;
@@ -281,4 +291,5 @@ __global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ 
             }
         }
     }
+    }   // persistent loop
 }

@@ -14,6 +14,8 @@
 // and is updated in place, row j being rewritten three ticks after it was read.
 // No step is recomputed, nothing is re-read from HBM, no atomics: results are deterministic.
 #pragma once
+#include <stdlib.h>
+#include <string.h>
 #include "common.cuh"
 #include "model_math.cuh"
 
@@ -25,7 +27,13 @@ struct FusedPlan {
     int maxpy = 0, maxncell = 0;
     int lam_smem = 0;                 // adjoint variable resident in shared memory
     size_t smem_fwd = 0, smem_adj = 0;
+    // persistent CTAs: one L2-persistent scratch slot per resident CTA (in-place state / adjoint variable)
+    int nslots = 0;
+    long long slot_stride = 0;        // doubles
+    double* scratch = nullptr;
+    int* counter = nullptr;
 };
+#define FK_SLOTS (148 * 3)          // B200: 148 SMs x 3 resident CTAs
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
 inline bool fused_fits(const Sub* subs, int nsub)
@@ -35,7 +43,12 @@ inline bool fused_fits(const Sub* subs, int nsub)
     return nsub > 0;
 }
 inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mode);
-inline void fused_plan_arrays(FusedPlan&, fused_take_fn, void*) {}
+inline void fused_plan_arrays(FusedPlan& fp, fused_take_fn take, void* arena)
+{
+    if (!fp.enabled) return;
+    fp.scratch = (double*)take(arena, sizeof(double) * (size_t)fp.nslots * fp.slot_stride);
+    fp.counter = (int*)take(arena, 64);
+}
 
 // ------------------------------------------------------------------------------------------
 // Per-thread view of the marching CTA.  Row conditions are uniform over the CTA (plain branches);
@@ -440,12 +453,31 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
     const bool can = with <= 227 * 1024;
     const bool two = with <= 113 * 1024;
     fp.lam_smem = lam_mode == 2 ? (can ? 1 : 0) : (lam_mode == 1 ? 0 : (two ? 1 : 0));
+    fp.nslots = nsub < FK_SLOTS ? nsub : FK_SLOTS;
+    fp.slot_stride = (3LL * fp.maxncell + 31) & ~31LL;
     fp.smem_fwd = fused_smem_forward(fp.maxpy);
     fp.smem_adj = fused_smem_adjoint(fp.maxpy, fp.maxncell, fp.lam_smem != 0);
 }
-inline int fused_setup(cudaStream_t, FusedPlan& fp, const Sub*)
+inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
 {
     if (!fp.enabled) return 0;
+    {   // keep the per-CTA scratch resident in L2; everything else streams through the rest
+        int dev = 0; cudaGetDevice(&dev);
+        cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
+        size_t bytes = sizeof(double) * (size_t)fp.nslots * fp.slot_stride;
+        size_t lim = bytes < (size_t)prop.persistingL2CacheMaxSize ? bytes : (size_t)prop.persistingL2CacheMaxSize;
+        if (lim > 0 && !getenv("DD4DVAR_NO_L2PIN")) {
+            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, lim);
+            cudaStreamAttrValue av; memset(&av, 0, sizeof(av));
+            av.accessPolicyWindow.base_ptr = fp.scratch;
+            av.accessPolicyWindow.num_bytes = bytes < (size_t)prop.accessPolicyMaxWindowSize ? bytes : (size_t)prop.accessPolicyMaxWindowSize;
+            av.accessPolicyWindow.hitRatio = lim >= bytes ? 1.0f : (float)lim / (float)bytes;
+            av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+            av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+            cudaStreamSetAttribute(stream, cudaStreamAttributeAccessPolicyWindow, &av);
+            cudaGetLastError();
+        }
+    }
     cudaError_t e = cudaFuncSetAttribute(fk_adjoint<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, true) <= 200 * 1024
                                              ? (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, true) : 200 * 1024);
