@@ -60,9 +60,10 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIBPATH):
+    path = os.environ.get("DD4DVAR_LIB", LIBPATH)     # override: an alternative build of the same ABI
+    if not os.path.exists(path):
         raise DD4DVarError("load_library", -4, f"{LIBPATH} is missing: run `python -m paper_2205_06649_b200.build`")
-    lib = C.CDLL(LIBPATH)
+    lib = C.CDLL(path)
     vp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_int)   # device pointers travel as integers
     hd = C.POINTER(C.c_double)
     lib.dd4dvar_create.argtypes = [C.POINTER(Grid), C.POINTER(Decomp), C.POINTER(Window), C.POINTER(Opts), vp, C.POINTER(vp)]

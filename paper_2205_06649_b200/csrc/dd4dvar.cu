@@ -303,6 +303,15 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
            L.pred_end, buf[L.Wmax & 1], L.gx, gw);
 }
 
+// the constant-memory row tables belong to the handle that launched last
+static const void* g_ctab_owner = nullptr;
+void ensure_tables(dd4dvar_t h)
+{
+    if (g_ctab_owner == h) return;
+    fused_upload_tables(h->stream, h->h_tab.data(), h->grid.nlat);
+    g_ctab_owner = h;
+}
+
 // one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
@@ -312,6 +321,7 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
         else if (!getenv("DD4DVAR_ADJ1")) {
+            ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
             fk_adjoint2<<<L.fp.nslots, FK_NT, L.fp.smem_adj, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
@@ -329,7 +339,13 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 }
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
-    if (L.path == 2) {
+    if (L.path == 2 && !getenv("DD4DVAR_FWD1")) {
+        ensure_tables(h);
+        cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
+        fk_forward2<<<L.fp.nslots_fwd, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
+                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
+        ++h->launches;
+    } else if (L.path == 2) {
         fk_forward<<<L.nsub, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost);
         ++h->launches;
     } else forward_generic(h, L, mask);
@@ -418,7 +434,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     if (rc) { delete h; return rc; }
     h->G.lbfgs = false; h->L.lbfgs = true;
     h->G.path = 1;
-    const bool fits = fused_fits(h->L.hs.data(), h->L.nsub);
+    const bool fits = fused_fits(h->L.hs.data(), h->L.nsub) && nlat + 2 <= FK_CTAB;
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
     h->L.path = (h->opt.path == 1 || !fits) ? 1 : 2;
     fused_plan_init(h->G.fp, nullptr, 0, 0);
@@ -772,6 +788,10 @@ long long dd4dvar_control_offset(dd4dvar_t h, int sub)
 int dd4dvar_active_path(dd4dvar_t h) { return h ? h->L.path : -1; }
 long long dd4dvar_launch_count(dd4dvar_t h) { return h ? h->launches : -1; }
 const char* dd4dvar_last_error(dd4dvar_t h) { return h ? h->err.c_str() : "null handle"; }
-void dd4dvar_destroy(dd4dvar_t h) { delete h; }
+void dd4dvar_destroy(dd4dvar_t h)
+{
+    if (g_ctab_owner == h) g_ctab_owner = nullptr;
+    delete h;
+}
 
 }  // extern "C"

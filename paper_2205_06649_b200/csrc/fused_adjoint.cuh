@@ -22,7 +22,7 @@ struct AdjRegs {
 };
 struct AdjCtx {
     FkGeo g;
-    FkTab tb;
+    int cj;                         // joff + 1: index of padded row 0 in the constant tables
     FkCol col;
     double* zr;                     // [8][3][FK_NT]
     double* uas;                    // [4][FK_NT]
@@ -69,7 +69,7 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
         const int j = t - 1;
         if (ST || (j >= g.jA0 && j < g.jA1)) {
             const double* zc = R.z[SL(1)];
-            const double cu = C.tb.dtcz[j] * zc[1], cv = C.dtcm * zc[2];
+            const double cu = ctab(CT_DTCZ, C.cj, j) * zc[1], cv = C.dtcm * zc[2];
             const double* zE = C.zr + (zr_slot<PH, 1>(h) * 3) * FK_NT + g.iE;
             const double* zW = C.zr + (zr_slot<PH, 1>(h) * 3) * FK_NT + g.iW;
             R.ha[S2(1)] = mm_stageA(zc[0], zE[0], zW[0], R.z[SL(0)][0], R.z[SL(2)][0], cu, cv, C.kap);
@@ -82,7 +82,7 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
         // lam row j (prefetched) -> hb, vb, UB (exact zeros outside the extended tile)
         double UB = 0.0, hb = 0.0, vb = 0.0;
         if (ST || (j >= g.jU0 && j < g.jU1)) {
-            if (g.cU) { hb = R.l0; vb = R.l2; UB = mm_UB(R.l1, R.l2, R.l3, C.tb.dtf[j], C.tb.dtt[j]); }
+            if (g.cU) { hb = R.l0; vb = R.l2; UB = mm_UB(R.l1, R.l2, R.l3, ctab(CT_DTF, C.cj, j), ctab(CT_DTT, C.cj, j)); }
             if (!ST && j == 0 && g.ws) R.vb[SL(2)] = -vb;
         } else if (!ST && j == C.py && g.wn) vb = -R.vb[SL(2)];
         R.hb[S2(1)] = hb; R.vb[SL(1)] = vb; R.UB[SL(1)] = UB;
@@ -98,10 +98,10 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
         double HB = 0.0, P = 0.0;
         if (ST || (j >= g.jA0 && j < g.jA1)) {
             HB = mm_HB(R.hb[S2(2)], R.vb[SL(1)], R.vb[SL(3)], C.ubs[S2(2) * FK_NT + g.iE],
-                       C.ubs[S2(2) * FK_NT + g.iW], C.gdtcm, C.tb.gdtcz[j]);
+                       C.ubs[S2(2) * FK_NT + g.iW], C.gdtcm, ctab(CT_GDTCZ, C.cj, j));
             P = -R.ha[S2(2)] * HB;
-            if (!ST && j == 0 && g.ws) R.P[SL(3)] = C.tb.rm[0] * P;
-        } else if (!ST && j == C.py && g.wn) P = C.tb.rp[C.py - 1] * R.P[SL(3)];
+            if (!ST && j == 0 && g.ws) R.P[SL(3)] = ctab(CT_RM, C.cj, 0) * P;
+        } else if (!ST && j == C.py && g.wn) P = ctab(CT_RP, C.cj, C.py - 1) * R.P[SL(3)];
         R.HB[S2(2)] = HB; R.P[SL(2)] = P;
         C.ps[S2(2) * FK_NT + i] = P;
     }
@@ -110,15 +110,15 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
         const int j = t - 3;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0;
         if (ST || (j >= g.jA0 && j < g.jA1)) {
-            const double dtcz = C.tb.dtcz[j], dtf = C.tb.dtf[j], dtt = C.tb.dtt[j];
+            const double dtcz = ctab(CT_DTCZ, C.cj, j), dtf = ctab(CT_DTF, C.cj, j), dtt = ctab(CT_DTT, C.cj, j);
             if (ST || (j >= g.jH0 && j < g.jH1)) {
                 const double D = mm_div(C.uas[SL(3) * FK_NT + g.iE], C.uas[SL(3) * FK_NT + g.iW], R.va[SL(2)],
-                                        R.va[SL(4)], dtcz, C.dtcm, C.tb.rp[j], C.tb.rm[j]);
+                                        R.va[SL(4)], dtcz, C.dtcm, ctab(CT_RP, C.cj, j), ctab(CT_RM, C.cj, j));
                 a0 = mm_Ah(R.HB[S2(3)], D);
             }
             a1 = mm_Au(R.UB[SL(3)], R.va[SL(3)], C.ps[S2(3) * FK_NT + g.iW], C.ps[S2(3) * FK_NT + g.iE], dtt, dtcz);
-            a2 = mm_Av(R.vb[SL(3)], R.UB[SL(3)], R.ua[SL(3)], C.tb.rp[j - 1] * R.P[SL(4)],
-                       C.tb.rm[j + 1] * R.P[SL(2)], dtf, dtt, C.dtcm);
+            a2 = mm_Av(R.vb[SL(3)], R.UB[SL(3)], R.ua[SL(3)], ctab(CT_RP, C.cj, j - 1) * R.P[SL(4)],
+                       ctab(CT_RM, C.cj, j + 1) * R.P[SL(2)], dtf, dtt, C.dtcm);
             if (!ST && j == 0 && g.ws) { R.A[SL(4)][0] = a0; R.A[SL(4)][1] = a1; R.A[SL(4)][2] = -a2; }
         } else if (!ST && j == C.py && g.wn) { a0 = R.A[SL(4)][0]; a1 = R.A[SL(4)][1]; a2 = -R.A[SL(4)][2]; }
         R.A[SL(3)][0] = a0; R.A[SL(3)][1] = a1; R.A[SL(3)][2] = a2;
@@ -129,7 +129,7 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
     {
         const int j = t - 4;
         if (ST || (j >= g.jU0 && j < g.jU1)) {
-            const double dtcz = C.tb.dtcz[j];
+            const double dtcz = ctab(CT_DTCZ, C.cj, j);
             const double* zc_ = C.zr + (zr_slot<PH, 4>(h) * 3) * FK_NT;
             const double* zN_ = C.zr + (zr_slot<PH, 3>(h) * 3) * FK_NT + i;
             const double* zS_ = C.zr + (zr_slot<PH, 5>(h) * 3) * FK_NT + i;
@@ -194,7 +194,7 @@ __global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ 
     const Sub s = subs[k];
     AdjCtx C;
     C.g = fk_geo(s);
-    C.tb = fk_tables(m, C.g, dsm);
+    C.cj = C.g.joff + 1;
     const FkGeo& g = C.g;
     const int n3 = 3 * s.ncell;
     double* lam = scratch + (long long)blockIdx.x * slot_stride;
@@ -210,12 +210,6 @@ __global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ 
         for (int c = threadIdx.x; c < n3; c += FK_NT) {
             const int f = c / s.ncell;
             lam[c] = succ ? 2.0 * cp.mu * (tw[c] - xn[c]) * cp.ib[f] : 0.0;
-        }
-        __syncthreads();
-        // metric ratios of the virtual mirrored pole rows (see header)
-        if (threadIdx.x == 0) {
-            if (g.ws) dsm[4 * (s.py + 2) + 0] = 1.0;               // r+ of row -1
-            if (g.wn) dsm[5 * (s.py + 2) + s.py + 1] = 1.0;        // r- of row py
         }
         __syncthreads();
     }

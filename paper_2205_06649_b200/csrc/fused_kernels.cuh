@@ -28,12 +28,13 @@ struct FusedPlan {
     int lam_smem = 0;                 // adjoint variable resident in shared memory
     size_t smem_fwd = 0, smem_adj = 0;
     // persistent CTAs: one L2-persistent scratch slot per resident CTA (in-place state / adjoint variable)
-    int nslots = 0;
+    int nslots = 0, nslots_fwd = 0;
     long long slot_stride = 0;        // doubles
     double* scratch = nullptr;
     int* counter = nullptr;
 };
-#define FK_SLOTS (148 * 3)          // B200: 148 SMs x 3 resident CTAs
+#define FK_SLOTS (148 * 3)          // B200: 148 SMs x 3 resident CTAs (adjoint)
+#define FK_SLOTS_FWD (148 * 4)      // forward kernel: 4 resident CTAs per SM
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
 inline bool fused_fits(const Sub* subs, int nsub)
@@ -46,7 +47,7 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
 inline void fused_plan_arrays(FusedPlan& fp, fused_take_fn take, void* arena)
 {
     if (!fp.enabled) return;
-    fp.scratch = (double*)take(arena, sizeof(double) * (size_t)fp.nslots * fp.slot_stride);
+    fp.scratch = (double*)take(arena, sizeof(double) * (size_t)fp.nslots_fwd * fp.slot_stride);
     fp.counter = (int*)take(arena, 64);
 }
 
@@ -429,7 +430,21 @@ __global__ void __launch_bounds__(FK_NT) fk_adjoint(const Sub* __restrict__ subs
     }
 }
 
+// Row tables in constant memory for the static-slot kernels: entry [k][gj + 1], with guard entries
+// r+_{-1} = 1 and r-_{nlat} = 1 for the virtual mirrored pole rows.  Uniform (per-CTA) index ->
+// constant-cache loads, which keep the tables off the L1TEX/shared-memory pipe.
+#define FK_CTAB 1026
+__constant__ double c_tab[6][FK_CTAB];
+#define CT_DTCZ 0
+#define CT_GDTCZ 1
+#define CT_DTF 2
+#define CT_DTT 3
+#define CT_RP 4
+#define CT_RM 5
+__device__ __forceinline__ double ctab(int k, int cj, int j) { return c_tab[k][cj + j]; }
+
 #include "fused_adjoint.cuh"
+#include "fused_forward.cuh"
 
 // dynamic shared memory of the two kernels (row tables, and the adjoint variable when resident)
 inline size_t fused_smem_forward(int maxpy) { return sizeof(double) * 6 * (size_t)(maxpy + 2); }
@@ -454,9 +469,24 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
     const bool two = with <= 113 * 1024;
     fp.lam_smem = lam_mode == 2 ? (can ? 1 : 0) : (lam_mode == 1 ? 0 : (two ? 1 : 0));
     fp.nslots = nsub < FK_SLOTS ? nsub : FK_SLOTS;
+    fp.nslots_fwd = nsub < FK_SLOTS_FWD ? nsub : FK_SLOTS_FWD;
     fp.slot_stride = (3LL * fp.maxncell + 31) & ~31LL;
     fp.smem_fwd = fused_smem_forward(fp.maxpy);
     fp.smem_adj = fused_smem_adjoint(fp.maxpy, fp.maxncell, fp.lam_smem != 0);
+}
+// copy the row tables (host, 6 x nlat, order dtcz gdtcz dtf dtt rp rm) into constant memory
+inline int fused_upload_tables(cudaStream_t stream, const double* h_tab, int nlat)
+{
+    if (nlat + 2 > FK_CTAB) return -1;
+    static double buf[6][FK_CTAB];
+    for (int k = 0; k < 6; ++k) {
+        for (int q = 0; q < FK_CTAB; ++q) buf[k][q] = 0.0;
+        for (int j = 0; j < nlat; ++j) buf[k][j + 1] = h_tab[(size_t)k * nlat + j];
+        buf[k][0] = buf[k][1]; buf[k][nlat + 1] = buf[k][nlat];
+    }
+    buf[CT_RP][0] = 1.0; buf[CT_RM][nlat + 1] = 1.0;
+    cudaStreamSynchronize(stream);
+    return cudaMemcpyToSymbol(c_tab, buf, sizeof(buf)) == cudaSuccess ? 0 : -1;
 }
 inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
 {
@@ -464,7 +494,7 @@ inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
     {   // keep the per-CTA scratch resident in L2; everything else streams through the rest
         int dev = 0; cudaGetDevice(&dev);
         cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
-        size_t bytes = sizeof(double) * (size_t)fp.nslots * fp.slot_stride;
+        size_t bytes = sizeof(double) * (size_t)fp.nslots_fwd * fp.slot_stride;
         size_t lim = bytes < (size_t)prop.persistingL2CacheMaxSize ? bytes : (size_t)prop.persistingL2CacheMaxSize;
         if (lim > 0 && !getenv("DD4DVAR_NO_L2PIN")) {
             cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, lim);
@@ -485,6 +515,8 @@ inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
     e = cudaFuncSetAttribute(fk_adjoint<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, false));
     if (e != cudaSuccess) return -1;
     e = cudaFuncSetAttribute(fk_adjoint2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_adjoint(fp.maxpy, fp.maxncell, false));
+    if (e != cudaSuccess) return -1;
+    e = cudaFuncSetAttribute(fk_forward2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fp.smem_fwd);
     if (e != cudaSuccess) return -1;
     e = cudaFuncSetAttribute(fk_forward, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fp.smem_fwd);
     return e == cudaSuccess ? 0 : -1;
