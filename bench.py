@@ -111,6 +111,22 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(values, device=None):
+    """Element-wise MAX over all ranks of a list of floats (identity without a process group).
+    This is the only cross-rank step of the benchmark: replicas share no data."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def whole_job_value(units_per_rank, world, seconds):
+    """Weak scaling: every rank processes `units_per_rank`; the job takes the slowest rank's time."""
+    return world * units_per_rank / seconds
+
+
 def workload(cfg):
     if cfg in synth.CONFIGS:
         return synth.CONFIGS[cfg]
@@ -264,10 +280,12 @@ def main():
     torch.cuda.synchronize(dev)
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
-    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms, e2e_s = float(tmax[0]), float(tmax[1])
+    # one outer iteration of Algorithm 1 (a5 L-BFGS + a6 exchange + the sweeps it needs), reported
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    g.run(1)
+    outer_s = time.perf_counter() - t0
+    ms, e2e_s, outer_s = max_over_ranks([ms, e2e_s, outer_s], dev)
 
     if rank == 0:
         ms_step = ms / args.steps
@@ -279,14 +297,16 @@ def main():
             kern, kb, kt = "gradient sweep, all per-stage launches of the generic path", fwd_b + adj_b, ms_step
         achieved = kb / (kt * 1e-3) / 1e9
         line = {
-            "metric": METRIC, "value": world * useful / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "metric": METRIC, "value": whole_job_value(useful, world, ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "counted": "useful = nlon*nlat*nsteps per sweep",
                        "processed_point_steps_per_sweep": pts, "processed_value": world * pts / (ms_step * 1e-3),
                        "subdomains": g.nsub, "path": "fused" if fused else "generic",
                        "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
-                       "parallelism": "replicas" if world > 1 else "single GPU"},
+                       "parallelism": "replicas" if world > 1 else "single GPU",
+                       "outer_iteration_ms": 1e3 * outer_s,
+                       "outer_iteration": "run(1): 5 L-BFGS iterations (a5) + exchange (a6) + J_global, not in the timed region"},
             "clocks": clocks,
             "e2e": {"value": world * useful / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.ctot * 8),
                     "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
