@@ -179,6 +179,48 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: time-to-analysis and grid-point.steps/s per layout on the fixed
+    0.5 deg / 128-step problem (one JSON line per layout; the paper's time-complexity analysis)."""
+    import torch
+    from paper_2205_06649_b200.binding import DD4DVar
+    dev = torch.device("cuda", 0)
+    base = synth.CONFIGS[2]
+    g0 = DD4DVar.from_workload(base.with_layout(1, 1, 1, 0), device="cuda:0")
+    prob = synth.make_problem(base, g0.forecast)
+    g0.close()
+    for w in synth.sweep_workloads():
+        if (w.p_lon, w.p_lat, w.q_time) == (1, 1, 1):
+            w = w.with_layout(1, 1, 1, 0)
+            if any(l.get("layout") == "1x1x1" for l in getattr(run_sweep, "done", [])):
+                continue
+        g = DD4DVar.from_workload(w, device="cuda:0")
+        g.set_background(prob.xb, prob.sigma_b)
+        g.set_observations(prob.obs)
+        for _ in range(3):
+            g.sweep_async(1)
+        torch.cuda.synchronize(dev)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record(); n = 5
+        for _ in range(n):
+            g.sweep_async(1)
+        ev[1].record(); torch.cuda.synchronize(dev)
+        ms = ev[0].elapsed_time(ev[1]) / n
+        outer = args.outer if args.outer is not None else w.outer_iters
+        t0 = time.perf_counter()
+        an, hist = g.run(outer)
+        torch.cuda.synchronize(dev)
+        tta = time.perf_counter() - t0
+        line = {"config": 4, "layout": f"{w.p_lon}x{w.p_lat}x{w.q_time}", "overlap": w.overlap, "subdomains": g.nsub,
+                "path": "fused" if g.active_path == 2 else "generic", "sweep_ms": ms,
+                "useful_point_steps_per_s": w.nlon * w.nlat * w.nsteps / (ms * 1e-3), "outer_iters": outer,
+                "time_to_analysis_s": tta, "J_first": float(hist[0, 0]), "J_last": float(hist[-1, 0]),
+                "delta_last": float(hist[-1, 2])}
+        run_sweep.done = getattr(run_sweep, "done", []) + [line]
+        print(json.dumps(line), flush=True)
+        g.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -188,8 +230,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic kernels, 2 fused kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
+    ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.sweep:
+        run_sweep(args)
+        return
     w = workload(args.config)
     if args.impl == "reference":
         run_reference(args, w)
