@@ -339,7 +339,7 @@ def main():
         peak, peak_src = peaks()
         fused = g.active_path == 2
         if fused:
-            kern, kb, kt = "fk_adjoint (fused adjoint sweep, one launch per gradient sweep)", adj_b, t_a
+            kern, kb, kt = "fk_adjoint2 (fused adjoint sweep, one launch per gradient sweep)", adj_b, t_a
         else:
             kern, kb, kt = "gradient sweep, all per-stage launches of the generic path", fwd_b + adj_b, ms_step
         achieved = kb / (kt * 1e-3) / 1e9

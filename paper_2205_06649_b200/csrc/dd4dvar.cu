@@ -316,11 +316,7 @@ void ensure_tables(dd4dvar_t h)
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
     if (L.path == 2) {
-        if (L.fp.lam_smem)
-            fk_adjoint<true><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
-                L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
-                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
-        else if (!getenv("DD4DVAR_ADJ1")) {
+        {
             ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
             fk_adjoint2<<<L.fp.nslots, FK_NT, L.fp.smem_adj, h->stream>>>(
@@ -328,10 +324,6 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
                 L.fp.slot_stride, L.fp.counter);
         }
-        else
-            fk_adjoint<false><<<L.nsub, FK_NT, L.fp.smem_adj, h->stream>>>(
-                L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
-                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw);
         ++h->launches;
         return;
     }
@@ -339,14 +331,11 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 }
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
-    if (L.path == 2 && !getenv("DD4DVAR_FWD1")) {
+    if (L.path == 2) {
         ensure_tables(h);
         cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
         fk_forward2<<<L.fp.nslots_fwd, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
                                                                       L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
-        ++h->launches;
-    } else if (L.path == 2) {
-        fk_forward<<<L.nsub, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost);
         ++h->launches;
     } else forward_generic(h, L, mask);
     cost_generic(h, L, mask, Jout);
@@ -438,10 +427,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
     h->L.path = (h->opt.path == 1 || !fits) ? 1 : 2;
     fused_plan_init(h->G.fp, nullptr, 0, 0);
-    {
-        const char* e = getenv("DD4DVAR_LAM");      // tuning knob: 1 = adjoint variable in global memory, 2 = shared
-        fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, e ? atoi(e) : 0);
-    }
+    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, 0);
     h->ws_bytes = plan_all(h, nullptr);
     *out = h;
     return 0;

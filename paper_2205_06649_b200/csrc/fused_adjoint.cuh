@@ -175,7 +175,6 @@ __global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ 
                                                         int nsub, double* scratch, long long slot_stride,
                                                         int* counter)
 {
-    extern __shared__ double dsm[];
     __shared__ int s_next;
     __shared__ double zr[FK_ZR * 3 * FK_NT];
     __shared__ double uas[4 * FK_NT];

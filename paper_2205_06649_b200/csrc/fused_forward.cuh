@@ -95,7 +95,6 @@ __global__ void __launch_bounds__(FK_NT, 4) fk_forward2(const Sub* __restrict__ 
                                                         const double* ghost, int nsub, double* scratch,
                                                         long long slot_stride, int* counter)
 {
-    extern __shared__ double dsm[];
     __shared__ double z0s[2 * 3 * FK_NT];
     __shared__ double uas[2 * FK_NT];
     __shared__ double h1s[2 * FK_NT];
