@@ -319,7 +319,11 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
         {
             ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
-            fk_adjoint2<<<L.fp.nslots, FK_NT, L.fp.smem_adj, h->stream>>>(
+            if (L.fp.nt == 64) fk64::fk_adjoint2<<<L.fp.nslots, 64, 0, h->stream>>>(
+                L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
+                L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
+                L.fp.slot_stride, L.fp.counter);
+            else fk128::fk_adjoint2<<<L.fp.nslots, 128, 0, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
                 L.fp.slot_stride, L.fp.counter);
@@ -334,7 +338,9 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
     if (L.path == 2) {
         ensure_tables(h);
         cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
-        fk_forward2<<<L.fp.nslots_fwd, FK_NT, L.fp.smem_fwd, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
+        if (L.fp.nt == 64) fk64::fk_forward2<<<L.fp.nslots_fwd, 64, 0, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
+                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
+        else fk128::fk_forward2<<<L.fp.nslots_fwd, 128, 0, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
                                                                       L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
         ++h->launches;
     } else forward_generic(h, L, mask);

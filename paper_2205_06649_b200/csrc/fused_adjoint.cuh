@@ -8,9 +8,7 @@
 // (v-like quantities negated), written once per step under a uniform branch, so the stage code has
 // no wall selects.  For P the mirror carries the metric ratio: P[-1] = r-_0 P[0], r+_{-1} := 1,
 // P[py] = r+_{py-1} P[py-1], r-_{py} := 1 (see model_math.cuh, A_v).
-#pragma once
-#include "common.cuh"
-#include "model_math.cuh"
+// (included once per CTA width from fused_kernels.cuh, inside a namespace; FK_NT = threads per CTA)
 
 struct AdjRegs {
     double z[4][3];                 // Z0 rows, slot = row & 3
@@ -162,7 +160,7 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
 }
 
 // adjoint sweep of one window (static-slot version); same contract as fk_adjoint<false>
-__global__ void __launch_bounds__(FK_NT, 3) fk_adjoint2(const Sub* __restrict__ subs, const int* __restrict__ mask,
+__global__ void __launch_bounds__(FK_NT, 384 / FK_NT) fk_adjoint2(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                         ModelP m, CostP cp, GeoP geo, const double* __restrict__ x,
                                                         const double* __restrict__ xbs,
                                                         const double* __restrict__ xfrozen,

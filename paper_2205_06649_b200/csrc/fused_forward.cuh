@@ -4,9 +4,7 @@
 // The current state of the window lives IN PLACE in this CTA's slot of the L2-pinned scratch (row j
 // of level n+1 overwrites row j of level n three ticks after the same thread read it), so HBM only
 // sees the trajectory store being written (streaming stores) and the frozen ghost ring being read.
-#pragma once
-#include "common.cuh"
-#include "model_math.cuh"
+// (included once per CTA width from fused_kernels.cuh, inside a namespace; FK_NT = threads per CTA)
 
 struct FwdRegs {
     double z[4][3];
@@ -90,7 +88,7 @@ __device__ __forceinline__ void fwd_tick(const int t, FwdRegs& R, const FwdCtx& 
 #undef S2
 }
 
-__global__ void __launch_bounds__(FK_NT, 4) fk_forward2(const Sub* __restrict__ subs, const int* __restrict__ mask,
+__global__ void __launch_bounds__(FK_NT, 512 / FK_NT) fk_forward2(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                         ModelP m, const double* __restrict__ x, double* traj,
                                                         const double* ghost, int nsub, double* scratch,
                                                         long long slot_stride, int* counter)

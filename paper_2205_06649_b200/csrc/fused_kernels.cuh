@@ -21,7 +21,7 @@
 #include "common.cuh"
 #include "model_math.cuh"
 
-#define FK_NT 128          // threads per CTA = maximum padded tile width
+#define FK_MAXNT 128       // widest padded tile the fused kernels take (threads per CTA: 64 or 128)
 #define FK_ZR 8            // depth of the Z0 row ring (adjoint reads rows t-5 .. t)
 
 struct FusedPlan {
@@ -29,19 +29,19 @@ struct FusedPlan {
     int maxpy = 0, maxncell = 0;
     size_t smem_fwd = 0, smem_adj = 0;
     // persistent CTAs: one L2-persistent scratch slot per resident CTA (in-place state / adjoint variable)
+    int nt = 128;                     // threads per CTA (64 for narrow tiles)
     int nslots = 0, nslots_fwd = 0;
     long long slot_stride = 0;        // doubles
     double* scratch = nullptr;
     int* counter = nullptr;
 };
-#define FK_SLOTS (148 * 3)          // B200: 148 SMs x 3 resident CTAs (adjoint)
-#define FK_SLOTS_FWD (148 * 4)      // forward kernel: 4 resident CTAs per SM
+#define FK_SMS 148                  // B200
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
 inline bool fused_fits(const Sub* subs, int nsub)
 {
     for (int k = 0; k < nsub; ++k)
-        if (subs[k].px > FK_NT || subs[k].py < 1) return false;
+        if (subs[k].px > FK_MAXNT || subs[k].py < 1) return false;
     return nsub > 0;
 }
 inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mode);
@@ -122,8 +122,20 @@ __constant__ double c_tab[6][FK_CTAB];
 #define CT_RM 5
 __device__ __forceinline__ double ctab(int k, int cj, int j) { return c_tab[k][cj + j]; }
 
+// the kernels are instantiated for CTAs of 128 threads (tiles up to 128 padded columns) and of 64
+// threads (narrow tiles, e.g. the 16x16x8 layout of config 4: 55 columns)
+#define FK_NT 128
+namespace fk128 {
 #include "fused_adjoint.cuh"
 #include "fused_forward.cuh"
+}
+#undef FK_NT
+#define FK_NT 64
+namespace fk64 {
+#include "fused_adjoint.cuh"
+#include "fused_forward.cuh"
+}
+#undef FK_NT
 
 inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mode)
 {
@@ -134,8 +146,12 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
         fp.maxpy = subs[k].py > fp.maxpy ? subs[k].py : fp.maxpy;
         fp.maxncell = subs[k].ncell > fp.maxncell ? subs[k].ncell : fp.maxncell;
     }
-    fp.nslots = nsub < FK_SLOTS ? nsub : FK_SLOTS;
-    fp.nslots_fwd = nsub < FK_SLOTS_FWD ? nsub : FK_SLOTS_FWD;
+    int maxpx = 0;
+    for (int k = 0; k < nsub; ++k) maxpx = subs[k].px > maxpx ? subs[k].px : maxpx;
+    fp.nt = maxpx <= 64 ? 64 : 128;
+    const int sa = FK_SMS * (384 / fp.nt), sf = FK_SMS * (512 / fp.nt);   // resident CTAs: adjoint, forward
+    fp.nslots = nsub < sa ? nsub : sa;
+    fp.nslots_fwd = nsub < sf ? nsub : sf;
     fp.slot_stride = (3LL * fp.maxncell + 31) & ~31LL;
     fp.smem_fwd = 0;
     fp.smem_adj = 0;
