@@ -728,7 +728,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         sweep(h, L, true, nullptr, L.st.J, L.g);
         if (l == 1 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
         for (int it = 0; it < h->opt.n_inner; ++it) {
-            LAUNCH(lk_direction<NT_LB>, nsub, NT_LB, L.dsubs, lp, L.st, L.g, L.S, L.Y, L.d);
+            LAUNCH(lk_direction<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.g, L.S, L.Y, L.d);
             for (int b = 0; b <= lp.max_bt; ++b) {
                 CU(cudaMemsetAsync(L.st.nactive, 0, sizeof(int), h->stream));
                 LAUNCH(lk_trial, vgrid, 256, L.dsubs, L.st.active, h->cp, L.st.t, L.w, L.d, L.xbs, L.wt, L.x);
@@ -741,7 +741,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
             }
             // gradient at the accepted points (their trajectories are still in the store)
             adjoint_only(h, L, L.st.ok, L.gn);
-            LAUNCH(lk_update<NT_LB>, nsub, NT_LB, L.dsubs, lp, L.st, L.w, L.wt, L.g, L.gn, L.S, L.Y);
+            LAUNCH(lk_update<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.w, L.wt, L.g, L.gn, L.S, L.Y);
         }
         // one more forward sweep so that the stored trajectory belongs to the accepted iterate
         LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,

@@ -139,3 +139,52 @@ def test_errors_are_reported_not_thrown():
     with pytest.raises(DD4DVarError) as e:
         g.set_background(np.zeros((3, 18, 36)), [1.0, -1.0, 1.0])
     assert e.value.code == -1
+
+
+def test_edge_cases_no_observations_zero_inner_single_step_window():
+    """Degenerate inputs: no observations at all; n_inner = 0 (the outer loop only exchanges);
+    windows of a single step (q_time = nsteps); one observation level only."""
+    from oracle import Oracle
+    from paper_2205_06649_b200.binding import DD4DVar
+    w = small_workload(nsteps=4, q_time=4, obs_every=4)
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    check_eval_local(o, g, perturbed_controls(o, prob, 3))
+    an_o, h_o = o.run(2); an_g, h_g = g.run(2)
+    assert rel(an_g.cpu().numpy(), an_o) <= TOL_AN
+    # no observations: J = background + overlap terms only
+    w2 = small_workload()
+    o2 = Oracle.from_workload(w2); t0 = synth.truth_initial(w2); sb, _ = synth.sigmas(t0)
+    xb = synth.background(w2, t0, sb)
+    o2.set_background(xb, sb)
+    g2 = DD4DVar.from_workload(w2); g2.set_background(xb, sb)
+    xs = [o2.get_control(k) + 0.3 * sb[:, None, None] * synth.random_fields(o2.sub_shape(k), 9 + k) for k in range(o2.nsub)]
+    costs, parts, grads = g2.eval_local(g2.pack(xs))
+    assert np.all(parts[:, 1] == 0.0)
+    for k in range(o2.nsub):
+        po, go, _ = o2.eval_local(k, xs[k])
+        assert abs(costs[k] - po[0]) <= TOL_EVAL * abs(po[0])
+        assert rel(g2.split(grads)[k].cpu().numpy(), go) <= TOL_EVAL
+    # n_inner = 0: controls do not move, history rows repeat
+    o3, prob3 = oracle_problem(w2, n_inner=0)
+    g3 = gpu_problem(w2, prob3, n_inner=0)
+    an_o, h_o = o3.run(2); an_g, h_g = g3.run(2)
+    assert rel(an_g.cpu().numpy(), an_o) <= 1e-14 and h_g[2, 2] == 0.0
+    assert np.all(np.abs(h_g[:, :2] - h_o[:, :2]) <= 1e-10 * np.abs(h_o[:, :2]))
+
+
+def test_observation_input_validation():
+    from paper_2205_06649_b200.binding import DD4DVarError
+    w = small_workload()
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    import copy
+    bad = copy.deepcopy(prob.obs)
+    bad.index = bad.index.copy(); bad.index[1] = bad.index[0]          # not strictly ascending
+    with pytest.raises(DD4DVarError) as e:
+        g.set_observations(bad)
+    assert e.value.code == -1
+    bad = copy.deepcopy(prob.obs); bad.levels = bad.levels.copy(); bad.levels[-1] = w.nsteps + 1
+    with pytest.raises(DD4DVarError) as e:
+        g.set_observations(bad)
+    assert e.value.code == -1
