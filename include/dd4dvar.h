@@ -67,8 +67,9 @@ typedef struct {
 
 /* Local minimiser (L-BFGS, R10): history length, iterations per outer iteration,
  * maximum number of step halvings, Armijo constant.
- * path: 0 = choose automatically, 1 = force the generic (per-step, global-memory) kernels,
- *       2 = force the fused persistent kernels (create fails with -2 if a tile does not fit). */
+ * path: 0 = choose automatically, 1 = force the generic kernels (one block-tiled launch per step,
+ *       any tile size), 2 = force the fused persistent kernels (create fails with -2 if a tile
+ *       does not fit), 3 = force the per-stage generic kernels (cross-check). */
 typedef struct {
     int lbfgs_m, n_inner, max_backtrack;
     double armijo_c1;

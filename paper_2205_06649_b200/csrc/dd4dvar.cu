@@ -17,6 +17,7 @@
 #include "fused_kernels.cuh"
 #include "generic_kernels.cuh"
 #include "lbfgs_kernels.cuh"
+#include "step_kernels.cuh"
 
 namespace {
 
@@ -41,7 +42,8 @@ void* ar_take_bytes(void* arena, size_t bytes) { return static_cast<Arena*>(aren
 struct Layout {
     int p1 = 1, p2 = 1, q = 1, o = 0, nsub = 0;
     bool lbfgs = false;
-    int path = 1;                       // 1 generic, 2 fused
+    int path = 1;                       // 1 generic (block-tiled step kernels), 2 fused, 3 generic per-stage kernels
+    int tiles_x = 1, ntiles = 1;        // 32x16 output tiles of the step kernels
     std::vector<Sub> hs;
     std::vector<int> colown, rowown, ncolcov, colcov, nrowcov, rowcov, tc_ei0, tc_ex, tr_ej0, tr_ey, wb;
     long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0;
@@ -185,6 +187,11 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
                 L.maxnpad = std::max(L.maxnpad, s.npad); L.maxncell = std::max(L.maxncell, s.ncell);
                 L.maxnring = std::max(L.maxnring, s.nring); L.Wmax = std::max(L.Wmax, s.W);
             }
+    {
+        int mex = 0, mey = 0;
+        for (const Sub& q : L.hs) { mex = std::max(mex, q.ex); mey = std::max(mey, q.ey); }
+        L.tiles_x = (mex + SK_TX - 1) / SK_TX; L.ntiles = L.tiles_x * ((mey + SK_TY - 1) / SK_TY);
+    }
     L.CB = std::min(64, std::max(1, (3 * L.maxncell + NT_RED * 32 - 1) / (NT_RED * 32)));
     return 0;
 }
@@ -266,6 +273,11 @@ void forward_generic(dd4dvar_t h, Layout& L, const int* mask)
 {
     // level 0 of the store = the control
     LAUNCH(gk_store_control, cell_grid(L), NT_GK, L.dsubs, mask, L.x, L.traj);
+    if (L.path != 3) {
+        for (int n = 0; n < L.Wmax; ++n)
+            LAUNCH(sk_forward_step, dim3(L.ntiles, L.nsub), SK_NT, L.dsubs, mask, n, h->mp, L.traj, L.ghost, L.tiles_x);
+        return;
+    }
     for (int n = 0; n < L.Wmax; ++n) {
         LAUNCH(gk_fill_pad, pad_grid(L), NT_GK, L.dsubs, mask, n, L.traj, L.ghost, L.Zp);
         LAUNCH(gk_stageA, pad_grid(L), NT_GK, L.dsubs, mask, n, h->mp, L.Zp, L.Za);
@@ -291,7 +303,11 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
         if (L.have_obs)
             LAUNCH(gk_obs_force, dim3(4, L.nsub), NT_GK, L.dsubs, mask, n, L.obs_start, L.obs_idx, L.obs_y,
                    L.obs_c, L.traj, cur);
-        if (n > 0) {
+        if (n > 0 && L.path != 3) {
+            sk_adjoint_step<<<dim3(L.ntiles, L.nsub), SK_NT, sizeof(double) * SK_ADJ_SMEM_DOUBLES, h->stream>>>(
+                L.dsubs, mask, n - 1, h->mp, L.traj, L.ghost, cur, nxt, L.tiles_x);
+            ++h->launches;
+        } else if (n > 0) {
             LAUNCH(gk_fill_pad, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, L.traj, L.ghost, L.Zp);
             LAUNCH(gk_stageA, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Zp, L.Za);
             LAUNCH(gk_adjHB, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Za, cur, L.traj, L.HB, L.P, L.UB);
@@ -431,7 +447,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     h->G.path = 1;
     const bool fits = fused_fits(h->L.hs.data(), h->L.nsub) && nlat + 2 <= FK_CTAB;
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
-    h->L.path = (h->opt.path == 1 || !fits) ? 1 : 2;
+    h->L.path = h->opt.path == 3 ? 3 : ((h->opt.path == 1 || !fits) ? 1 : 2);
     fused_plan_init(h->G.fp, nullptr, 0, 0);
     fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, 0);
     h->ws_bytes = plan_all(h, nullptr);
@@ -458,6 +474,9 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
     if (rc) return rc;
     rc = upload_layout(h, h->L);
     if (rc) return rc;
+    if (cudaFuncSetAttribute(sk_adjoint_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(sizeof(double) * SK_ADJ_SMEM_DOUBLES)) != cudaSuccess)
+        return fail(h, -4, "shared-memory opt-in of sk_adjoint_step failed");
     rc = fused_setup(h->stream, h->L.fp, h->L.dsubs);
     if (rc) return fail(h, -4, "fused kernel setup failed (shared-memory opt-in)");
     h->have_ws = true; h->have_bg = false; h->G.have_obs = h->L.have_obs = false;

@@ -23,7 +23,7 @@ LAYOUTS = {
     "time_only": dict(p_lon=1, p_lat=1, q_time=4, overlap=0),
     "cols4x1x1_o1": dict(nlon=48, nlat=12, nsteps=6, p_lon=4, p_lat=1, q_time=1, overlap=1),
 }
-PATHS = [1, 2]
+PATHS = [1, 2, 3]
 
 
 def make_pair(name, path):
