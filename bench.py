@@ -111,6 +111,16 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def measured_traffic(kernel, cfg):
+    """DRAM bytes per launch of `kernel` from the committed ncu capture (config 3 only), else None."""
+    try:
+        if cfg != 3:
+            return None
+        return int(json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[kernel])
+    except Exception:
+        return None
+
+
 def max_over_ranks(values, device=None):
     """Element-wise MAX over all ranks of a list of floats (identity without a process group).
     This is the only cross-rank step of the benchmark: replicas share no data."""
@@ -359,7 +369,7 @@ def main():
                     "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": kern, "peak_source": peak_src,
+                         "traffic": measured_traffic("fk_adjoint2", args.config) if fused else None, "kernel": kern, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb, "kernel_ms": kt,
                          "sweep_algorithmic_GBps": (fwd_b + adj_b) / (ms_step * 1e-3) / 1e9,
                          "forward_ms": t_f, "adjoint_ms": t_a,
