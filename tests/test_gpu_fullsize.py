@@ -82,3 +82,25 @@ def test_config3_sampled_subdomains_and_invariants():
             assert abs(parts[k, q] - po[1 + q]) <= TOL_EVAL * abs(po[0]), (k, q)
         assert rel(gl[k].cpu().numpy(), go) <= TOL_EVAL, (k, rel(gl[k].cpu().numpy(), go))
         assert rel(g.get_local_trajectory(k).cpu().numpy(), tr) <= 1e-12, k
+
+
+def test_config4_large_tile_layout_follows_the_oracle_iteration():
+    """Config 4, layout 2x2x2 overlap 1 on the 0.5 deg problem (tiles 362x181: generic step
+    kernels, many 32x16 blocks per tile): cost / gradient of every subdomain and the history of the
+    first two outer iterations equal the oracle's (this layout's J_global rises - both sides agree)."""
+    w = synth.CONFIGS[2].with_layout(2, 2, 2, 1)
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    assert g.active_path == 1 and g.nsub == 8
+    xs = perturbed(o, prob, range(o.nsub), 41)
+    costs, parts, grads = g.eval_local(g.pack([xs[k] for k in range(o.nsub)]))
+    gl = g.split(grads)
+    for k in range(o.nsub):
+        po, go, _ = o.eval_local(k, xs[k])
+        assert abs(costs[k] - po[0]) <= TOL_EVAL * abs(po[0]), k
+        assert rel(gl[k].cpu().numpy(), go) <= TOL_EVAL, k
+    an_o, hist_o = o.run(2)
+    an_g, hist_g = g.run(2)
+    assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2]))
+    for f in range(3):
+        assert rel(an_g.cpu().numpy()[f], an_o[f]) <= TOL_AN
