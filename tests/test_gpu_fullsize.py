@@ -104,3 +104,26 @@ def test_config4_large_tile_layout_follows_the_oracle_iteration():
     assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2]))
     for f in range(3):
         assert rel(an_g.cpu().numpy()[f], an_o[f]) <= TOL_AN
+
+
+def test_config2_one_outer_iteration():
+    """Config 2 (0.5 deg, 8x8x8 = 512 subdomains, wavenumber-4 perturbation): one outer iteration
+    of Algorithm 1 against the oracle, and sampled evaluations with the exchanged data."""
+    w = synth.CONFIGS[2]
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    assert g.active_path == 2 and g.nsub == 512
+    an_o, hist_o = o.run(1)
+    an_g, hist_g = g.run(1)
+    an_g = an_g.cpu().numpy()
+    for f in range(3):
+        assert rel(an_g[f], an_o[f]) <= TOL_AN, f
+    assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2]))
+    assert abs(hist_g[1, 2] - hist_o[1, 2]) <= 1e-6 * hist_o[1, 2]
+    sample = [0, 63, 64 * 3 + 27, 64 * 7 + 63]
+    ctr = g.get_controls()
+    costs, parts, grads = g.eval_local(ctr)
+    for k in sample:
+        po, go, _ = o.eval_local(k, o.get_control(k))
+        assert abs(costs[k] - po[0]) <= 1e-8 * abs(po[0]), k
+        assert rel(g.split(grads)[k].cpu().numpy(), go) <= 1e-8, k
