@@ -189,6 +189,28 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def run_driver(args):
+    """Time to analysis of Algorithm 1 on one config: run(outer_iters), cost history, RMSE vs truth."""
+    import torch
+    from paper_2205_06649_b200.binding import DD4DVar
+    w = workload(args.config)
+    g = DD4DVar.from_workload(w, path=args.path)
+    prob = synth.make_problem(w, g.forecast)
+    g.set_background(prob.xb, prob.sigma_b); g.set_observations(prob.obs)
+    outer = args.outer if args.outer is not None else w.outer_iters
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    an, hist = g.run(outer)
+    torch.cuda.synchronize(); dt = time.perf_counter() - t0
+    an = an.cpu().numpy()
+    rm = lambda a, b: float(np.sqrt(np.mean((a - b) ** 2)))
+    print(json.dumps({"config": args.config, "workload": w.name, "outer_iters": outer, "time_to_analysis_s": dt,
+                      "launches": int(g.launch_count), "J_global": [float(x) for x in hist[:, 0]],
+                      "sumJ_local": [float(x) for x in hist[:, 1]], "delta": [float(x) for x in hist[:, 2]],
+                      "rmse_background_h_u_v": [rm(prob.xb[f], prob.truth0[f]) for f in range(3)],
+                      "rmse_analysis_h_u_v": [rm(an[f], prob.truth0[f]) for f in range(3)]}))
+    g.close()
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: time-to-analysis and grid-point.steps/s per layout on the fixed
     0.5 deg / 128-step problem (one JSON line per layout; the paper's time-complexity analysis)."""
@@ -240,12 +262,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic kernels, 2 fused kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
     ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
         run_sweep(args)
+        return
+    if args.run:
+        run_driver(args)
         return
     w = workload(args.config)
     if args.impl == "reference":
