@@ -188,3 +188,25 @@ def test_observation_input_validation():
     with pytest.raises(DD4DVarError) as e:
         g.set_observations(bad)
     assert e.value.code == -1
+
+
+def test_violent_regime_large_background_noise_many_backtracks():
+    """Background noise 8x the recipe's (sigma_b(h) ~ 140 m, winds ~ 6 m/s): strongly nonlinear, the
+    line search halves several times; the GPU must follow the oracle's branches."""
+    from oracle import Oracle
+    w = small_workload(outer=3)
+    o = Oracle.from_workload(w)
+    t0 = synth.truth_initial(w)
+    sb, so = synth.sigmas(t0)
+    sb = 8.0 * sb
+    prob = synth.Problem(w, t0, synth.background(w, t0, sb), sb, so)
+    prob.obs = synth.make_observations(w, o.forecast(t0, synth.obs_levels(w)), so)
+    o.set_background(prob.xb, prob.sigma_b); o.set_observations(prob.obs)
+    an_o, hist_o = o.run(3)
+    for path in (1, 2):
+        g = gpu_problem(w, prob, path=path)
+        an_g, hist_g = g.run(3)
+        an_g = an_g.cpu().numpy()
+        for f in range(3):
+            assert rel(an_g[f] - prob.xb[f], an_o[f] - prob.xb[f]) <= 1e-6, (path, f)
+        assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2])), (hist_g, hist_o)
