@@ -210,3 +210,32 @@ def test_violent_regime_large_background_noise_many_backtracks():
         for f in range(3):
             assert rel(an_g[f] - prob.xb[f], an_o[f] - prob.xb[f]) <= 1e-6, (path, f)
         assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2])), (hist_g, hist_o)
+
+
+@pytest.mark.parametrize("path", [1, 2])
+def test_gpu_gradient_vs_centred_finite_differences_of_gpu_costs(path):
+    """Independent of the oracle: the CUDA adjoint sweep differentiates the CUDA forward sweep.
+    Directional derivatives of sum_k J_k along random directions (all subdomains at once; frozen
+    neighbour data do not move, so the sum's gradient is the concatenation of the local gradients)."""
+    w = small_workload(**LAYOUTS["ragged3x2x3_o2"])
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob, path=path)
+    import torch
+    x = g.pack(perturbed_controls(o, prob, 21, amp=0.3))
+    costs, _, grads = g.eval_local(x)
+    sb = np.concatenate([np.repeat(prob.sigma_b, np.prod(g.sub_shape(k)[1:])) for k in range(g.nsub)])
+    scale = torch.zeros_like(x)
+    for k in range(g.nsub):
+        n = int(np.prod(g.sub_shape(k)))
+        scale[g.offsets[k]:g.offsets[k] + n] = torch.as_tensor(
+            np.repeat(prob.sigma_b, n // 3), device=x.device)
+    J0 = costs.sum()
+    for seed in range(4):
+        gen = torch.Generator(device="cpu").manual_seed(100 + seed)
+        d = (torch.randn(x.numel(), generator=gen, dtype=torch.float64).to(x.device)) * scale
+        h = 1e-5
+        Jp = g.eval_local(x + h * d, want_grad=False)[0].sum()
+        Jm = g.eval_local(x - h * d, want_grad=False)[0].sum()
+        fd = (Jp - Jm) / (2 * h)
+        an = float((grads * d).sum())
+        assert abs(fd - an) <= 2e-7 * abs(an) + 8 * 2.2e-16 * J0 / h, (seed, fd, an)
