@@ -160,7 +160,7 @@ __device__ __forceinline__ void adj_tick(const int t, const int h, AdjRegs& R, c
 }
 
 // adjoint sweep of one window (static-slot version); same contract as fk_adjoint<false>
-__global__ void __launch_bounds__(FK_NT, 384 / FK_NT) fk_adjoint2(const Sub* __restrict__ subs, const int* __restrict__ mask,
+__global__ void __launch_bounds__(FK_NT, FK_ADJ_CTAS * 128 / FK_NT) fk_adjoint2(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                         ModelP m, CostP cp, GeoP geo, const double* __restrict__ x,
                                                         const double* __restrict__ xbs,
                                                         const double* __restrict__ xfrozen,

@@ -36,6 +36,9 @@ struct FusedPlan {
     int* counter = nullptr;
 };
 #define FK_SMS 148                  // B200
+#ifndef FK_ADJ_CTAS
+#define FK_ADJ_CTAS 3                // resident adjoint CTAs per SM at 128 threads (register budget 168)
+#endif
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
 inline bool fused_fits(const Sub* subs, int nsub)
@@ -149,7 +152,7 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
     int maxpx = 0;
     for (int k = 0; k < nsub; ++k) maxpx = subs[k].px > maxpx ? subs[k].px : maxpx;
     fp.nt = maxpx <= 64 ? 64 : 128;
-    const int sa = FK_SMS * (384 / fp.nt), sf = FK_SMS * (512 / fp.nt);   // resident CTAs: adjoint, forward
+    const int sa = FK_SMS * (FK_ADJ_CTAS * 128 / fp.nt), sf = FK_SMS * (512 / fp.nt);   // resident CTAs: adjoint, forward
     fp.nslots = nsub < sa ? nsub : sa;
     fp.nslots_fwd = nsub < sf ? nsub : sf;
     fp.slot_stride = (3LL * fp.maxncell + 31) & ~31LL;
