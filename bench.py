@@ -401,7 +401,7 @@ def main():
                          "forward_ms": t_f, "adjoint_ms": t_a,
                          "bytes_per_processed_point_step": (fwd_b + adj_b) / pts},
         }
-        if not args.no_cpu_baseline and world >= 1:
+        if not args.no_cpu_baseline and world == 1:
             t0 = time.perf_counter()
             o, k1 = oracle_sweep_sample(w)
             t1 = time.perf_counter()
