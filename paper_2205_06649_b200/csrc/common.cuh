@@ -21,6 +21,7 @@ struct Sub {
     long long goff;          // offset in the ghost store [W][3][nring]
     long long poff;          // offset in padded scratch arrays [3][npad] (single-field: poff/3)
     long long ooff;          // index into obs_start: entries ooff .. ooff+W+1
+    long long eoff;          // offset in the edge store [W][py][2] (frozen u^a of ghost columns 1, px-2)
 };
 
 // Model constants with dt folded in (row tables live in device memory, length nlat).

@@ -18,6 +18,7 @@
 #include "generic_kernels.cuh"
 #include "lbfgs_kernels.cuh"
 #include "step_kernels.cuh"
+#include "wave_forward.cuh"
 
 namespace {
 
@@ -39,21 +40,29 @@ struct Arena {
 
 void* ar_take_bytes(void* arena, size_t bytes) { return static_cast<Arena*>(arena)->take<char>(bytes); }
 
+// plan of the wavefront kernels (wave_common.cuh) for one layout
+struct WavePlan {
+    int enabled = 0, K = 3, grid = 0;
+    int maxex = 0, maxey = 0, maxpx = 0, maxpy = 0;
+    size_t smem_fwd = 0, smem_adj = 0;
+    int* counter = nullptr;
+};
+
 struct Layout {
     int p1 = 1, p2 = 1, q = 1, o = 0, nsub = 0;
     bool lbfgs = false;
-    int path = 1;                       // 1 generic (block-tiled step kernels), 2 fused, 3 generic per-stage kernels
+    int path = 1;                       // 1 generic (block-tiled step kernels), 2 fused row-marching, 3 generic per-stage kernels, 4 wavefront
     int tiles_x = 1, ntiles = 1;        // 32x16 output tiles of the step kernels
     std::vector<Sub> hs;
     std::vector<int> colown, rowown, ncolcov, colcov, nrowcov, rowcov, tc_ei0, tc_ex, tr_ej0, tr_ey, wb;
-    long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0;
+    long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0, etot = 0;
     int maxnpad = 0, maxncell = 0, maxnring = 0, Wmax = 0, CB = 1, maxcov = 1;
     // device
     Sub* dsubs = nullptr;
     GeoP geo{};
     int* itab = nullptr;
     double *x = nullptr, *xbs = nullptr, *xfrozen = nullptr, *pred_end = nullptr, *gx = nullptr;
-    double *traj = nullptr, *ghost = nullptr;
+    double *traj = nullptr, *ghost = nullptr, *gedge = nullptr;
     double *Zp = nullptr, *Za = nullptr, *lamA = nullptr, *lamB = nullptr, *A = nullptr;
     double *H1 = nullptr, *HB = nullptr, *P = nullptr, *UB = nullptr;
     double *partial = nullptr, *parts = nullptr, *Jev = nullptr, *dmax = nullptr;
@@ -64,8 +73,10 @@ struct Layout {
     bool have_obs = false;
     long long* obs_start = nullptr;
     int* obs_idx = nullptr;
-    double *obs_y = nullptr, *obs_c = nullptr;
+    int* obs_lj = nullptr;
+    double *obs_y = nullptr, *obs_c = nullptr, *obs_r = nullptr;
     FusedPlan fp{};
+    WavePlan wp{};
 };
 
 }  // namespace
@@ -163,7 +174,7 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
     for (int v : L.nrowcov) mr = std::max(mr, v);
     L.maxcov = mc * mr;
     L.hs.resize(L.nsub);
-    L.ctot = L.ttot = L.gtot = L.ptot1 = L.otot = 0;
+    L.ctot = L.ttot = L.gtot = L.ptot1 = L.otot = L.etot = 0;
     L.maxnpad = L.maxncell = L.maxnring = L.Wmax = 0;
     for (int jw = 0; jw < q; ++jw)
         for (int b = 0; b < p2; ++b)
@@ -178,6 +189,7 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
                 if (s.W < 1) return -2;
                 s.ncell = s.ex * s.ey; s.npad = s.px * s.py; s.nring = s.npad - s.ncell;
                 s.coff = L.ctot; s.toff = L.ttot; s.goff = L.gtot; s.poff = 3 * L.ptot1; s.ooff = L.otot;
+                s.eoff = L.etot; L.etot += (long long)s.W * 2 * s.py;
                 // keep every plane 16-byte aligned relative to 256-byte aligned array bases
                 L.ctot += 3LL * s.ncell; L.ctot = (L.ctot + 1) & ~1LL;
                 L.ttot += (long long)(s.W + 1) * 3 * s.ncell; L.ttot = (L.ttot + 1) & ~1LL;
@@ -229,6 +241,31 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
         L.st.nactive = ar.take<int>(4);
     }
     fused_plan_arrays(L.fp, ar_take_bytes, &ar);
+    if (L.wp.enabled) {
+        L.gedge = ar.take<double>(std::max<long long>(L.etot, 2));
+        L.wp.counter = ar.take<int>(16);
+    }
+}
+
+// eligibility and shared-memory budget of the wavefront kernels (wave_common.cuh)
+void wave_plan_init(WavePlan& wp, const Sub* subs, int nsub)
+{
+    wp = WavePlan();
+    if (!subs || nsub <= 0) return;
+    for (int k = 0; k < nsub; ++k) {
+        const Sub& s = subs[k];
+        if (s.gx != DD_GHOST || (s.ex & 1) || s.ey > 1000 || s.ex < 2) return;
+        if ((s.gys != 0 && s.gys != DD_GHOST) || (s.gyn != 0 && s.gyn != DD_GHOST)) return;
+        wp.maxex = std::max(wp.maxex, s.ex); wp.maxey = std::max(wp.maxey, s.ey);
+        wp.maxpx = std::max(wp.maxpx, s.px); wp.maxpy = std::max(wp.maxpy, s.py);
+    }
+    if (wp.maxpx - 4 <= 64) wp.K = 2;
+    else if (wp.maxpx - 4 <= 96) wp.K = 3;
+    else return;
+    wp.smem_fwd = sizeof(double) * (size_t)wk_layout(false, wp.maxex, wp.maxey, wp.maxpx, wp.maxpy).total;
+    wp.smem_adj = sizeof(double) * (size_t)wk_layout(true, wp.maxex, wp.maxey, wp.maxpx, wp.maxpy).total;
+    if (wp.smem_fwd > WK_SMEM_MAX || wp.smem_adj > WK_SMEM_MAX) return;
+    wp.enabled = 1;
 }
 
 int upload_layout(dd4dvar_t h, Layout& L)
@@ -328,10 +365,24 @@ void ensure_tables(dd4dvar_t h)
     g_ctab_owner = h;
 }
 
+WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* gw)
+{
+    WkArgs a;
+    a.subs = L.dsubs; a.mask = mask; a.nsub = L.nsub; a.counter = L.wp.counter;
+    a.m = h->mp; a.cp = h->cp; a.geo = L.geo;
+    a.x = L.x; a.xbs = L.xbs; a.xfrozen = L.xfrozen; a.pred_end = L.pred_end;
+    a.traj = L.traj; a.ghost = L.ghost; a.gedge = L.gedge;
+    a.obs_start = L.have_obs ? L.obs_start : nullptr; a.obs_idx = L.obs_idx; a.obs_lj = L.obs_lj;
+    a.obs_y = L.obs_y; a.obs_c = L.obs_c; a.obs_r = L.obs_r;
+    a.parts = L.parts; a.J = Jout; a.gx = L.gx; a.gw = gw;
+    a.maxex = L.wp.maxex; a.maxey = L.wp.maxey; a.maxpx = L.wp.maxpx; a.maxpy = L.wp.maxpy;
+    return a;
+}
+
 // one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
-    if (L.path == 2) {
+    if (L.path == 2 || L.path == 4) {
         {
             ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
@@ -351,6 +402,16 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 }
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
+    if (L.path == 4) {
+        // forward sweep, trajectory store and cost terms in one wavefront kernel
+        cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
+        const WkArgs a = wave_args(h, L, mask, Jout, gw);
+        if (L.wp.K == 2) wk_forward<2><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
+        else wk_forward<3><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
+        ++h->launches;
+        if (with_adjoint) adjoint_only(h, L, mask, gw);
+        return;
+    }
     if (L.path == 2) {
         ensure_tables(h);
         cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
@@ -371,6 +432,9 @@ void exchange(dd4dvar_t h, Layout& L)
     if (L.maxnring > 0)
         LAUNCH(xk_ghost_fill, dim3((L.maxnring + 127) / 128, L.nsub, std::min(L.Wmax, 8)), 128, L.dsubs, L.geo,
                L.traj, L.ghost);
+    if (L.wp.enabled)
+        LAUNCH(xk_edge_ua, dim3((2 * L.wp.maxpy + 63) / 64, L.nsub, std::min(L.Wmax, 8)), 64, L.dsubs, h->mp,
+               L.ghost, L.gedge);
 }
 
 int sync_check(dd4dvar_t h)
@@ -446,10 +510,16 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     h->G.lbfgs = false; h->L.lbfgs = true;
     h->G.path = 1;
     const bool fits = fused_fits(h->L.hs.data(), h->L.nsub) && nlat + 2 <= FK_CTAB;
+    wave_plan_init(h->L.wp, h->L.hs.data(), h->L.nsub);
+    const bool wave = h->L.wp.enabled && fits;
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
-    h->L.path = h->opt.path == 3 ? 3 : ((h->opt.path == 1 || !fits) ? 1 : 2);
+    if (h->opt.path == 4 && !wave) { delete h; return -2; }
+    if (h->opt.path < 0 || h->opt.path > 4) { delete h; return -1; }
+    if (h->opt.path == 0) h->L.path = wave ? 4 : (fits ? 2 : 1);
+    else h->L.path = h->opt.path;
+    if (h->L.path != 4) h->L.wp = WavePlan();
     fused_plan_init(h->G.fp, nullptr, 0, 0);
-    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, 0);
+    fused_plan_init(h->L.fp, (h->L.path == 2 || h->L.path == 4) ? h->L.hs.data() : nullptr, h->L.nsub, 0);
     h->ws_bytes = plan_all(h, nullptr);
     *out = h;
     return 0;
@@ -477,6 +547,16 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
     if (cudaFuncSetAttribute(sk_adjoint_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(sizeof(double) * SK_ADJ_SMEM_DOUBLES)) != cudaSuccess)
         return fail(h, -4, "shared-memory opt-in of sk_adjoint_step failed");
+    if (h->L.wp.enabled) {
+        int dev = 0, nsm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        h->L.wp.grid = std::max(1, std::min(nsm, h->L.nsub));
+        cudaError_t e1 = h->L.wp.K == 2
+            ? cudaFuncSetAttribute(wk_forward<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_fwd)
+            : cudaFuncSetAttribute(wk_forward<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_fwd);
+        if (e1 != cudaSuccess) return fail(h, -4, "shared-memory opt-in of the wavefront kernels failed");
+    }
     rc = fused_setup(h->stream, h->L.fp, h->L.dsubs);
     if (rc) return fail(h, -4, "fused kernel setup failed (shared-memory opt-in)");
     h->have_ws = true; h->have_bg = false; h->G.have_obs = h->L.have_obs = false;
@@ -510,7 +590,7 @@ int dd4dvar_set_background(dd4dvar_t h, const double* d_xb, const double h_sigma
 size_t dd4dvar_obs_workspace_bytes(dd4dvar_t h, long long n_obs_total)
 {
     if (!h || n_obs_total < 0) return 0;
-    const size_t per = 4 + 8 + 8;
+    const size_t per = 4 + 4 + 8 + 8 + 8;
     size_t nb = (size_t)n_obs_total * (1 + 2 * (size_t)h->L.maxcov);
     return nb * per + (size_t)(h->G.otot + h->L.otot + 8) * 8 + 4096;
 }
@@ -548,14 +628,44 @@ static int bin_observations(dd4dvar_t h, Layout& L, int n_times, const int* leve
     for (long long b = 0; b < L.otot; ++b) start[b + 1] += start[b];
     const long long nb = start[L.otot];
     std::vector<long long> fill(start.begin(), start.end() - 1);
-    std::vector<int> oi(nb + 1); std::vector<double> oy(nb + 1), oc(nb + 1);
+    std::vector<int> oi(nb + 1), ol(nb + 1); std::vector<double> oy(nb + 1), oc(nb + 1);
     visit([&](long long bin, int lidx, double y, double wt, int f) {
         const long long p = fill[bin]++;
         oi[p] = lidx; oy[p] = y; oc[p] = h->cp.lambda * wt / (h->sig_o[f] * h->sig_o[f]);
     });
+    // inside a bin: ascending (tile row, field, column), the order in which the wavefront kernels
+    // meet the cells; obs_lj = tile row of every entry
+    {
+        std::vector<long long> sub_of_bin(L.otot, 0);
+        for (int k = 0; k < L.nsub; ++k)
+            for (int n = 0; n <= L.hs[k].W + 1; ++n) if (L.hs[k].ooff + n < L.otot) sub_of_bin[L.hs[k].ooff + n] = k;
+        std::vector<long long> ord; std::vector<int> ti; std::vector<double> ty, tc;
+        for (long long b = 0; b < L.otot; ++b) {
+            const long long a0 = start[b], a1 = start[b + 1];
+            if (a1 <= a0) continue;
+            const Sub& sb = L.hs[sub_of_bin[b]];
+            auto key = [&](long long p) {
+                const int f = oi[p] / sb.ncell, c = oi[p] - f * sb.ncell;
+                const int lj = c / sb.ex, li = c - lj * sb.ex;
+                return ((long long)lj * 3 + f) * sb.ex + li;
+            };
+            ord.resize(a1 - a0);
+            for (long long p = a0; p < a1; ++p) ord[p - a0] = p;
+            std::sort(ord.begin(), ord.end(), [&](long long p, long long q) { return key(p) < key(q); });
+            ti.resize(a1 - a0); ty.resize(a1 - a0); tc.resize(a1 - a0);
+            for (long long p = 0; p < a1 - a0; ++p) { ti[p] = oi[ord[p]]; ty[p] = oy[ord[p]]; tc[p] = oc[ord[p]]; }
+            for (long long p = 0; p < a1 - a0; ++p) {
+                oi[a0 + p] = ti[p]; oy[a0 + p] = ty[p]; oc[a0 + p] = tc[p];
+                ol[a0 + p] = (ti[p] % sb.ncell) / sb.ex;
+            }
+        }
+    }
     L.obs_start = ar.take<long long>(L.otot + 1);
-    L.obs_idx = ar.take<int>(nb + 1); L.obs_y = ar.take<double>(nb + 1); L.obs_c = ar.take<double>(nb + 1);
+    L.obs_idx = ar.take<int>(nb + 1); L.obs_lj = ar.take<int>(nb + 1);
+    L.obs_y = ar.take<double>(nb + 1); L.obs_c = ar.take<double>(nb + 1); L.obs_r = ar.take<double>(nb + 1);
     if (ar.off > ar.cap) return fail(h, -1, "set_observations: observation workspace too small");
+    CU(cudaMemcpyAsync(L.obs_lj, ol.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemsetAsync(L.obs_r, 0, sizeof(double) * (nb + 1), h->stream));
     CU(cudaMemcpyAsync(L.obs_start, start.data(), sizeof(long long) * (L.otot + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(L.obs_idx, oi.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(L.obs_y, oy.data(), sizeof(double) * (nb + 1), cudaMemcpyHostToDevice, h->stream));

@@ -5,6 +5,7 @@
 // l.194-201).
 #pragma once
 #include "common.cuh"
+#include "model_math.cuh"
 
 // ghost[k][n][f][r] <- traj[owner][n][f][cell]: every ghost cell takes the value of the tile
 // that OWNS it, same window, all levels that start a step (R14).
@@ -119,4 +120,43 @@ __global__ void xk_gather(const Sub* __restrict__ subs, GeoP geo, int mode, int 
             }
 #pragma unroll
     for (int f = 0; f < DD_NF; ++f) out[((long long)f * geo.nlat + gj) * geo.nlon + gi] = acc[f];
+}
+
+// Frozen boundary data derived from the ghost ring (wavefront kernels, wave_common.cuh): the
+// stage-A value u^a (R3; eq (61) l.948-951 advective part) in the ghost columns 1 and
+// px-2 of every padded row and every level that starts a step.  It depends on ghost cells only
+// (columns 0..2 resp. px-3..px-1, rows r-1..r+1), so it changes with the exchange, not with the
+// control.  Layout per (subdomain, level): [S rows gys][N rows gyn][tile rows ey] x {west, east}.
+__global__ void xk_edge_ua(const Sub* __restrict__ subs, ModelP m, const double* __restrict__ ghost,
+                           double* __restrict__ gedge)
+{
+    const int k = blockIdx.y;
+    const Sub s = subs[k];
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= 2 * s.py) return;
+    const int r = q >> 1, side = q & 1;
+    const int c = side ? s.px - 2 : 1;
+    const bool ws = s.gys == 0, wn = s.gyn == 0;
+    const int gj = s.ej0 - s.gys + r;
+    const double dtcz = m.dtcz[gj < 0 ? 0 : (gj >= m.nlat ? m.nlat - 1 : gj)];
+    int slot;                                   // position of padded row r in the layout above
+    if (r < s.gys) slot = r;
+    else if (r >= s.gys + s.ey) slot = s.gys + (r - s.gys - s.ey);
+    else slot = s.gys + s.gyn + (r - s.gys);
+    for (int n = blockIdx.z; n < s.W; n += gridDim.z) {
+        const double* gz = ghost + s.goff + (long long)n * DD_NF * s.nring;
+        auto G = [&](int f, int rr, int cc) -> double {
+            const double* p = gz + (long long)f * s.nring;
+            if (rr < s.gys) return p[rr * s.px + cc];
+            if (rr >= s.gys + s.ey) return p[s.gys * s.px + (rr - s.gys - s.ey) * s.px + cc];
+            return p[(s.gys + s.gyn) * s.px + (rr - s.gys) * 2 * s.gx + (cc < s.gx ? cc : cc - s.ex)];
+        };
+        // north / south neighbours: the mirrored edge row at a pole wall (u is even under the mirror);
+        // on an open side rows 0 and py-1 lie outside the range of stage A and are never used
+        const int rN = r + 1 < s.py ? r + 1 : r, rS = r > 0 ? r - 1 : r;
+        (void)ws; (void)wn;
+        const double u = G(1, r, c), v = G(2, r, c);
+        const double ua = mm_stageA(u, G(1, r, c + 1), G(1, r, c - 1), G(1, rN, c), G(1, rS, c), dtcz * u, m.dtcm * v, m.kap);
+        gedge[s.eoff + (long long)n * 2 * s.py + slot * 2 + side] = ua;
+    }
 }

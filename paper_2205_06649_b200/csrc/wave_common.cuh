@@ -1,0 +1,178 @@
+// wave_common.cuh -- shared pieces of the WAVEFRONT sweep kernels (wave_forward.cuh, wave_adjoint.cuh).
+//
+// Design ("smem-resident tile, temporal wavefront").  One CTA of WK_NW warps owns one
+// space-time subdomain Delta_j x Omega_i (Def 3 l.128-154) at a time; the state of the window
+// (forward: Z^n, adjoint: the adjoint variable lambda^n and u^n) lives IN PLACE in shared memory for
+// the whole window.  Warp w works on a DIFFERENT TIME STEP than its neighbours: it marches over the
+// rows of the tile a few rows behind the warp that produces its input level (its "leader") and a
+// few rows ahead of the warp that consumes its output (its "follower").  All sub-stages of one
+// model step (R3) run software-pipelined on different rows inside one warp, so
+//   - north/south neighbours are the lane's own registers (row history),
+//   - east/west neighbours are the lane's own registers or ONE warp shuffle per K columns
+//     (every lane owns K adjacent columns; a warp spans the whole tile width),
+//   - there is no __syncthreads and no shared-memory exchange inside a step: the only
+//     inter-warp communication is the state row itself plus a progress word (release/acquire),
+//   - HBM sees exactly the algorithmic traffic: trajectory rows leave (forward) or arrive (adjoint)
+//     through TMA bulk copies (cp.async.bulk + mbarrier), the frozen ghost ring arrives the same
+//     way; nothing is staged through registers, nothing is re-read.
+// Eligibility (host, wave_plan): every tile has a ghost ring in longitude (p_lon >= 2), an even
+// number of columns (16-byte aligned rows for the bulk copies), at most 32 K + 4 padded columns
+// (K = 2 or 3 columns per lane) and the shared-memory layout fits in 227 KB.  Other layouts run
+// the row-marching kernels (fused_kernels.cuh) or the generic kernels.
+#pragma once
+#include <stdint.h>
+#include "common.cuh"
+#include "model_math.cuh"
+
+#define WK_NW 8                 // warps per CTA = time steps in flight per subdomain
+#define WK_NT (WK_NW * 32)
+#define WK_EWC 4                // tile rows per staged chunk of east/west ghost cells
+#define WK_HDR 128              // doubles reserved at the start of shared memory (barriers, flags)
+#define WK_SMEM_MAX 232448      // 227 KB: largest opt-in dynamic shared memory of one CTA on sm_100a
+
+// Kernel arguments (by value; everything the two kernels need).
+struct WkArgs {
+    const Sub* subs; const int* mask; int nsub; int* counter;
+    ModelP m; CostP cp; GeoP geo;
+    const double *x, *xbs, *xfrozen, *pred_end;
+    double* traj; const double* ghost; const double* gedge;
+    const long long* obs_start; const int* obs_idx; const int* obs_lj;
+    const double *obs_y, *obs_c; double* obs_r;
+    double *parts, *J;          // forward outputs: [nsub][5], [nsub]
+    double *gx, *gw;            // adjoint outputs
+    int maxex, maxey, maxpx, maxpy;
+};
+
+// Shared-memory layout in doubles (same function on host and device).
+//   header | row tables [(maxpy+2)][8] | resident state | per-warp staging
+// forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
+//   [tile ex][E ghosts 3][pad 2][W ghosts of the NEXT row 3], so that padded column c of tile row
+//   lj is at  st + f*FS + lj*P + (c - 3)  for every c (W ghosts sit in the previous row's tail).
+// adjoint resident state: lambda [3][maxey*maxex] and u1 [maxey*maxex], tile only (lambda is zero
+//   outside the extended tile).
+struct WkLayout {
+    int tab, st, P, FS, u1, wbase, wsz, sn, zr, ZP, ew, eds, ede, total;
+};
+__host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, int maxpx, int maxpy)
+{
+    WkLayout L;
+    int o = WK_HDR;
+    L.tab = o; o += (maxpy + 2) * 8;
+    if (!adj) {
+        L.P = maxex + 8; L.FS = maxey * L.P;
+        L.st = o + 8; o += 8 + 3 * L.FS;
+        L.u1 = 0;
+    } else {
+        L.P = maxex; L.FS = maxey * maxex;
+        L.st = o; o += 3 * L.FS; o = (o + 1) & ~1;
+        L.u1 = o; o += L.FS; o = (o + 1) & ~1;
+    }
+    L.wbase = o;
+    int p = 0;
+    L.ZP = maxpx + 2;
+    if (!adj) { L.sn = p; p += 9 * maxpx; L.zr = 0; }
+    else { L.zr = p; p += 9 * L.ZP; L.sn = 0; }
+    L.ew = p; p += 2 * 3 * 6 * WK_EWC;
+    L.eds = p; p += 16;
+    L.ede = p; p += 2 * 2 * WK_EWC;
+    L.wsz = (p + 1) & ~1;
+    L.total = L.wbase + WK_NW * L.wsz;
+    return L;
+}
+
+// ------------------------------------------------------------------------------------------
+// PTX wrappers: mbarrier, TMA bulk copies (cp.async.bulk), proxy fence, release/acquire flags.
+__device__ __forceinline__ uint32_t wk_s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void wk_mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(wk_s32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void wk_mbar_expect(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(wk_s32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool wk_mbar_try(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(wk_s32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void wk_mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    while (!wk_mbar_try(bar, parity)) {}
+}
+// global -> shared bulk copy; completion is signalled on `bar` (complete_tx); 16-byte aligned
+__device__ __forceinline__ void wk_g2s(double* dst, const double* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(wk_s32(dst)), "l"(src), "r"(bytes), "r"(wk_s32(bar)) : "memory");
+}
+// shared -> global bulk copy (bulk async-group)
+__device__ __forceinline__ void wk_s2g(double* dst, const double* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(dst), "r"(wk_s32(src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void wk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void wk_wait_read()
+{
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+// generic-proxy writes to shared memory -> visible to the async proxy (TMA store source)
+__device__ __forceinline__ void wk_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void wk_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void wk_publish(uint32_t addr, unsigned v)
+{
+    asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned wk_peek(uint32_t addr)
+{
+    unsigned v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+// wait until the progress word at `addr` has reached `need` (monotone counters, wrap-safe compare)
+__device__ __forceinline__ void wk_wait_prog(uint32_t addr, unsigned need)
+{
+    while ((int)(wk_peek(addr) - need) < 0) __nanosleep(40);
+}
+
+// ------------------------------------------------------------------------------------------
+// Per-subdomain geometry as a warp sees it (uniform over the CTA).
+struct WkGeo {
+    int ex, ey, px, py, gys, gyn, ncell, nring, W, joff;
+    bool ws, wn;            // pole walls (R4)
+};
+__device__ __forceinline__ WkGeo wk_geo(const Sub& s)
+{
+    WkGeo g;
+    g.ex = s.ex; g.ey = s.ey; g.px = s.px; g.py = s.py; g.gys = s.gys; g.gyn = s.gyn;
+    g.ncell = s.ncell; g.nring = s.nring; g.W = s.W; g.joff = s.ej0 - s.gys;
+    g.ws = s.gys == 0; g.wn = s.gyn == 0;
+    return g;
+}
+// row tables of this tile into shared memory: entry r+1 for padded row r = -1 .. py, with the guard
+// values r+_{-1} = 1 and r-_{nlat} = 1 of the virtual mirrored pole rows (model_math.cuh, A_v)
+__device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const WkGeo& g)
+{
+    for (int q = threadIdx.x; q < g.py + 2; q += WK_NT) {
+        const int gj = g.joff + q - 1;
+        const int cj = gj < 0 ? 0 : (gj >= m.nlat ? m.nlat - 1 : gj);
+        double* t = tab + q * 8;
+        t[0] = m.dtcz[cj]; t[1] = m.gdtcz[cj]; t[2] = m.dtf[cj]; t[3] = m.dtt[cj];
+        t[4] = gj < 0 ? 1.0 : m.rp[cj];
+        t[5] = gj >= m.nlat ? 1.0 : m.rm[cj];
+        t[6] = 0.0; t[7] = 0.0;
+    }
+}
+#define WK_T_DTCZ 0
+#define WK_T_GDTCZ 1
+#define WK_T_DTF 2
+#define WK_T_DTT 3
+#define WK_T_RP 4
+#define WK_T_RM 5
+
+// 64-bit shuffles
+__device__ __forceinline__ double wk_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double wk_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }

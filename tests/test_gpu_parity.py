@@ -22,8 +22,17 @@ LAYOUTS = {
     "bands1x3x2": dict(nlon=48, nlat=30, nsteps=10, p_lon=1, p_lat=3, q_time=2, overlap=2),
     "time_only": dict(p_lon=1, p_lat=1, q_time=4, overlap=0),
     "cols4x1x1_o1": dict(nlon=48, nlat=12, nsteps=6, p_lon=4, p_lat=1, q_time=1, overlap=1),
+    # layouts for the wavefront kernels (even tile widths, ghost ring in longitude):
+    # exact fit 94 + 6 = 100 padded columns (K = 3, all 32 lanes), ragged rows, 11 steps per window
+    "wave_fit100": dict(nlon=180, nlat=23, dt=300.0, nsteps=22, p_lon=2, p_lat=3, q_time=2, overlap=2,
+                        obs_frac=0.2, obs_every=3),
+    # K = 3 with idle lanes (px = 76), interior tile row with ghost rows on both sides, 9 windows steps > WK_NW
+    "wave_px76": dict(nlon=132, nlat=27, dt=300.0, nsteps=19, p_lon=2, p_lat=3, q_time=2, overlap=2,
+                      obs_frac=0.3, obs_every=1),
+    # K = 2 (px = 38), many short windows
+    "wave_k2": dict(nlon=56, nlat=20, nsteps=12, p_lon=2, p_lat=2, q_time=4, overlap=2),
 }
-PATHS = [1, 2, 3]
+PATHS = [1, 2, 3, 4]
 
 
 def make_pair(name, path):
@@ -32,8 +41,8 @@ def make_pair(name, path):
     try:
         g = gpu_problem(w, prob, path=path)
     except Exception as e:       # fused path refuses layouts whose tiles do not fit (-2)
-        if path == 2 and getattr(e, "code", 0) == -2:
-            pytest.skip("layout not eligible for the fused path")
+        if path in (2, 4) and getattr(e, "code", 0) == -2:
+            pytest.skip("layout not eligible for this kernel family")
         raise
     return w, o, prob, g
 
