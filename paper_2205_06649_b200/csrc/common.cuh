@@ -22,6 +22,15 @@ struct Sub {
     long long poff;          // offset in padded scratch arrays [3][npad] (single-field: poff/3)
     long long ooff;          // index into obs_start: entries ooff .. ooff+W+1
     long long eoff;          // offset in the edge store [W][py][2] (frozen u^a of ghost columns 1, px-2)
+    int nb0, nnb;            // this subdomain's overlap rectangles: entries nb0 .. nb0+nnb-1 of the NbRect table
+};
+
+// One rectangle Omega_i ∩ Omega_k of the spatial overlap (eq (20)-(22) l.294-306, case 1 l.310-314):
+// cells (i0 + di, j0 + dj) of this tile coincide with cells (ni0 + di, nj0 + dj) of the
+// neighbour tile in the same window, whose control starts at coff2 (shape [3][ncell2], row length ex2).
+struct NbRect {
+    long long coff2;
+    int ex2, ncell2, i0, j0, w, h, ni0, nj0;
 };
 
 // Model constants with dt folded in (row tables live in device memory, length nlat).

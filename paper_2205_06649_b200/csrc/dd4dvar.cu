@@ -54,6 +54,8 @@ struct Layout {
     int path = 1;                       // 1 generic (block-tiled step kernels), 2 fused row-marching, 3 generic per-stage kernels, 4 wavefront
     int tiles_x = 1, ntiles = 1;        // 32x16 output tiles of the step kernels
     std::vector<Sub> hs;
+    std::vector<NbRect> hnb;
+    NbRect* dnb = nullptr;
     std::vector<int> colown, rowown, ncolcov, colcov, nrowcov, rowcov, tc_ei0, tc_ex, tr_ej0, tr_ey, wb;
     long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0, etot = 0;
     int maxnpad = 0, maxncell = 0, maxnring = 0, Wmax = 0, CB = 1, maxcov = 1;
@@ -199,6 +201,30 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
                 L.maxnpad = std::max(L.maxnpad, s.npad); L.maxncell = std::max(L.maxncell, s.ncell);
                 L.maxnring = std::max(L.maxnring, s.nring); L.Wmax = std::max(L.Wmax, s.W);
             }
+    // spatial-overlap rectangles of every subdomain with the other tiles of its window (periodic in longitude)
+    L.hnb.clear();
+    for (int k = 0; k < L.nsub; ++k) {
+        Sub& s = L.hs[k];
+        s.nb0 = (int)L.hnb.size();
+        for (int b2 = 0; b2 < p2; ++b2)
+            for (int a2 = 0; a2 < p1; ++a2) {
+                if (a2 == s.a && b2 == s.b) continue;
+                const Sub& t = L.hs[(s.jw * p2 + b2) * p1 + a2];
+                const int j0 = std::max(s.ej0, t.ej0), j1 = std::min(s.ej0 + s.ey, t.ej0 + t.ey);
+                if (j1 <= j0) continue;
+                for (int sh = -1; sh <= 1; ++sh) {
+                    const int t0 = t.ei0 + sh * nlon;
+                    const int i0 = std::max(s.ei0, t0), i1 = std::min(s.ei0 + s.ex, t0 + t.ex);
+                    if (i1 <= i0) continue;
+                    NbRect r;
+                    r.coff2 = t.coff; r.ex2 = t.ex; r.ncell2 = t.ncell;
+                    r.i0 = i0 - s.ei0; r.j0 = j0 - s.ej0; r.w = i1 - i0; r.h = j1 - j0;
+                    r.ni0 = i0 - t0; r.nj0 = j0 - t.ej0;
+                    L.hnb.push_back(r);
+                }
+            }
+        s.nnb = (int)L.hnb.size() - s.nb0;
+    }
     {
         int mex = 0, mey = 0;
         for (const Sub& q : L.hs) { mex = std::max(mex, q.ex); mey = std::max(mey, q.ey); }
@@ -212,6 +238,7 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
 void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
 {
     L.dsubs = ar.take<Sub>(L.nsub);
+    L.dnb = ar.take<NbRect>(L.hnb.size() + 1);
     const size_t nit = (size_t)nlon * 6 + (size_t)nlat * 6 + 2 * L.p1 + 2 * L.p2 + L.q + 1;
     L.itab = ar.take<int>(nit);
     L.x = ar.take<double>(L.ctot); L.xbs = ar.take<double>(L.ctot); L.gx = ar.take<double>(L.ctot);
@@ -254,7 +281,7 @@ void wave_plan_init(WavePlan& wp, const Sub* subs, int nsub)
     if (!subs || nsub <= 0) return;
     for (int k = 0; k < nsub; ++k) {
         const Sub& s = subs[k];
-        if (s.gx != DD_GHOST || (s.ex & 1) || s.ey > 1000 || s.ex < 2) return;
+        if (s.gx != DD_GHOST || (s.ex & 1) || s.ey > 1000 || s.ex < 2 || s.ex > 255) return;
         if ((s.gys != 0 && s.gys != DD_GHOST) || (s.gyn != 0 && s.gyn != DD_GHOST)) return;
         wp.maxex = std::max(wp.maxex, s.ex); wp.maxey = std::max(wp.maxey, s.ey);
         wp.maxpx = std::max(wp.maxpx, s.px); wp.maxpy = std::max(wp.maxpy, s.py);
@@ -272,6 +299,8 @@ int upload_layout(dd4dvar_t h, Layout& L)
 {
     const int nlon = h->grid.nlon, nlat = h->grid.nlat;
     CU(cudaMemcpyAsync(L.dsubs, L.hs.data(), sizeof(Sub) * L.nsub, cudaMemcpyHostToDevice, h->stream));
+    if (!L.hnb.empty())
+        CU(cudaMemcpyAsync(L.dnb, L.hnb.data(), sizeof(NbRect) * L.hnb.size(), cudaMemcpyHostToDevice, h->stream));
     std::vector<int> t;
     auto put = [&](const std::vector<int>& v) { size_t o = t.size(); t.insert(t.end(), v.begin(), v.end()); return o; };
     const size_t o_colown = put(L.colown), o_ncolcov = put(L.ncolcov), o_colcov = put(L.colcov);
@@ -368,7 +397,7 @@ void ensure_tables(dd4dvar_t h)
 WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* gw)
 {
     WkArgs a;
-    a.subs = L.dsubs; a.mask = mask; a.nsub = L.nsub; a.counter = L.wp.counter;
+    a.subs = L.dsubs; a.nbr = L.dnb; a.mask = mask; a.nsub = L.nsub; a.counter = L.wp.counter;
     a.m = h->mp; a.cp = h->cp; a.geo = L.geo;
     a.x = L.x; a.xbs = L.xbs; a.xfrozen = L.xfrozen; a.pred_end = L.pred_end;
     a.traj = L.traj; a.ghost = L.ghost; a.gedge = L.gedge;
@@ -405,10 +434,30 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
     if (L.path == 4) {
         // forward sweep, trajectory store and cost terms in one wavefront kernel
         cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
-        const WkArgs a = wave_args(h, L, mask, Jout, gw);
+        WkArgs a = wave_args(h, L, mask, Jout, gw);
+#ifdef WK_PROF      // profiling build (_work only): per-phase cycle counters of wk_forward on stderr
+        static unsigned long long* d_prof = nullptr;
+        if (!d_prof) cudaMalloc(&d_prof, 8 * 16 * 8);
+        cudaMemsetAsync(d_prof, 0, 8 * 16 * 8, h->stream);
+        a.gw = reinterpret_cast<double*>(d_prof);
+#endif
         if (L.wp.K == 2) wk_forward<2><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         else wk_forward<3><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         ++h->launches;
+#ifdef WK_PROF
+        {
+            unsigned long long hp[8 * 16];
+            cudaStreamSynchronize(h->stream);
+            cudaMemcpy(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost);
+            static int nprint = 0;
+            if (nprint++ < 2)
+                for (int w = 0; w < 8; ++w) {
+                    fprintf(stderr, "[wkprof fwd] warp %d:", w);
+                    for (int q = 0; q < 12; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
+                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, chunk+ghostcopy, loads+A+h1+u1, v1+STS+fence, obs, lane0 block, -, loop-gap | init, steps, epilogue, fetch)\n");
+                }
+        }
+#endif
         if (with_adjoint) adjoint_only(h, L, mask, gw);
         return;
     }
@@ -634,7 +683,7 @@ static int bin_observations(dd4dvar_t h, Layout& L, int n_times, const int* leve
         oi[p] = lidx; oy[p] = y; oc[p] = h->cp.lambda * wt / (h->sig_o[f] * h->sig_o[f]);
     });
     // inside a bin: ascending (tile row, field, column), the order in which the wavefront kernels
-    // meet the cells; obs_lj = tile row of every entry
+    // meet the cells; obs_lj = packed (tile row, field, column) of every entry
     {
         std::vector<long long> sub_of_bin(L.otot, 0);
         for (int k = 0; k < L.nsub; ++k)
@@ -656,7 +705,11 @@ static int bin_observations(dd4dvar_t h, Layout& L, int n_times, const int* leve
             for (long long p = 0; p < a1 - a0; ++p) { ti[p] = oi[ord[p]]; ty[p] = oy[ord[p]]; tc[p] = oc[ord[p]]; }
             for (long long p = 0; p < a1 - a0; ++p) {
                 oi[a0 + p] = ti[p]; oy[a0 + p] = ty[p]; oc[a0 + p] = tc[p];
-                ol[a0 + p] = (ti[p] % sb.ncell) / sb.ex;
+                {   // packed (tile row << 12) | (field << 8) | column  (wave kernels: no divisions)
+                    const int f = ti[p] / sb.ncell, c = ti[p] - f * sb.ncell;
+                    const int lj = c / sb.ex, li = c - lj * sb.ex;
+                    ol[a0 + p] = (lj << 12) | (f << 8) | li;
+                }
             }
         }
     }

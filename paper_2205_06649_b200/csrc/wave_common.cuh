@@ -32,7 +32,7 @@
 
 // Kernel arguments (by value; everything the two kernels need).
 struct WkArgs {
-    const Sub* subs; const int* mask; int nsub; int* counter;
+    const Sub* subs; const NbRect* nbr; const int* mask; int nsub; int* counter;
     ModelP m; CostP cp; GeoP geo;
     const double *x, *xbs, *xfrozen, *pred_end;
     double* traj; const double* ghost; const double* gedge;
@@ -57,10 +57,10 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
 {
     WkLayout L;
     int o = WK_HDR;
-    L.tab = o; o += (maxpy + 2) * 8;
+    L.tab = o; o += (maxpy + 8) * 8;
     if (!adj) {
         L.P = maxex + 8; L.FS = maxey * L.P;
-        L.st = o + 8; o += 8 + 3 * L.FS;
+        L.st = o + 8; o += 8 + 3 * L.FS + 64;       // 64 doubles of slack: lanes beyond px read past a row
         L.u1 = 0;
     } else {
         L.P = maxex; L.FS = maxey * maxex;
@@ -76,7 +76,7 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
     L.eds = p; p += 16;
     L.ede = p; p += 2 * 2 * WK_EWC;
     L.wsz = (p + 1) & ~1;
-    L.total = L.wbase + WK_NW * L.wsz;
+    L.total = L.wbase + WK_NW * L.wsz + 64;
     return L;
 }
 
@@ -113,6 +113,32 @@ __device__ __forceinline__ void wk_s2g(double* dst, const double* src, uint32_t 
 {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
                  ::"l"(dst), "r"(wk_s32(src)), "r"(bytes) : "memory");
+}
+// the same with 32-bit shared-window addresses (no generic-to-shared conversion in the hot loop)
+__device__ __forceinline__ void wk_mbar_init32(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void wk_mbar_expect32(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void wk_mbar_wait32(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void wk_g2s32(uint32_t dst, const double* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void wk_s2g32(double* dst, uint32_t src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void wk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void wk_wait_read()
@@ -172,6 +198,16 @@ __device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const 
 #define WK_T_DTT 3
 #define WK_T_RP 4
 #define WK_T_RM 5
+
+// one elected lane of the (converged) warp; tells the compiler the region is single-threaded
+__device__ __forceinline__ bool wk_elect()
+{
+    uint32_t p;
+    asm volatile("{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\tselp.u32 %0, 1, 0, q;\n\t}" : "=r"(p));
+    return p != 0;
+}
+// broadcast from lane 0: marks a value as warp-uniform for the compiler (uniform datapath, no vote loops)
+__device__ __forceinline__ int wk_uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
 // 64-bit shuffles
 __device__ __forceinline__ double wk_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
