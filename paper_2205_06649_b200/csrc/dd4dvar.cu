@@ -19,6 +19,7 @@
 #include "lbfgs_kernels.cuh"
 #include "step_kernels.cuh"
 #include "wave_forward.cuh"
+#include "wave_adjoint.cuh"
 
 namespace {
 
@@ -411,7 +412,15 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
 // one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
-    if (L.path == 2 || L.path == 4) {
+    if (L.path == 4) {
+        cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
+        const WkArgs a = wave_args(h, L, mask, nullptr, gw);
+        if (L.wp.K == 2) wk_adjoint<2><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
+        else wk_adjoint<3><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
+        ++h->launches;
+        return;
+    }
+    if (L.path == 2) {
         {
             ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
@@ -568,7 +577,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     else h->L.path = h->opt.path;
     if (h->L.path != 4) h->L.wp = WavePlan();
     fused_plan_init(h->G.fp, nullptr, 0, 0);
-    fused_plan_init(h->L.fp, (h->L.path == 2 || h->L.path == 4) ? h->L.hs.data() : nullptr, h->L.nsub, 0);
+    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, 0);
     h->ws_bytes = plan_all(h, nullptr);
     *out = h;
     return 0;
@@ -604,7 +613,10 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
         cudaError_t e1 = h->L.wp.K == 2
             ? cudaFuncSetAttribute(wk_forward<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_fwd)
             : cudaFuncSetAttribute(wk_forward<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_fwd);
-        if (e1 != cudaSuccess) return fail(h, -4, "shared-memory opt-in of the wavefront kernels failed");
+        cudaError_t e2 = h->L.wp.K == 2
+            ? cudaFuncSetAttribute(wk_adjoint<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_adj)
+            : cudaFuncSetAttribute(wk_adjoint<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_adj);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(h, -4, "shared-memory opt-in of the wavefront kernels failed");
     }
     rc = fused_setup(h->stream, h->L.fp, h->L.dsubs);
     if (rc) return fail(h, -4, "fused kernel setup failed (shared-memory opt-in)");
