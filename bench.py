@@ -111,14 +111,34 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def csrc_hash():
+    """sha256 over the CUDA sources: ties profiles/traffic.json to the kernels it was captured from."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2205_06649_b200", "csrc")
+    hh = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        hh.update(f.encode()); hh.update(open(os.path.join(d, f), "rb").read())
+    return hh.hexdigest()[:16]
+
+
 def measured_traffic(kernel, cfg):
-    """DRAM bytes per launch of `kernel` from the committed ncu capture (config 3 only), else None."""
+    """DRAM bytes per launch of `kernel` (dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` capture, committed as profiles/traffic.json).  None unless the capture was
+    taken on config 3 from exactly the CUDA sources of this build (csrc hash recorded in the file)."""
     try:
         if cfg != 3:
             return None
-        return int(json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[kernel])
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        if t.get("csrc_sha16") != csrc_hash():
+            return None
+        return int(t["kernels"][kernel])
     except Exception:
         return None
+
+
+PATH_NAMES = {1: "generic (block-tiled step kernels)", 2: "row-marching fused kernels", 3: "per-stage generic kernels",
+              4: "wavefront forward (wk_forward) + row-marching adjoint (fk_adjoint2)",
+              5: "wavefront forward (wk_forward) + wavefront adjoint (wk_adjoint)"}
 
 
 def max_over_ranks(values, device=None):
@@ -163,6 +183,45 @@ def cpu_cores():
         return len(os.sched_getaffinity(0))
     except Exception:
         return os.cpu_count() or 1
+
+
+def _omp_threads(n):
+    """Thread count of the OpenMP runtime the oracle library uses (libgomp); the oracle is untouched."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except Exception:
+        return False
+
+
+def cpu_baseline(w):
+    """The correctness oracle as it stands (gcc -O2, -ffp-contract=off, long-double sums; never tuned
+    as a baseline), timed on a bounded sample: one warm-up sweep, then the median of 3 sweeps with
+    OpenMP over subdomains on all cores, and the median of 3 single-thread sweeps on a smaller sample."""
+    t0 = time.perf_counter()
+    o, k1 = oracle_sweep_sample(w)
+    t1 = time.perf_counter()
+    cores = cpu_cores()
+    o.sweep_range(0, k1)                                   # warm-up
+    ts = []
+    for _ in range(3):
+        a = time.perf_counter(); p, _ = o.sweep_range(0, k1); ts.append(time.perf_counter() - a)
+    tm = float(np.median(ts))
+    out = {"value": o.useful_ratio * p / tm, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "note": "untuned correctness oracle (gcc -O2 -ffp-contract=off), OpenMP over subdomains; a reported baseline, not a target",
+           "sample": f"gradient sweep of subdomains 0..{k1 - 1} of {o.nsub} ({int(p)} processed point-steps), "
+                     f"median of 3 after 1 warm-up: {tm:.2f} s (oracle setup {t1 - t0:.1f} s not timed)"}
+    k1s = max(1, k1 // max(cores, 1))
+    if _omp_threads(1):
+        o.sweep_range(0, k1s)
+        ts1 = []
+        for _ in range(3):
+            a = time.perf_counter(); p1, _ = o.sweep_range(0, k1s); ts1.append(time.perf_counter() - a)
+        _omp_threads(cores)
+        out["single_thread"] = {"value": o.useful_ratio * p1 / float(np.median(ts1)), "unit": UNIT, "cores": 1,
+                                "sample": f"subdomains 0..{k1s - 1}, median of 3 after 1 warm-up: {float(np.median(ts1)):.2f} s"}
+    return out
 
 
 def run_reference(args, w):
@@ -244,7 +303,7 @@ def run_sweep(args):
         torch.cuda.synchronize(dev)
         tta = time.perf_counter() - t0
         line = {"config": 4, "layout": f"{w.p_lon}x{w.p_lat}x{w.q_time}", "overlap": w.overlap, "subdomains": g.nsub,
-                "path": "fused" if g.active_path == 2 else "generic", "sweep_ms": ms,
+                "path": PATH_NAMES.get(g.active_path, str(g.active_path)), "sweep_ms": ms,
                 "useful_point_steps_per_s": w.nlon * w.nlat * w.nsteps / (ms * 1e-3), "outer_iters": outer,
                 "time_to_analysis_s": tta, "J_first": float(hist[0, 0]), "J_last": float(hist[-1, 0]),
                 "delta_last": float(hist[-1, 2])}
@@ -260,12 +319,16 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic kernels, 2 fused kernels")
+    ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 row-marching, 3 per-stage, 4 wavefront fwd + row-marching adj, 5 wavefront")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
     ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
+    ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the CUDA sources (for profiles/traffic.json)")
     args = ap.parse_args()
+    if args.csrc_hash:
+        print(csrc_hash())
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
         run_sweep(args)
@@ -373,10 +436,14 @@ def main():
     if rank == 0:
         ms_step = ms / args.steps
         peak, peak_src = peaks()
-        fused = g.active_path == 2
-        if fused:
-            kern, kb, kt = "fk_adjoint2 (fused adjoint sweep, one launch per gradient sweep)", adj_b, t_a
+        ap = g.active_path
+        fused = ap in (2, 4, 5)
+        if fused:   # the dominant kernel of the sweep = the adjoint sweep (one launch per gradient sweep)
+            kname = "wk_adjoint" if ap == 5 else "fk_adjoint2"
+            fname = "fk_forward2" if ap == 2 else "wk_forward"
+            kern, kb, kt = kname + " (adjoint sweep, one launch per gradient sweep)", adj_b, t_a
         else:
+            kname = fname = None
             kern, kb, kt = "gradient sweep, all per-stage launches of the generic path", fwd_b + adj_b, ms_step
         achieved = kb / (kt * 1e-3) / 1e9
         line = {
@@ -385,7 +452,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "counted": "useful = nlon*nlat*nsteps per sweep",
                        "processed_point_steps_per_sweep": pts, "processed_value": world * pts / (ms_step * 1e-3),
-                       "subdomains": g.nsub, "path": "fused" if fused else "generic",
+                       "subdomains": g.nsub, "path": PATH_NAMES.get(ap, str(ap)),
                        "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "outer_iteration_ms": 1e3 * outer_s,
@@ -395,21 +462,20 @@ def main():
                     "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
             "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": measured_traffic("fk_adjoint2", args.config) if fused else None, "kernel": kern, "peak_source": peak_src,
+                         "traffic": measured_traffic(kname, args.config) if fused else None,
+                         "traffic_source": "profiles/traffic.json (ncu --set full capture of this build's sources; null = no capture of this build)",
+                         "kernel": kern, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": kb, "kernel_ms": kt,
                          "sweep_algorithmic_GBps": (fwd_b + adj_b) / (ms_step * 1e-3) / 1e9,
                          "forward_ms": t_f, "adjoint_ms": t_a,
+                         "forward_kernel": {"name": fname, "algorithmic_bytes_per_launch": fwd_b,
+                                            "achieved": fwd_b / (t_f * 1e-3) / 1e9, "frac": fwd_b / (t_f * 1e-3) / 1e9 / peak,
+                                            "traffic": measured_traffic(fname, args.config) if fused else None,
+                                            "note": "forward sweep + trajectory store + cost terms"},
                          "bytes_per_processed_point_step": (fwd_b + adj_b) / pts},
         }
         if not args.no_cpu_baseline and world == 1:
-            t0 = time.perf_counter()
-            o, k1 = oracle_sweep_sample(w)
-            t1 = time.perf_counter()
-            p, _ = o.sweep_range(0, k1)
-            t2 = time.perf_counter()
-            line["cpu_baseline"] = {"value": o.useful_ratio * p / (t2 - t1), "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
-                                    "sample": f"gradient sweep of subdomains 0..{k1 - 1} of {o.nsub} "
-                                              f"({int(p)} processed point-steps, {t2 - t1:.1f} s; oracle setup {t1 - t0:.1f} s not timed)"}
+            line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line))
     g.close()
     if world > 1:

@@ -69,7 +69,11 @@ typedef struct {
  * maximum number of step halvings, Armijo constant.
  * path: 0 = choose automatically, 1 = force the generic kernels (one block-tiled launch per step,
  *       any tile size), 2 = force the fused persistent kernels (create fails with -2 if a tile
- *       does not fit), 3 = force the per-stage generic kernels (cross-check). */
+ *       does not fit), 3 = force the per-stage generic kernels (cross-check),
+ *       4 = wavefront forward kernel (shared-memory resident tile, TMA-staged rows, cost terms fused)
+ *       + row-marching adjoint kernel, 5 = wavefront forward + wavefront adjoint kernels
+ *       (4 and 5: create fails with -2 unless every tile has a ghost ring in longitude, an even
+ *       number of columns and at most 100 padded columns). */
 typedef struct {
     int lbfgs_m, n_inner, max_backtrack;
     double armijo_c1;

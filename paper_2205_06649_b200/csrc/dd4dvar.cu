@@ -412,7 +412,7 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
 // one evaluation of J_ji (and its gradient) on every (unmasked) subdomain: steps a1-a4
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
-    if (L.path == 4) {
+    if (L.path == 5) {
         cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
         const WkArgs a = wave_args(h, L, mask, nullptr, gw);
         if (L.wp.K == 2) wk_adjoint<2><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
@@ -420,7 +420,7 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
         ++h->launches;
         return;
     }
-    if (L.path == 2) {
+    if (L.path == 2 || L.path == 4) {
         {
             ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
@@ -440,7 +440,7 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 }
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
-    if (L.path == 4) {
+    if (L.path == 4 || L.path == 5) {
         // forward sweep, trajectory store and cost terms in one wavefront kernel
         cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
         WkArgs a = wave_args(h, L, mask, Jout, gw);
@@ -571,13 +571,13 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     wave_plan_init(h->L.wp, h->L.hs.data(), h->L.nsub);
     const bool wave = h->L.wp.enabled && fits;
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
-    if (h->opt.path == 4 && !wave) { delete h; return -2; }
-    if (h->opt.path < 0 || h->opt.path > 4) { delete h; return -1; }
+    if ((h->opt.path == 4 || h->opt.path == 5) && !wave) { delete h; return -2; }
+    if (h->opt.path < 0 || h->opt.path > 5) { delete h; return -1; }
     if (h->opt.path == 0) h->L.path = wave ? 4 : (fits ? 2 : 1);
     else h->L.path = h->opt.path;
-    if (h->L.path != 4) h->L.wp = WavePlan();
+    if (h->L.path != 4 && h->L.path != 5) h->L.wp = WavePlan();
     fused_plan_init(h->G.fp, nullptr, 0, 0);
-    fused_plan_init(h->L.fp, h->L.path == 2 ? h->L.hs.data() : nullptr, h->L.nsub, 0);
+    fused_plan_init(h->L.fp, (h->L.path == 2 || h->L.path == 4) ? h->L.hs.data() : nullptr, h->L.nsub, 0);
     h->ws_bytes = plan_all(h, nullptr);
     *out = h;
     return 0;

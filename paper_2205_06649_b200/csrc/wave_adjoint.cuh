@@ -418,13 +418,8 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             R.uaL2 = R.uaR2 = 0.0; R.pa = C.I_ZR + 1; R.pe = C.I_EDS; R.pe2 = C.I_EDS;
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
-            const int T3 = (C.T + 2) / 3 * 3;
 #pragma unroll 1
-            for (int t = 0; t < T3; t += 3) {
-                wa_tick<K>(t, R, C, sm, tab);
-                wa_tick<K>(t + 1, R, C, sm, tab);
-                wa_tick<K>(t + 2, R, C, sm, tab);
-            }
+            for (int t = 0; t < C.T; ++t) wa_tick<K>(t, R, C, sm, tab);
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);
             __syncwarp();
         }

@@ -32,7 +32,7 @@ LAYOUTS = {
     # K = 2 (px = 38), many short windows
     "wave_k2": dict(nlon=56, nlat=20, nsteps=12, p_lon=2, p_lat=2, q_time=4, overlap=2),
 }
-PATHS = [1, 2, 3, 4]
+PATHS = [1, 2, 3, 4, 5]
 
 
 def make_pair(name, path):
@@ -41,7 +41,7 @@ def make_pair(name, path):
     try:
         g = gpu_problem(w, prob, path=path)
     except Exception as e:       # fused path refuses layouts whose tiles do not fit (-2)
-        if path in (2, 4) and getattr(e, "code", 0) == -2:
+        if path in (2, 4, 5) and getattr(e, "code", 0) == -2:
             pytest.skip("layout not eligible for this kernel family")
         raise
     return w, o, prob, g
