@@ -10,6 +10,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 WORKER = r'''
 import os, sys
 sys.path.insert(0, %r)
+OUT = %r
 import torch.distributed as dist
 import bench
 dist.init_process_group("gloo")
@@ -19,7 +20,7 @@ assert out == [2.0, 10.0, 5.0], out
 assert bench.whole_job_value(100.0, dist.get_world_size(), out[0]) == 100.0
 dist.barrier()
 dist.destroy_process_group()
-print("rank", r, "ok")
+open(os.path.join(OUT, "rank%%d.ok" %% r), "w").write("ok")     # one file per rank: stdout of two ranks interleaves
 '''
 
 
@@ -32,10 +33,10 @@ def _run(args, **kw):
 
 def test_max_over_ranks_with_two_gloo_ranks(tmp_path):
     script = tmp_path / "worker.py"
-    script.write_text(WORKER % ROOT)
+    script.write_text(WORKER % (ROOT, str(tmp_path)))
     p = _run([str(script)])
     assert p.returncode == 0, p.stdout + p.stderr
-    assert "rank 0 ok" in p.stdout and "rank 1 ok" in p.stdout
+    assert (tmp_path / "rank0.ok").exists() and (tmp_path / "rank1.ok").exists()
 
 
 def test_reference_arm_under_torchrun_prints_one_line_from_rank0():

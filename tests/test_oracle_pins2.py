@@ -1,0 +1,141 @@
+"""Second set of oracle pins (round 2): the parts of the model step and of the exchange that the
+round-1 pins left free.
+
+Every expected value comes from outside the oracle:
+  - a hand calculation of ONE model step on a 4 x 2 grid, written out below cell by cell
+    (R1-R4; eq (60)-(62) PAPER.md:945-954; discretisation PAPER.md:971-989),
+  - the identity  m_{j+1} v_{j+1} - m_{j-1} v_{j-1} = 0  for  v_j = C / m_j, which makes the
+    meridional mass flux divergence of eq (62) vanish only if the metric ratios r_j^+, r_j^- sit
+    on the right neighbours,
+  - the closed form  u^1 - U = dt t_j U V  of eq (61)'s metric term on a uniform wind,
+  - the fact that a decomposed run whose controls cannot move (n_inner = 0) must keep reproducing
+    the global forecast after every exchange (boundary data = the neighbours' own
+    trajectories), bit for bit.
+A plausible mistake in any of these (r+ and r- swapped, the sign of t u v, the exchanged ghost ring
+read one level off) fails at least one test here while leaving the oracle self-consistent.
+"""
+import math
+
+import numpy as np
+
+from oracle import Oracle
+from paper_2205_06649_b200 import synth
+
+
+def test_one_step_on_a_4x2_grid_by_hand():
+    """nlon = 4, nlat = 2 (theta = -45, +45 degrees), radius a = 2/pi so that a dlambda = a dtheta = 1
+    and cz = cm = 1/2; cos_clamp = 1 (m = 1, r+ = r- = 1); dt = 1, kappa = 1/4, g = 1, Omega = 1/2:
+    f_j = -+S, t_j = -+S pi/2 with S = sin 45 deg.  Rows j = 0, 1 are both pole-wall rows (mirror
+    ghost row: h, u even, v odd).  Initial state (row j = 0 first):
+        h = [[10,12,11,9],[8,10,13,11]]  u = [[1,2,0,-1],[2,1,-1,0]]  v = [[0,1,-1,2],[1,0,2,-1]]
+    Cell (i=1, j=0): E = (2,0), W = (0,0), N = (1,1), S = mirror of itself; u0 = 2, v0 = 1.
+      stage A   h^a = 12 - [1/2*2*(11-10) + 1/2*1*(10-12)] + 1/4*(11+10+10+12-48) = 12 - 0 - 1.25 = 10.75
+                u^a = 2  - [1/2*2*(0-1)   + 1/2*1*(1-2)]   + 1/4*(0+1+1+2-8)      = 2 + 1.5 - 1   = 2.5
+                v^a = 1  - [1/2*2*(-1-0)  + 1/2*1*(0-(-1))] + 1/4*(-1+0+0-1-4)     = 1 + 0.5 - 1.5 = 0
+      height    D = 1/2*(u^a_E - u^a_W) + 1/2*(v^a_N - v^a_S) = 1/2*(-0.5+0.5) + 1/2*(0.5 - (-0)) = 0.25
+                h^1 = 10.75 - 10.75*0.25 = 8.0625
+      u         u^1 = 2.5 - 1*1/2*(h^1_E - h^1_W) + (f + t*2.5)*0 = 2.5 - 1/2*(21.4375 + 6.1875) = -11.3125
+      v         v^1 = 0 - 1*1/2*(h^1_N - h^1_S) - (f + t u^1) u^1,  h^1_N = 6.1875, h^1_S = h^1 (mirror)
+                    = 0.9375 - (-0.70710678 + 1.11072073*11.3125)*(-11.3125) = 0.9375 + 134.14273729 = 135.08023729
+    The other cells follow the same way; all 24 numbers are listed."""
+    S = math.sin(math.pi / 4)
+    o = Oracle(4, 2, 1.0, 1, radius=2.0 / math.pi, omega=0.5, gravity=1.0, cos_clamp=1.0, diffusion=0.25)
+    t = o.row_tables()
+    assert np.allclose(t["cz"], 0.5, rtol=1e-15) and np.isclose(t["cm"], 0.5, rtol=1e-15)
+    assert np.allclose(t["f"], [-S, S], rtol=1e-15) and np.allclose(t["t"], [-S * math.pi / 2, S * math.pi / 2], rtol=1e-15)
+    Z = np.array([[[10, 12, 11, 9], [8, 10, 13, 11]],
+                  [[1, 2, 0, -1], [2, 1, -1, 0]],
+                  [[0, 1, -1, 2], [1, 0, 2, -1]]], dtype=np.float64)
+    h1 = [[-6.1875, 8.0625, 21.4375, 9.6875], [2.9375, 6.1875, 26.8125, 14.0625]]
+    u1 = [[0.08488037912487245, -11.3125, -1.6159928278335034, 13.540119620875128],
+          [3.2857535860832483, -7.695545691232237, -4.068733574228172, 13.699967148456343]]
+    v1 = [[-2.9944781222462646, 135.08023728880983, 1.0703930926873688, 209.52061782887057],
+          [-19.877415877008552, -58.899390451474574, -18.698000482549606, -219.34501454403585]]
+    out = o.step(Z)
+    assert np.allclose(out[0], h1, rtol=1e-13, atol=0)
+    assert np.allclose(out[1], u1, rtol=1e-12, atol=1e-13)
+    assert np.allclose(out[2], v1, rtol=1e-12, atol=1e-13)
+
+
+def test_metric_ratios_sit_on_the_right_neighbours():
+    """g = Omega = 0, kappa = 0, h = h0, u = 0, v_j = C / m_j on the SPHERE (default clamp at 50 deg):
+    the flux m v is constant in latitude, so eq (62)'s d(h v cos)/dtheta term vanishes and h can only
+    drift through the O(dt) self-advection of v.  With r+ and r- exchanged the drift is
+    O(h0 cm C dtheta tan(theta)) ~ 1e-3 m/s instead (rows equatorward of the clamp, away from the walls)."""
+    for nlat in (18, 36, 72):
+        nlon = 2 * nlat
+        o = Oracle(nlon, nlat, 60.0, 1, omega=0.0, gravity=0.0, diffusion=0.0)
+        mc = o.row_tables()["mc"]
+        Z = np.zeros((3, nlat, nlon)); Z[0] = synth.H0; Z[2] = (10.0 / mc)[:, None]
+        out = o.step(Z)
+        drift = np.abs(out[0] - synth.H0) / 60.0
+        sphere = np.where(mc > math.cos(math.radians(50.0)) * (1 + 1e-12))[0]
+        assert sphere.size >= nlat // 2 - 2
+        assert drift[sphere[1:-1]].max() < 1e-5, (nlat, drift[sphere[1:-1]].max())
+        # the test has teeth: the same rows see a varying metric
+        assert np.abs(np.diff(mc[sphere])).max() > 1e-3
+
+
+def test_metric_term_t_u_v_of_the_u_equation_closed_form():
+    """Uniform wind (U, V), uniform height, g = Omega = 0, kappa = 0: every difference vanishes away
+    from the pole walls, so stage A leaves (U, V) alone and eq (61)'s metric term gives exactly
+    u^1 - U = dt t_j U V with t_j = sin(theta_j) / (a m_j): positive in the northern hemisphere for
+    U, V > 0, antisymmetric about the equator."""
+    nlon, nlat, dt, U, V = 24, 18, 120.0, 7.0, 3.0
+    o = Oracle(nlon, nlat, dt, 1, omega=0.0, gravity=0.0, diffusion=0.0)
+    th = -np.pi / 2 + (np.arange(nlat) + 0.5) * np.pi / nlat
+    mc = np.maximum(np.cos(th), math.cos(math.radians(50.0)))
+    Z = np.zeros((3, nlat, nlon)); Z[0] = synth.H0; Z[1] = U; Z[2] = V
+    out = o.step(Z)
+    du = out[1][1:-1] - U                                   # rows 0 and nlat-1 feel the mirrored v
+    ref = dt * np.sin(th[1:-1]) / (synth.RADIUS * mc[1:-1]) * U * V
+    assert np.allclose(du, ref[:, None], rtol=1e-9, atol=0)
+    assert du[-1, 0] > 0 and du[0, 0] < 0
+    assert np.allclose(du[::-1], -du, rtol=1e-9, atol=0)
+
+
+def test_frozen_ghost_ring_after_an_exchange_still_reproduces_the_global_forecast():
+    """2x2x2 decomposition with n_inner = 0: the controls cannot move, so after any number of outer
+    iterations (each ends with the exchange of PAPER.md:465) every local trajectory computed with
+    the EXCHANGED ghost ring must still equal the global background forecast on its tile, bit for
+    bit (same operation order).  Exercises the owner lookup, the level indexing and the
+    previous-iteration store that the first (background) iteration never touches."""
+    w = synth.CONFIGS[0]
+    o = Oracle.from_workload(w, n_inner=0)
+    prob = synth.make_problem(w, o.forecast)
+    o.set_background(prob.xb, prob.sigma_b)
+    o.set_observations(prob.obs)
+    ub = o.forecast(prob.xb, np.arange(w.nsteps + 1))
+    an, hist = o.run(2)
+    assert np.array_equal(an, prob.xb)
+    assert hist[1, 2] == 0.0 and hist[2, 2] == 0.0
+    for k, s in enumerate(o.subs):
+        _, _, tr = o.eval_local(k, o.get_control(k), want_grad=False, want_traj=True)
+        jj = s["ej0"] + np.arange(s["ey"]); ii = (s["ei0"] + np.arange(s["ex"])) % w.nlon
+        ref = ub[s["s"]:s["e"] + 1][:, :, jj[:, None], ii[None, :]]
+        assert np.array_equal(tr, ref), k
+
+
+def _energy(Z, mc):
+    """total energy (kinetic + potential) with the clamped-metric area weights"""
+    h, u, v = Z
+    return float(np.sum(mc[:, None] * (0.5 * h * (u * u + v * v) + 0.5 * synth.GRAVITY * h * h)))
+
+
+def test_stability_gate_s0_configs_0_to_2():
+    """the forward model run over the full window of
+    configs 0-2, from the truth and from the noisy background, stays bounded: finite,
+    max|h - h0| < 3000 m, wind < 150 m/s, energy ratio end/start in [0.5, 1.3] (the configs' time
+    steps are beyond the explicit limit at the polar rows; the clamp + split scheme must hold)."""
+    for cfg in (0, 1, 2):
+        w = synth.CONFIGS[cfg]
+        o = Oracle.from_workload(w.with_layout(1, 1, 1, 0))
+        mc = o.row_tables()["mc"]
+        t0 = synth.truth_initial(w)
+        sb, _ = synth.sigmas(t0)
+        for x0 in (t0, synth.background(w, t0, sb)):
+            end = o.forecast(x0, np.array([w.nsteps]))[0]
+            assert np.all(np.isfinite(end)), cfg
+            assert np.abs(end[0] - synth.H0).max() < 3000.0, cfg
+            assert np.sqrt(end[1] ** 2 + end[2] ** 2).max() < 150.0, cfg
+            assert 0.5 <= _energy(end, mc) / _energy(x0, mc) <= 1.3, cfg
