@@ -24,9 +24,18 @@
  *     values synchronise that stream before returning.
  *   - Return value: 0 on success, otherwise
  *       -1 invalid argument            -2 decomposition does not fit the grid / window
- *       -3 called out of order         -4 CUDA error          -5 non-finite cost
+ *       -3 called out of order         -4 CUDA error          -5 non-finite cost or gradient
  *     Nothing is thrown across the ABI; dd4dvar_last_error gives the text of the last failure.
  *   - There is no CPU fallback: without a CUDA device every compute call returns -4.
+ *   - Handles share nothing: every table and buffer a kernel reads belongs to one handle, so
+ *     several live handles may work concurrently on different streams (one host thread per handle
+ *     at a time; a handle itself is not re-entrant).  One side effect reaches beyond the handle:
+ *     when the row-marching adjoint kernel is in use (paths 2 and 4), dd4dvar_set_workspace raises
+ *     the device's cudaLimitPersistingL2CacheSize (never lowers it) and puts a persisting
+ *     access-policy window for its scratch on the caller's stream; dd4dvar_destroy restores the
+ *     stream's previous window, releases the persisting lines and resets the limit to the value
+ *     found at set_workspace.  Two handles on the SAME stream would overwrite each other's window
+ *     (performance only, never results).
  */
 #ifndef DD4DVAR_H
 #define DD4DVAR_H

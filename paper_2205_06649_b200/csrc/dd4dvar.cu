@@ -94,7 +94,9 @@ struct dd4dvar_s {
     long long launches = 0;
     // model tables
     std::vector<double> h_tab;          // 6 x nlat
+    std::vector<double> h_ctab;         // staging of the row-marching kernels' padded tables
     double* d_tab = nullptr;
+    double* d_ctab = nullptr;           // [6][FK_CTAB], per handle
     ModelP mp{};
     CostP cp{};
     double sig_o[3] = { 1, 1, 1 };
@@ -386,14 +388,6 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
            L.pred_end, buf[L.Wmax & 1], L.gx, gw);
 }
 
-// the constant-memory row tables belong to the handle that launched last
-static const void* g_ctab_owner = nullptr;
-void ensure_tables(dd4dvar_t h)
-{
-    if (g_ctab_owner == h) return;
-    fused_upload_tables(h->stream, h->h_tab.data(), h->grid.nlat);
-    g_ctab_owner = h;
-}
 
 WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* gw)
 {
@@ -422,16 +416,15 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
     }
     if (L.path == 2 || L.path == 4) {
         {
-            ensure_tables(h);
             cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
             if (L.fp.nt == 64) fk64::fk_adjoint2<<<L.fp.nslots, 64, 0, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
-                L.fp.slot_stride, L.fp.counter);
+                L.fp.slot_stride, L.fp.counter, h->d_ctab);
             else fk128::fk_adjoint2<<<L.fp.nslots, 128, 0, h->stream>>>(
                 L.dsubs, mask, h->mp, h->cp, L.geo, L.x, L.xbs, L.xfrozen, L.pred_end, L.traj, L.ghost,
                 L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c, L.gx, gw, L.nsub, L.fp.scratch,
-                L.fp.slot_stride, L.fp.counter);
+                L.fp.slot_stride, L.fp.counter, h->d_ctab);
         }
         ++h->launches;
         return;
@@ -471,12 +464,11 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
         return;
     }
     if (L.path == 2) {
-        ensure_tables(h);
         cudaMemsetAsync(L.fp.counter, 0, sizeof(int), h->stream);
         if (L.fp.nt == 64) fk64::fk_forward2<<<L.fp.nslots_fwd, 64, 0, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
-                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
+                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter, h->d_ctab);
         else fk128::fk_forward2<<<L.fp.nslots_fwd, 128, 0, h->stream>>>(L.dsubs, mask, h->mp, L.x, L.traj, L.ghost,
-                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter);
+                                                                      L.nsub, L.fp.scratch, L.fp.slot_stride, L.fp.counter, h->d_ctab);
         ++h->launches;
     } else forward_generic(h, L, mask);
     cost_generic(h, L, mask, Jout);
@@ -514,6 +506,7 @@ size_t plan_all(dd4dvar_t h, char* base)
 {
     Arena ar; ar.base = base;
     h->d_tab = ar.take<double>(6 * (size_t)h->grid.nlat);
+    h->d_ctab = ar.take<double>(6 * (size_t)FK_CTAB);
     plan_layout(h->G, ar, h->grid.nlon, h->grid.nlat, h->opt.lbfgs_m);
     plan_layout(h->L, ar, h->grid.nlon, h->grid.nlat, h->opt.lbfgs_m);
     return ar.off + 256;
@@ -618,8 +611,14 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
             : cudaFuncSetAttribute(wk_adjoint<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_adj);
         if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(h, -4, "shared-memory opt-in of the wavefront kernels failed");
     }
+    if (h->L.fp.enabled) {
+        h->h_ctab.assign(6 * (size_t)FK_CTAB, 0.0);
+        if (fused_upload_tables(h->stream, h->h_tab.data(), nlat, h->h_ctab.data(), h->d_ctab))
+            return fail(h, -4, "upload of the row tables failed");
+    }
+    fused_teardown(h->stream, h->L.fp);         // (a second set_workspace on the same handle)
     rc = fused_setup(h->stream, h->L.fp, h->L.dsubs);
-    if (rc) return fail(h, -4, "fused kernel setup failed (shared-memory opt-in)");
+    if (rc) return fail(h, -4, "fused kernel setup failed (persisting-L2 window)");
     h->have_ws = true; h->have_bg = false; h->G.have_obs = h->L.have_obs = false;
     return sync_check(h);
 }
@@ -904,6 +903,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         return global_cost(h, out);
     };
     if ((rc = gather_and_cost(&h_history[0]))) return rc;
+    CU(cudaMemsetAsync(L.st.nactive, 0, 2 * sizeof(int), h->stream));
     h_history[1] = 0.0; h_history[2] = 0.0;
     const dim3 vgrid(std::min(64, (3 * L.maxncell + 255) / 256), nsub);
     if (outer_iters == 0) {
@@ -928,10 +928,11 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
                 LAUNCH(lk_trial, vgrid, 256, L.dsubs, L.st.active, h->cp, L.st.t, L.w, L.d, L.xbs, L.wt, L.x);
                 sweep(h, L, false, L.st.active, L.st.Jt, nullptr);
                 LAUNCH(lk_lscheck, (nsub + 127) / 128, 128, nsub, lp, L.st);
-                int nact = 0;
-                CU(cudaMemcpyAsync(&nact, L.st.nactive, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                int nact[2] = { 0, 0 };
+                CU(cudaMemcpyAsync(nact, L.st.nactive, 2 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
                 if ((rc = sync_check(h))) return rc;
-                if (nact == 0) break;
+                if (nact[1]) return fail(h, -5, "run: non-finite gradient");
+                if (nact[0] == 0) break;
             }
             // gradient at the accepted points (their trajectories are still in the store)
             adjoint_only(h, L, L.st.ok, L.gn);
@@ -976,7 +977,8 @@ long long dd4dvar_launch_count(dd4dvar_t h) { return h ? h->launches : -1; }
 const char* dd4dvar_last_error(dd4dvar_t h) { return h ? h->err.c_str() : "null handle"; }
 void dd4dvar_destroy(dd4dvar_t h)
 {
-    if (g_ctab_owner == h) g_ctab_owner = nullptr;
+    if (!h) return;
+    fused_teardown(h->stream, h->L.fp);
     delete h;
 }
 

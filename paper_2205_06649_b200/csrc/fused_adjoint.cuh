@@ -20,7 +20,8 @@ struct AdjRegs {
 };
 struct AdjCtx {
     FkGeo g;
-    int cj;                         // joff + 1: index of padded row 0 in the constant tables
+    int cj;                         // joff + 1: index of padded row 0 in the row tables
+    const double* tb;               // this handle's row tables [6][FK_CTAB]
     FkCol col;
     double* zr;                     // [8][3][FK_NT]
     double* uas;                    // [4][FK_NT]
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__(FK_NT, FK_ADJ_CTAS * 128 / FK_NT) fk_adjoint2(
                                                         const double* __restrict__ obs_y,
                                                         const double* __restrict__ obs_c, double* gx, double* gw,
                                                         int nsub, double* scratch, long long slot_stride,
-                                                        int* counter)
+                                                        int* counter, const double* __restrict__ ctabp)
 {
     __shared__ int s_next;
     __shared__ double zr[FK_ZR * 3 * FK_NT];
@@ -192,6 +193,7 @@ __global__ void __launch_bounds__(FK_NT, FK_ADJ_CTAS * 128 / FK_NT) fk_adjoint2(
     AdjCtx C;
     C.g = fk_geo(s);
     C.cj = C.g.joff + 1;
+    C.tb = ctabp;
     const FkGeo& g = C.g;
     const int n3 = 3 * s.ncell;
     double* lam = scratch + (long long)blockIdx.x * slot_stride;

@@ -13,7 +13,8 @@ struct FwdRegs {
 };
 struct FwdCtx {
     FkGeo g;
-    int cj;                         // joff + 1: index of padded row 0 in the constant tables
+    int cj;                         // joff + 1: index of padded row 0 in the row tables
+    const double* tb;               // this handle's row tables [6][FK_CTAB]
     FkCol col;
     double* z0s;      // [2][3][FK_NT]
     double* uas;      // [2][FK_NT]
@@ -91,7 +92,8 @@ __device__ __forceinline__ void fwd_tick(const int t, FwdRegs& R, const FwdCtx& 
 __global__ void __launch_bounds__(FK_NT, 512 / FK_NT) fk_forward2(const Sub* __restrict__ subs, const int* __restrict__ mask,
                                                         ModelP m, const double* __restrict__ x, double* traj,
                                                         const double* ghost, int nsub, double* scratch,
-                                                        long long slot_stride, int* counter)
+                                                        long long slot_stride, int* counter,
+                                                        const double* __restrict__ ctabp)
 {
     __shared__ double z0s[2 * 3 * FK_NT];
     __shared__ double uas[2 * FK_NT];
@@ -108,6 +110,7 @@ __global__ void __launch_bounds__(FK_NT, 512 / FK_NT) fk_forward2(const Sub* __r
         FwdCtx C;
         C.g = fk_geo(s);
         C.cj = C.g.joff + 1;
+        C.tb = ctabp;
         const FkGeo& g = C.g;
         double* state = scratch + (long long)blockIdx.x * slot_stride;
         C.z0s = z0s; C.uas = uas; C.h1s = h1s;

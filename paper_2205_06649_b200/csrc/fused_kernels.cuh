@@ -26,6 +26,10 @@
 
 struct FusedPlan {
     int enabled = 0;
+    // what fused_setup changed and fused_teardown puts back (device limit, stream attribute)
+    bool l2_set = false;
+    size_t l2_prev_limit = 0;
+    cudaStreamAttrValue l2_prev_attr;
     int maxpy = 0, maxncell = 0;
     size_t smem_fwd = 0, smem_adj = 0;
     // persistent CTAs: one L2-persistent scratch slot per resident CTA (in-place state / adjoint variable)
@@ -112,18 +116,18 @@ __device__ __forceinline__ void fk_load_row(const FkGeo& g, const FkCol& c, int 
     z[0] = p[0]; z[1] = p[fs]; z[2] = p[2 * fs];
 }
 
-// Row tables in constant memory for the static-slot kernels: entry [k][gj + 1], with guard entries
-// r+_{-1} = 1 and r-_{nlat} = 1 for the virtual mirrored pole rows.  Uniform (per-CTA) index ->
-// constant-cache loads, which keep the tables off the L1TEX/shared-memory pipe.
+// Row tables of the static-slot kernels: entry [k][gj + 1], with guard entries r+_{-1} = 1 and
+// r-_{nlat} = 1 for the virtual mirrored pole rows.  They live in a per-HANDLE device buffer (no
+// process-global state: two handles on two streams never share tables) and are read with uniform
+// (per-CTA) indices through the read-only path; `C.tb` is the tick context's pointer to them.
 #define FK_CTAB 1026
-__constant__ double c_tab[6][FK_CTAB];
 #define CT_DTCZ 0
 #define CT_GDTCZ 1
 #define CT_DTF 2
 #define CT_DTT 3
 #define CT_RP 4
 #define CT_RM 5
-__device__ __forceinline__ double ctab(int k, int cj, int j) { return c_tab[k][cj + j]; }
+#define ctab(k, cj, j) __ldg(C.tb + (k) * FK_CTAB + (cj) + (j))
 
 // the kernels are instantiated for CTAs of 128 threads (tiles up to 128 padded columns) and of 64
 // threads (narrow tiles, e.g. the 16x16x8 layout of config 4: 55 columns)
@@ -159,19 +163,19 @@ inline void fused_plan_init(FusedPlan& fp, const Sub* subs, int nsub, int lam_mo
     fp.smem_fwd = 0;
     fp.smem_adj = 0;
 }
-// copy the row tables (host, 6 x nlat, order dtcz gdtcz dtf dtt rp rm) into constant memory
-inline int fused_upload_tables(cudaStream_t stream, const double* h_tab, int nlat)
+// copy the row tables (host, 6 x nlat, order dtcz gdtcz dtf dtt rp rm) into this handle's device buffer
+// d_ctab [6][FK_CTAB]; `stage` (host, same size, owned by the handle) must outlive the async copy
+inline int fused_upload_tables(cudaStream_t stream, const double* h_tab, int nlat, double* stage, double* d_ctab)
 {
     if (nlat + 2 > FK_CTAB) return -1;
-    static double buf[6][FK_CTAB];
     for (int k = 0; k < 6; ++k) {
-        for (int q = 0; q < FK_CTAB; ++q) buf[k][q] = 0.0;
-        for (int j = 0; j < nlat; ++j) buf[k][j + 1] = h_tab[(size_t)k * nlat + j];
-        buf[k][0] = buf[k][1]; buf[k][nlat + 1] = buf[k][nlat];
+        double* b = stage + (size_t)k * FK_CTAB;
+        for (int q = 0; q < FK_CTAB; ++q) b[q] = 0.0;
+        for (int j = 0; j < nlat; ++j) b[j + 1] = h_tab[(size_t)k * nlat + j];
+        b[0] = b[1]; b[nlat + 1] = b[nlat];
     }
-    buf[CT_RP][0] = 1.0; buf[CT_RM][nlat + 1] = 1.0;
-    cudaStreamSynchronize(stream);
-    return cudaMemcpyToSymbol(c_tab, buf, sizeof(buf)) == cudaSuccess ? 0 : -1;
+    stage[(size_t)CT_RP * FK_CTAB] = 1.0; stage[(size_t)CT_RM * FK_CTAB + nlat + 1] = 1.0;
+    return cudaMemcpyAsync(d_ctab, stage, sizeof(double) * 6 * FK_CTAB, cudaMemcpyHostToDevice, stream) == cudaSuccess ? 0 : -1;
 }
 inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
 {
@@ -182,16 +186,30 @@ inline int fused_setup(cudaStream_t stream, FusedPlan& fp, const Sub*)
         size_t bytes = sizeof(double) * (size_t)fp.nslots_fwd * fp.slot_stride;
         size_t lim = bytes < (size_t)prop.persistingL2CacheMaxSize ? bytes : (size_t)prop.persistingL2CacheMaxSize;
         if (lim > 0) {
-            cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, lim);
+            memset(&fp.l2_prev_attr, 0, sizeof(fp.l2_prev_attr));
+            cudaDeviceGetLimit(&fp.l2_prev_limit, cudaLimitPersistingL2CacheSize);
+            cudaStreamGetAttribute(stream, cudaStreamAttributeAccessPolicyWindow, &fp.l2_prev_attr);
+            fp.l2_set = true;
+            if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, lim > fp.l2_prev_limit ? lim : fp.l2_prev_limit) != cudaSuccess) return -1;
             cudaStreamAttrValue av; memset(&av, 0, sizeof(av));
             av.accessPolicyWindow.base_ptr = fp.scratch;
             av.accessPolicyWindow.num_bytes = bytes < (size_t)prop.accessPolicyMaxWindowSize ? bytes : (size_t)prop.accessPolicyMaxWindowSize;
             av.accessPolicyWindow.hitRatio = lim >= bytes ? 1.0f : (float)lim / (float)bytes;
             av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
             av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
-            cudaStreamSetAttribute(stream, cudaStreamAttributeAccessPolicyWindow, &av);
-            cudaGetLastError();
+            if (cudaStreamSetAttribute(stream, cudaStreamAttributeAccessPolicyWindow, &av) != cudaSuccess) return -1;
         }
     }
     return 0;
+}
+// undo fused_setup: the stream gets its previous access-policy window back, persisting lines are
+// released, the device-wide persisting-L2 limit returns to what it was
+inline void fused_teardown(cudaStream_t stream, FusedPlan& fp)
+{
+    if (!fp.l2_set) return;
+    cudaStreamSynchronize(stream);
+    cudaStreamSetAttribute(stream, cudaStreamAttributeAccessPolicyWindow, &fp.l2_prev_attr);
+    cudaCtxResetPersistingL2Cache();
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, fp.l2_prev_limit);
+    fp.l2_set = false;
 }

@@ -30,7 +30,7 @@ struct LbfgsState {
     int* trial;      // halvings so far
     double* rho;     // [nsub][m]
     double* gam;     // [nsub][m]  s.y / y.y of the pair in that slot
-    int* nactive;    // [1] counter
+    int* nactive;    // [0] counter of subdomains still searching, [1] non-finite-gradient flag
 };
 
 // Sum over the whole cluster (= over the whole subdomain vector) of per-thread partial sums:
@@ -86,8 +86,9 @@ __global__ void __cluster_dims__(LK_CL, 1, 1) __launch_bounds__(NT) lk_direction
     double* dk = d + s.coff;
     const double gg = cdot<NT>(gk, gk, n, sh, xch, xs);
     const double gnorm = sqrt(gg);
-    if (!(gnorm > 0.0)) {
-        if (lead) { st.done[k] = 1; st.active[k] = 0; st.ok[k] = 0; }
+    if (!(gnorm > 0.0) || isinf(gnorm)) {
+        // zero gradient: converged.  NaN / Inf gradient: frozen too, but reported (nactive[1] -> run returns -5)
+        if (lead) { st.done[k] = 1; st.active[k] = 0; st.ok[k] = 0; if (!(gnorm == 0.0)) atomicExch(st.nactive + 1, 1); }
         cl.sync();
         return;
     }
