@@ -15,6 +15,29 @@ from helpers import oracle_problem, gpu_problem, rel
 pytestmark = pytest.mark.gpu
 TOL_EVAL = 1e-10
 TOL_AN = 1e-8
+TOL_MAX = 1e-9          # largest single-element gradient error relative to the largest element
+
+
+def check_sample(o, g, prob, sample, seed, tol=TOL_EVAL, tol_max=TOL_MAX, traj=False):
+    """Perturbed controls on a sample of subdomains (the others keep their current controls):
+    cost, the five parts, gradient (2-norm and element-wise) and optionally the stored trajectory."""
+    xs = perturbed(o, prob, sample, seed)
+    flat = g.get_controls().clone()
+    for k in sample:
+        n = int(np.prod(g.sub_shape(k)))
+        flat[g.offsets[k]:g.offsets[k] + n] = g._dev(xs[k]).reshape(-1)
+    costs, parts, grads = g.eval_local(flat)
+    gl = g.split(grads)
+    for k in sample:
+        po, go, tr = o.eval_local(k, xs[k], want_traj=traj)
+        gk = gl[k].cpu().numpy()
+        assert abs(costs[k] - po[0]) <= tol * abs(po[0]), k
+        for q in range(5):
+            assert abs(parts[k, q] - po[1 + q]) <= tol * abs(po[0]), (k, q)
+        assert rel(gk, go) <= tol, (k, rel(gk, go))
+        assert np.abs(gk - go).max() <= tol_max * np.abs(go).max(), (k, np.abs(gk - go).max() / np.abs(go).max())
+        if traj:
+            assert rel(g.get_local_trajectory(k).cpu().numpy(), tr) <= 1e-12, k
 
 
 def perturbed(o, prob, ks, seed, amp=0.5):
@@ -127,3 +150,65 @@ def test_config2_one_outer_iteration():
         po, go, _ = o.eval_local(k, o.get_control(k))
         assert abs(costs[k] - po[0]) <= 1e-8 * abs(po[0]), k
         assert rel(g.split(grads)[k].cpu().numpy(), go) <= 1e-8, k
+
+
+def test_config3_two_outer_iterations_and_exchanged_data():
+    """The headline config through Algorithm 1: run(2) against the oracle (analysis 1e-8 per field,
+    history 1e-8, step norm 1e-6), then 16 sampled subdomains re-evaluated on the EXCHANGED data:
+    pole-row tiles, tiles across the clamp latitude (50 deg: tile rows 3 and 12 of 16), first,
+    middle and last windows."""
+    w = synth.CONFIGS[3]
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    assert g.active_path in (2, 4) and g.nsub == 2048
+    an_o, hist_o = o.run(2)
+    an_g, hist_g = g.run(2)
+    an_g = an_g.cpu().numpy()
+    for f in range(3):
+        assert rel(an_g[f], an_o[f]) <= TOL_AN, (f, rel(an_g[f], an_o[f]))
+    assert rel(an_g - prob.xb, an_o - prob.xb) <= 1e-6
+    assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2]) + 1e-300), (hist_g, hist_o)
+    assert np.all(np.abs(hist_g[:, 2] - hist_o[:, 2]) <= 1e-6 * np.abs(hist_o[:, 2]) + 1e-12)
+    p12 = w.p_lon * w.p_lat
+    tile = lambda a, b: b * w.p_lon + a
+    sample = [0 * p12 + tile(0, 0), 0 * p12 + tile(9, 3), 0 * p12 + tile(15, 15), 1 * p12 + tile(4, 12),
+              2 * p12 + tile(7, 8), 3 * p12 + tile(0, 15), 3 * p12 + tile(11, 3), 4 * p12 + tile(8, 0),
+              4 * p12 + tile(15, 7), 5 * p12 + tile(2, 12), 5 * p12 + tile(13, 1), 6 * p12 + tile(6, 14),
+              7 * p12 + tile(0, 0), 7 * p12 + tile(15, 15), 7 * p12 + tile(5, 4), 7 * p12 + tile(10, 11)]
+    check_sample(o, g, prob, sample, 91, tol=1e-8, tol_max=1e-7)
+
+
+def test_config2_three_outer_iterations():
+    w = synth.CONFIGS[2]
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    an_o, hist_o = o.run(3)
+    an_g, hist_g = g.run(3)
+    an_g = an_g.cpu().numpy()
+    for f in range(3):
+        assert rel(an_g[f], an_o[f]) <= TOL_AN, (f, rel(an_g[f], an_o[f]))
+    assert np.all(np.abs(hist_g[:, :2] - hist_o[:, :2]) <= 1e-8 * np.abs(hist_o[:, :2]) + 1e-300)
+    assert np.all(np.abs(hist_g[:, 2] - hist_o[:, 2]) <= 1e-6 * np.abs(hist_o[:, 2]) + 1e-12)
+
+
+SWEEP_LAYOUTS = [(1, 1, 1, 0), (2, 2, 2, 2), (4, 4, 4, 1), (4, 4, 4, 2), (8, 8, 8, 1), (8, 8, 8, 2),
+                 (16, 16, 8, 1), (16, 16, 8, 2)]
+
+
+@pytest.mark.parametrize("lay", SWEEP_LAYOUTS, ids=lambda l: "%dx%dx%d_o%d" % l)
+def test_config4_every_layout_at_full_size(lay):
+    """BASELINE.json configs[4]: every layout of the decomposition sweep on the 720x360 / 128-step
+    problem, whichever kernel family serves it (generic for the large tiles, wavefront / row-marching
+    for the small ones, incl. the ragged 22/23-row tiles of 16x16x8): sampled subdomains at perturbed
+    controls, cost / parts / gradient element-wise / stored trajectory."""
+    w = synth.CONFIGS[2].with_layout(*lay)
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    n = o.nsub
+    sample = sorted(set([0, n - 1, n // 2, n // 3 + 1, (2 * n) // 3, n // 5]))[:6] if n > 8 else list(range(n))
+    check_sample(o, g, prob, sample, 17 + lay[0], traj=n > 1)
+    if n == 1:      # the undecomposed layout is plain global 4D-Var: eval_global agrees as well
+        x = prob.xb + 0.3 * prob.sigma_b[:, None, None] * synth.random_fields(prob.xb.shape, 3)
+        Jo, go, _ = o.eval_global(x)
+        Jg, gg = g.eval_global(x)
+        assert abs(Jg - Jo) <= TOL_EVAL * abs(Jo) and rel(gg.cpu().numpy(), go) <= TOL_EVAL
