@@ -324,10 +324,15 @@ def main():
     ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
     ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
+    ap.add_argument("--peaks", action="store_true", help="run the library's fp64 / shared-memory / shuffle microbenchmarks")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the CUDA sources (for profiles/traffic.json)")
     args = ap.parse_args()
     if args.csrc_hash:
         print(csrc_hash())
+        return
+    if args.peaks:
+        from paper_2205_06649_b200 import binding
+        print(json.dumps(binding.measure_peaks("cuda:0")))
         return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:

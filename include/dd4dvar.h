@@ -175,6 +175,22 @@ int dd4dvar_subdomain_info(dd4dvar_t h, int sub, int out[16]);
 long long dd4dvar_control_offset(dd4dvar_t h, int sub);
 /* which kernels serve the local sweeps: 1 generic, 2 fused persistent */
 int dd4dvar_active_path(dd4dvar_t h);
+
+/* Weight of the background term (25a) l.338 in the time windows j > 0 (R7).  The paper is
+ * at odds with itself here: (25a) is printed for every window, but eq (19) l.288 (J = sum of the
+ * local functionals) only holds beyond the background state if the term is counted where eq (6)
+ * l.111 has it, at t_0.  Default 0 (only window 0 carries (25a); the windows j > 0 are anchored by
+ * the predecessor term of (25c) instead); 1 = as printed.  Takes effect at the next evaluation;
+ * returns 0 or -1 (negative weight). */
+int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later);
+
+/* Measurement aid ("which roofline binds"): microbenchmarks of the device's
+ * fp64 FMA rate, fp64 ADD rate, shared-memory load bandwidth and 64-bit warp-shuffle rate, the
+ * secondary bounds of the stencil sweep next to HBM (SURVEY.md section 8(d) asks for the fp64 peak to
+ * be measured on the box).  h_out: [0] fp64 FMA TFLOP/s, [1] fp64 ADD 1e12 instr/s, [2] LDS.64
+ * bytes/s over all SMs, [3] 64-bit shuffles/s (per thread), [4] SM count, [5] SM clock MHz.
+ * Needs no handle; runs ~0.1 s on `cuda_stream`; returns 0, -1 (null argument) or -4. */
+int dd4dvar_measure_peaks(void* cuda_stream, double h_out[6]);
 /* number of kernel launches issued by this handle so far (bench.py's gpu_launches) */
 long long dd4dvar_launch_count(dd4dvar_t h);
 

@@ -342,6 +342,7 @@ typedef struct {
     int nsteps;
     int p1, p2, q, o;
     double mu, lambda;
+    double bgw;   /* weight of (25a) in windows j > 0 (0 = only at t_0, reading R7, the default; 1 = in every window as (25a) is printed) */
     int lbfgs_m, n_inner, max_bt; double c1;
     int nsub; Sub* sub;
     int *colown, *rowown;         /* owner tile column / row of a global column / row */
@@ -520,6 +521,7 @@ static void local_eval(const DD* d, int k, const double* x, CostParts* cp, doubl
     /* cost terms, eq (25) l.338-344, squared weighted 2-norms without 1/2 (R5) */
     long double Jbg = 0, Jobs = 0, Jsp = 0, Jpred = 0, Jsucc = 0;
     const double* ubs = ub_level(d, s->s);
+    const double bgw = s->jw == 0 ? 1.0 : d->bgw;      /* DESIGN.md R7 */
     for (int fl = 0; fl < NF; ++fl) {
         double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
         for (int lj = 0; lj < s->ey; ++lj)
@@ -528,7 +530,7 @@ static void local_eval(const DD* d, int k, const double* x, CostParts* cp, doubl
                 long c = (long)lj * s->ex + li;
                 double xv = x[(size_t)fl * nc + c];
                 double db = xv - ubs[gidx(d, fl, gj, gi)];
-                Jbg += (long double)(w_space(d, gi, gj) * db * db * ib);                    /* (25a) */
+                Jbg += (long double)(bgw * w_space(d, gi, gj) * db * db * ib);              /* (25a) */
                 /* (25c) case 1: every other extended tile of this window that contains the cell */
                 for (int cb = 0; cb < d->nrowcov[gj]; ++cb)
                     for (int ca = 0; ca < d->ncolcov[gi]; ++ca) {
@@ -618,7 +620,7 @@ static void local_eval(const DD* d, int k, const double* x, CostParts* cp, doubl
                     long c = (long)lj * s->ex + li;
                     double xv = x[(size_t)fl * nc + c];
                     double gsum = lam[(size_t)fl * nc + c];
-                    gsum += 2.0 * w_space(d, gi, gj) * (xv - ubs[gidx(d, fl, gj, gi)]) * ib;
+                    gsum += 2.0 * (s->jw == 0 ? 1.0 : d->bgw) * w_space(d, gi, gj) * (xv - ubs[gidx(d, fl, gj, gi)]) * ib;
                     for (int cb = 0; cb < d->nrowcov[gj]; ++cb)
                         for (int ca = 0; ca < d->ncolcov[gi]; ++ca) {
                             int a2 = d->colcov[4 * gi + ca], b2 = d->rowcov[4 * gj + cb];
@@ -826,7 +828,7 @@ void* orc_create(int nlon, int nlat, double radius, double omega, double gravity
     d->m.nlon = nlon; d->m.nlat = nlat; d->m.a = radius; d->m.Omega = omega; d->m.g = gravity;
     d->m.cos_clamp = cos_clamp; d->m.kappa = diffusion; d->m.dt = dt;
     d->nsteps = nsteps; d->p1 = p_lon; d->p2 = p_lat; d->q = q_time; d->o = overlap;
-    d->mu = mu; d->lambda = lambda;
+    d->mu = mu; d->lambda = lambda; d->bgw = 0.0;
     d->lbfgs_m = lbfgs_m; d->n_inner = n_inner; d->max_bt = max_bt; d->c1 = c1;
     if (nlon < 3 || nlat < 2 || nsteps < 1) { *status = -1; free(d); return NULL; }
     model_tables(&d->m);
@@ -839,6 +841,8 @@ void* orc_create(int nlon, int nlat, double radius, double omega, double gravity
     *status = 0;
     return d;
 }
+/* weight of the background term (25a) in the windows j > 0 (R7: default 0; 1 = as printed) */
+void orc_set_bg_weight(void* h, double w) { ((DD*)h)->bgw = w; }
 static void free_local(DD* d)
 {
     for (int k = 0; k < d->nsub; ++k) {

@@ -71,7 +71,7 @@ class Oracle:
     def __init__(self, nlon, nlat, dt, nsteps, p_lon=1, p_lat=1, q_time=1, overlap=0,
                  mu=1.0, lam=1.0, radius=6.371e6, omega=7.292e-5, gravity=9.806,
                  cos_clamp=float(np.cos(np.deg2rad(50.0))), diffusion=0.02,
-                 lbfgs_m=5, n_inner=5, max_backtrack=20, armijo_c1=1e-4):
+                 lbfgs_m=5, n_inner=5, max_backtrack=20, armijo_c1=1e-4, bg_later=0.0):
         lib = _load()
         st = C.c_int(0)
         self._h = lib.orc_create(nlon, nlat, radius, omega, gravity, cos_clamp, diffusion,
@@ -84,13 +84,14 @@ class Oracle:
         self.shape = (3, nlat, nlon)
         self.nsub = lib.orc_nsub(self._h)
         self.subs = [self.sub_info(k) for k in range(self.nsub)]
+        self.set_bg_weight(bg_later)
 
     @classmethod
     def from_workload(cls, w, **kw):
         args = dict(nlon=w.nlon, nlat=w.nlat, dt=w.dt, nsteps=w.nsteps, p_lon=w.p_lon,
                     p_lat=w.p_lat, q_time=w.q_time, overlap=w.overlap, mu=w.mu, lam=w.lam,
                     lbfgs_m=w.lbfgs_m, n_inner=w.n_inner, max_backtrack=w.max_backtrack,
-                    armijo_c1=w.armijo_c1)
+                    armijo_c1=w.armijo_c1, bg_later=getattr(w, "bg_later", 0.0))
         args.update(kw)
         return cls(**args)
 
@@ -104,6 +105,12 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+    def set_bg_weight(self, w):
+        """weight of (25a) in windows j > 0 (R7): 0 = only at t_0 (default), 1 = as printed"""
+        self.lib.orc_set_bg_weight.argtypes = [C.c_void_p, C.c_double]
+        self.lib.orc_set_bg_weight.restype = None
+        self.lib.orc_set_bg_weight(self._h, float(w))
 
     # ---- geometry
     def sub_info(self, k):

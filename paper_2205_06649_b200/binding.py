@@ -51,6 +51,7 @@ EXPORTS = [
     "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
+    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight",
     "dd4dvar_last_error", "dd4dvar_destroy",
 ]
 
@@ -90,6 +91,8 @@ def load_library():
     lib.dd4dvar_active_path.argtypes = [vp]
     lib.dd4dvar_launch_count.restype = C.c_longlong
     lib.dd4dvar_launch_count.argtypes = [vp]
+    lib.dd4dvar_measure_peaks.argtypes = [vp, hd]
+    lib.dd4dvar_set_bg_weight.argtypes = [vp, C.c_double]
     lib.dd4dvar_last_error.restype = C.c_char_p
     lib.dd4dvar_last_error.argtypes = [vp]
     lib.dd4dvar_destroy.restype = None
@@ -102,13 +105,31 @@ def _hd(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
+def measure_peaks(device="cuda:0"):
+    """dd4dvar_measure_peaks: fp64 FMA / ADD rates, LDS.64 bandwidth, 64-bit shuffle rate of the device."""
+    import numpy as np
+    import torch
+    lib = load_library()
+    dev = torch.device(device)
+    out = np.zeros(6)
+    with torch.cuda.device(dev):
+        st = torch.cuda.current_stream(dev)
+        rc = lib.dd4dvar_measure_peaks(C.c_void_p(st.cuda_stream), _hd(out))
+    if rc:
+        raise DD4DVarError("dd4dvar_measure_peaks", rc)
+    nsm, mhz = out[4], out[5]
+    return {"fp64_fma_tflops": out[0], "fp64_add_tinstr_s": out[1], "lds64_bytes_per_s": out[2],
+            "lds64_bytes_per_clk_per_sm": out[2] / (nsm * mhz * 1e6), "shfl64_per_s": out[3],
+            "shfl64_bytes_per_clk_per_sm": 8.0 * out[3] / (nsm * mhz * 1e6), "sm_count": int(nsm), "sm_clock_mhz": mhz}
+
+
 class DD4DVar:
     """One DD-4DVar problem on one GPU.  Tensors in and out are torch CUDA fp64 tensors."""
 
     def __init__(self, nlon, nlat, dt, nsteps, p_lon=1, p_lat=1, q_time=1, overlap=0, mu=1.0, lam=1.0,
                  radius=6.371e6, omega=7.292e-5, gravity=9.806,
                  cos_clamp=float(np.cos(np.deg2rad(50.0))), diffusion=0.02, lbfgs_m=5, n_inner=5,
-                 max_backtrack=20, armijo_c1=1e-4, path=0, device="cuda:0", stream=None):
+                 max_backtrack=20, armijo_c1=1e-4, path=0, device="cuda:0", stream=None, bg_later=0.0):
         import torch
         self.torch = torch
         self.lib = load_library()
@@ -127,6 +148,9 @@ class DD4DVar:
         if rc:
             raise DD4DVarError("dd4dvar_create", rc)
         self._h = h
+        rc = self.lib.dd4dvar_set_bg_weight(h, float(bg_later))
+        if rc:
+            raise DD4DVarError("dd4dvar_set_bg_weight", rc)
         self.nlon, self.nlat, self.nsteps = nlon, nlat, nsteps
         self.shape = (3, nlat, nlon)
         self.nsub = self.lib.dd4dvar_num_subdomains(h)
@@ -144,7 +168,8 @@ class DD4DVar:
     def from_workload(cls, w, **kw):
         args = dict(nlon=w.nlon, nlat=w.nlat, dt=w.dt, nsteps=w.nsteps, p_lon=w.p_lon, p_lat=w.p_lat,
                     q_time=w.q_time, overlap=w.overlap, mu=w.mu, lam=w.lam, lbfgs_m=w.lbfgs_m,
-                    n_inner=w.n_inner, max_backtrack=w.max_backtrack, armijo_c1=w.armijo_c1)
+                    n_inner=w.n_inner, max_backtrack=w.max_backtrack, armijo_c1=w.armijo_c1,
+                    bg_later=getattr(w, "bg_later", 0.0))
         args.update(kw)
         return cls(**args)
 

@@ -68,6 +68,7 @@ struct CostP {
     double ib[3];        // 1 / sigma_b^2 per field
     double sb[3];        // sigma_b
     double mu, lambda;
+    double bgw;          // weight of (25a) in the windows j > 0 (R7): 0 = only at t_0, 1 = as printed
 };
 
 __device__ __forceinline__ int imodd(int a, int n) { int r = a % n; return r < 0 ? r + n : r; }

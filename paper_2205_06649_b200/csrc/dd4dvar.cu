@@ -17,6 +17,7 @@
 #include "fused_kernels.cuh"
 #include "generic_kernels.cuh"
 #include "lbfgs_kernels.cuh"
+#include "peaks_kernels.cuh"
 #include "step_kernels.cuh"
 #include "wave_forward.cuh"
 #include "wave_adjoint.cuh"
@@ -552,7 +553,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     const double cm = 1.0 / (2.0 * a * dth);
     h->mp.nlon = nlon; h->mp.nlat = nlat; h->mp.kap = grid->diffusion;
     h->mp.dtcm = dt * cm; h->mp.gdtcm = grid->gravity * dt * cm;
-    h->cp.mu = decomp->mu; h->cp.lambda = decomp->lambda;
+    h->cp.mu = decomp->mu; h->cp.lambda = decomp->lambda; h->cp.bgw = 0.0;
     for (int f = 0; f < 3; ++f) { h->cp.ib[f] = 1.0; h->cp.sb[f] = 1.0; }
     int rc = build_layout(h->G, nlon, nlat, window->nsteps, 1, 1, 1, 0);
     if (!rc) rc = build_layout(h->L, nlon, nlat, window->nsteps, decomp->p_lon, decomp->p_lat, decomp->q_time,
@@ -953,6 +954,19 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
     }
     LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
     return sync_check(h);
+}
+
+int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
+{
+    if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
+    h->cp.bgw = w_later;
+    return 0;
+}
+
+int dd4dvar_measure_peaks(void* cuda_stream, double h_out[6])
+{
+    if (!h_out) return -1;
+    return measure_peaks((cudaStream_t)cuda_stream, h_out);
 }
 
 int dd4dvar_num_subdomains(dd4dvar_t h) { return h ? h->L.nsub : -1; }

@@ -268,7 +268,7 @@ __global__ void __launch_bounds__(FK_NT, FK_ADJ_CTAS * 128 / FK_NT) fk_adjoint2(
                 const long long o = s.coff + (long long)f * s.ncell + c;
                 const double xv = x[o];
                 double gg = lam[f * s.ncell + c];
-                gg += 2.0 * wsp * (xv - xbs[o]) * cp.ib[f];
+                gg += 2.0 * (s.jw == 0 ? 1.0 : cp.bgw) * wsp * (xv - xbs[o]) * cp.ib[f];
                 if (nc * nr > 1)
                     for (int cb = 0; cb < nr; ++cb)
                         for (int ca = 0; ca < nc; ++ca) {

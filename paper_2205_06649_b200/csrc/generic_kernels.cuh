@@ -335,7 +335,7 @@ __global__ void gk_cost_partial(const Sub* __restrict__ subs, const int* __restr
         for (int f = 0; f < DD_NF; ++f) {
             const double xv = xk[(long long)f * s.ncell + c];
             const double db = xv - xb[(long long)f * s.ncell + c];
-            bg += wsp * db * db * cp.ib[f];
+            bg += (s.jw == 0 ? 1.0 : cp.bgw) * wsp * db * db * cp.ib[f];
             if (nc * nr > 1)
                 for (int cb = 0; cb < nr; ++cb)
                     for (int ca = 0; ca < nc; ++ca) {
@@ -414,7 +414,7 @@ __global__ void gk_grad_final(const Sub* __restrict__ subs, const int* __restric
         const long long o = s.coff + (long long)f * s.ncell + c;
         const double xv = x[o];
         double g = lam[s.poff + (long long)f * s.npad + pc];
-        g += 2.0 * wsp * (xv - xbs[o]) * cp.ib[f];
+        g += 2.0 * (s.jw == 0 ? 1.0 : cp.bgw) * wsp * (xv - xbs[o]) * cp.ib[f];
         if (nc * nr > 1)
             for (int cb = 0; cb < nr; ++cb)
                 for (int ca = 0; ca < nc; ++ca) {

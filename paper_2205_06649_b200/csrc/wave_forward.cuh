@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
                 const int nr = A.geo.nrowcov[s.ej0 + lj];
                 for (int li = lane; li < g.ex; li += 32) {
                     int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
-                    const double wsp = 1.0 / (double)(A.geo.ncolcov[gi] * nr);
+                    const double wsp = (s.jw == 0 ? 1.0 : A.cp.bgw) / (double)(A.geo.ncolcov[gi] * nr);
                     const long long cg = s.coff + (long long)lj * g.ex + li;
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {

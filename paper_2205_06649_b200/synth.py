@@ -59,6 +59,7 @@ class Workload:
     seed_cfg: int | None = None   # config whose seeds are used (config 4 reuses config 2's)
     mu: float = 1.0
     lam: float = 1.0
+    bg_later: float = 0.0         # weight of the background term (25a) in windows j > 0 (R7)
     lbfgs_m: int = 5
     n_inner: int = 5
     max_backtrack: int = 20

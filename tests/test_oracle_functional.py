@@ -211,14 +211,16 @@ def test_lbfgs_cost_is_monotone_and_handles_zero_gradient():
 
 
 # ------------------------------------------------------------------ O9: outer loop
-def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity():
+@pytest.mark.parametrize("bgw", [0.0, 1.0])
+def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity(bgw):
     """Phi = identity decouples the grid points: each local solve is a per-point weighted mean
     of background, observations and the neighbours' frozen values (eq (25)); iterate that
-    Jacobi map in NumPy and compare every outer iteration's gathered analysis."""
+    Jacobi map in NumPy and compare every outer iteration's gathered analysis.  Both readings of
+    where (25a) acts (R7: weight bgw of the background term in the windows j > 0)."""
     w = synth.CONFIGS[0]
     nlon, nlat, N, ov, mu, lam = 12, 8, 4, 1, 0.8, 1.3
     o = Oracle(nlon, nlat, 0.0, N, p_lon=2, p_lat=2, q_time=2, overlap=ov, mu=mu, lam=lam,
-               diffusion=0.0, n_inner=60, lbfgs_m=10)
+               diffusion=0.0, n_inner=60, lbfgs_m=10, bg_later=bgw)
     rng = np.random.default_rng(9)
     xb = rng.standard_normal((3, nlat, nlon)); sb = np.array([1.0, 2.0, 0.5]); so = np.array([0.7, 0.9, 1.1])
     levels = np.array([0, 2, 4], dtype=np.int32)
@@ -241,7 +243,8 @@ def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity():
         for k, s in enumerate(subs):
             num = np.zeros_like(xb); den = np.zeros_like(xb)
             for f in range(3):
-                num[f] += xb[f] / mult / sb[f] ** 2; den[f] += 1.0 / mult / sb[f] ** 2
+                wb = 1.0 if s["jw"] == 0 else bgw
+                num[f] += wb * xb[f] / mult / sb[f] ** 2; den[f] += wb * 1.0 / mult / sb[f] ** 2
                 for t, lev in enumerate(levels):
                     if s["s"] <= lev <= s["e"]:
                         wt = 1.0 / mult.reshape(-1)[cells] / (2.0 if lev == 2 else 1.0)
@@ -261,7 +264,7 @@ def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity():
         X = Xn
         an_ref = sum(np.where(cover[k][None], X[k], 0.0) for k in range(4)) / mult
         o2 = Oracle(nlon, nlat, 0.0, N, p_lon=2, p_lat=2, q_time=2, overlap=ov, mu=mu, lam=lam,
-                    diffusion=0.0, n_inner=60, lbfgs_m=10)
+                    diffusion=0.0, n_inner=60, lbfgs_m=10, bg_later=bgw)
         o2.set_background(xb, sb); o2.set_observations(obs)
         an, hist = o2.run(it)
         assert np.abs(an - an_ref).max() < 1e-8, it
@@ -270,13 +273,15 @@ def test_outer_loop_reaches_the_consensus_fixed_point_when_model_is_identity():
 
 def test_config0_run_history_behaviour(c0):
     """Reported behaviour (no guarantee in the paper beyond Theorem 1's convex case): on config 0
-    J(gathered analysis), sum J_ji and delta_l all fall; the analysis beats the background."""
+    J(gathered analysis) and sum J_ji fall at every outer iteration, delta_l falls by more than 10x
+    over six iterations (not monotonically: the windows j > 0 are anchored only through (25c),
+    DESIGN.md R7); the analysis beats the background."""
     _, prob = c0
     o, _ = make(prob.w)
     an, hist = o.run(6)
     assert hist[0, 0] == pytest.approx(hist[0, 1], rel=1e-13)
     assert np.all(np.diff(hist[:, 0]) < 0) and np.all(np.diff(hist[1:, 1]) < 0)
-    assert np.all(np.diff(hist[1:, 2]) < 0)
+    assert hist[-1, 2] < 0.1 * hist[1, 2]
     for f in range(3):
         assert np.linalg.norm(an[f] - prob.truth0[f]) < 0.6 * np.linalg.norm(prob.xb[f] - prob.truth0[f])
     tr = o.get_trajectory(0)
