@@ -209,6 +209,19 @@ __device__ __forceinline__ bool wk_elect()
 // broadcast from lane 0: marks a value as warp-uniform for the compiler (uniform datapath, no vote loops)
 __device__ __forceinline__ int wk_uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
+// shared-memory access with an explicit 32-bit shared-window address and a compile-time byte offset
+// (the steady ticks keep running addresses in registers; volatile: program order is the schedule)
+template <int OFF> __device__ __forceinline__ double wk_lds(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+template <int OFF> __device__ __forceinline__ void wk_sts(uint32_t a, double v)
+{
+    asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(a), "n"(OFF), "d"(v) : "memory");
+}
+
 // 64-bit shuffles
 __device__ __forceinline__ double wk_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 __device__ __forceinline__ double wk_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }

@@ -266,6 +266,139 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
     if (t < g.py) { R.pa = ra; R.pfs = rfs; R.pe = re; }
 }
 
+// The same tick for the rows well inside the tile (rows t+1 .. t-3 are all tile rows, no wall event):
+// running 32-bit shared addresses, no row-kind branches.  Bit-identical arithmetic to wf_tick.
+template <int K>
+__device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<K>& C, double* __restrict__ sm,
+                                               const double* __restrict__ tab)
+{
+    const WkGeo& g = C.g;
+    const int lj = t - g.gys;
+    const uint32_t P8 = 8u * C.P, FS8 = 8u * C.FS;
+    WKP(7)
+    if (C.has_leader) wk_wait_prog(C.a_lead, C.need0 + (unsigned)t + 4u);
+    WKP(0)
+    // ---- loads: own columns of row t, E/W halo and edge u^a of row t-1
+    const uint32_t urow = C.sm32 + 8u * (C.st + lj * C.P);          // tile row lj, tile column 0, field 0
+    const uint32_t a0 = urow + 8u * (C.c0 - 3), a1 = a0 + FS8, a2 = a1 + FS8;
+    double z0[3][K], hz[3][2];
+    z0[0][0] = wk_lds<0>(a0); z0[1][0] = wk_lds<0>(a1); z0[2][0] = wk_lds<0>(a2);
+    if (K > 1) { z0[0][1] = wk_lds<8>(a0); z0[1][1] = wk_lds<8>(a1); z0[2][1] = wk_lds<8>(a2); }
+    if (K > 2) { z0[0][2] = wk_lds<16>(a0); z0[1][2] = wk_lds<16>(a1); z0[2][2] = wk_lds<16>(a2); }
+    hz[0][0] = wk_lds<-8>(a0 - P8); hz[1][0] = wk_lds<-8>(a1 - P8); hz[2][0] = wk_lds<-8>(a2 - P8);
+    hz[0][1] = wk_lds<8 * K>(a0 - P8); hz[1][1] = wk_lds<8 * K>(a1 - P8); hz[2][1] = wk_lds<8 * K>(a2 - P8);
+    const uint32_t ue = urow - P8 + 8u * (g.ex + 3);
+    const double eL = wk_lds<0>(ue), eR = wk_lds<8>(ue);
+    // ---- stage A on row t-1
+    double ha1[K], ua1[K], va1[K];
+    {
+        const double dtcz1 = tab[t * 8 + WK_T_DTCZ];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const double cu = dtcz1 * R.z1[1][i], cv = C.dtcm * R.z1[2][i];
+            double xa[3];
+#pragma unroll
+            for (int f = 0; f < 3; ++f) {
+                const double xE = i < K - 1 ? R.z1[f][i + 1 < K ? i + 1 : i] : hz[f][1];
+                const double xW = i > 0 ? R.z1[f][i > 0 ? i - 1 : 0] : hz[f][0];
+                xa[f] = mm_stageA(R.z1[f][i], xE, xW, z0[f][i], R.z2[f][i], cu, cv, C.kap);
+            }
+            ha1[i] = xa[0]; ua1[i] = xa[1]; va1[i] = xa[2];
+        }
+    }
+    double uaL1 = wk_up(ua1[K - 1]), uaR1 = wk_dn(ua1[0]);
+    uaL1 = C.injL ? eL : uaL1;
+    uaR1 = C.injR ? eR : uaR1;
+    // ---- h^1 and u^1 on row t-2
+    double h12[K], u12[K];
+    {
+        const double* tb = tab + t * 8 - 8;
+        const double dtcz2 = tb[WK_T_DTCZ], gdtcz2 = tb[WK_T_GDTCZ], dtf2 = tb[WK_T_DTF], dtt2 = tb[WK_T_DTT];
+        const double rp2 = tb[WK_T_RP], rm2 = tb[WK_T_RM];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const double uE = i < K - 1 ? R.ua2[i + 1 < K ? i + 1 : i] : R.uaR2;
+            const double uW = i > 0 ? R.ua2[i > 0 ? i - 1 : 0] : R.uaL2;
+            h12[i] = mm_h1(R.ha2[i], mm_div(uE, uW, va1[i], R.va3[i], dtcz2, C.dtcm, rp2, rm2));
+        }
+        const double hL = wk_up(h12[K - 1]), hR = wk_dn(h12[0]);
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const double hE = i < K - 1 ? h12[i + 1 < K ? i + 1 : i] : hR;
+            const double hW = i > 0 ? h12[i > 0 ? i - 1 : 0] : hL;
+            u12[i] = mm_u1(R.ua2[i], R.va2[i], hE, hW, gdtcz2, dtf2, dtt2);
+        }
+    }
+    WKP(2)
+    // ---- v^1 on row t-3 -> row t-3 of Z^{n+1}
+    {
+        const double dtf3 = tab[t * 8 - 16 + WK_T_DTF], dtt3 = tab[t * 8 - 16 + WK_T_DTT];
+        const uint32_t o0 = a0 - 3u * P8, o1 = o0 + FS8, o2 = o1 + FS8;
+        double v1[K];
+#pragma unroll
+        for (int i = 0; i < K; ++i) v1[i] = mm_v1(R.va3[i], R.u13[i], h12[i], R.h14[i], C.gdtcm, dtf3, dtt3);
+        if (C.tmask & 1u) { wk_sts<0>(o0, R.h13[0]); wk_sts<0>(o1, R.u13[0]); wk_sts<0>(o2, v1[0]); }
+        if (K > 1 && (C.tmask & 2u)) { wk_sts<8>(o0, R.h13[K > 1 ? 1 : 0]); wk_sts<8>(o1, R.u13[K > 1 ? 1 : 0]); wk_sts<8>(o2, v1[K > 1 ? 1 : 0]); }
+        if (K > 2 && (C.tmask & 4u)) { wk_sts<16>(o0, R.h13[K > 2 ? 2 : 0]); wk_sts<16>(o1, R.u13[K > 2 ? 2 : 0]); wk_sts<16>(o2, v1[K > 2 ? 2 : 0]); }
+        wk_fence_async();
+    }
+    WKP(3)
+    // ---- E/W ghost cells and edge u^a of row t+1 next to its tile row
+    const int l1 = lj + 1, l3 = lj - 3;
+    {
+        const int slot = (l1 / WK_EWC) & 1, lr = l1 % WK_EWC;
+        if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * slot, (C.par >> (1 + slot)) & 1u); C.par ^= 2u << slot; }
+        if (C.lane < 20) {
+            const double gv = wk_lds<0>(C.sm32 + 8u * (C.gcp_base + slot * C.gcp_ss + lr * C.gcp_rs));
+            wk_sts<0>(urow + P8 + 8u * C.gcp_dst, gv);
+        }
+    }
+    __syncwarp();
+    WKP(1)
+    // ---- one lane: progress word, trajectory stores, next E/W chunk
+    if (wk_elect()) {
+        wk_wait_read<2>();
+        wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
+        uint32_t src = urow - 3u * P8;
+        double* dst = C.tout + l3 * g.ex;
+#pragma unroll 1
+        for (int f = 0; f < 3; ++f) { wk_s2g32(dst, src, g.ex * 8u); dst += g.ncell; src += FS8; }
+        wk_commit();
+        if ((l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
+    }
+    WKP(4)
+    // ---- H (25b) at level n+1 on row t-3
+    if (C.have_obs) {
+        const WkArgs& A = *C.A;
+        for (;;) {
+            const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == l3);
+            const int cnt = __popc(mm);
+            if (cnt == 0) break;
+            if (C.lane < cnt) {
+                const double rr = sm[C.st + ((C.p_pk >> 8) & 3) * C.FS + l3 * C.P + (C.p_pk & 255)] - C.p_y;
+                C.obw += C.p_c * rr * rr;
+                A.obs_r[C.qcur + C.lane] = 2.0 * C.p_c * rr;
+            }
+            C.qcur += cnt;
+            C.p_pk = 0x7fffffff;
+            if (C.qcur + C.lane < C.qend) {
+                C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_y = A.obs_y[C.qcur + C.lane]; C.p_c = A.obs_c[C.qcur + C.lane];
+            }
+            if (cnt < 32) break;
+        }
+    }
+    WKP(5)
+    // ---- rotate the row histories
+#pragma unroll
+    for (int i = 0; i < K; ++i) {
+#pragma unroll
+        for (int f = 0; f < 3; ++f) { R.z2[f][i] = R.z1[f][i]; R.z1[f][i] = z0[f][i]; }
+        R.ha2[i] = ha1[i]; R.ua2[i] = ua1[i]; R.va3[i] = R.va2[i]; R.va2[i] = va1[i];
+        R.h14[i] = R.h13[i]; R.h13[i] = h12[i]; R.u13[i] = u12[i];
+    }
+    R.uaL2 = uaL1; R.uaR2 = uaR1;
+}
+
 template <int K>
 __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ WkArgs A)
 {
@@ -440,12 +573,22 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
                 wf_prep_row<K>(C, sm, 0);
                 __syncwarp();
             }
-            const int T3 = (C.T + 2) / 3 * 3;
+            // steady ticks: rows t-3 .. t+1 are tile rows and no wall event falls on the tick
+            int ts0 = g.gys + 3; if (ts0 < 4) ts0 = 4;
+            const int ts1 = g.gys + g.ey - 1;
 #pragma unroll 1
-            for (int t = 0; t < T3; t += 3) {
-                wf_tick<K>(t, R, C, sm, tab);
-                wf_tick<K>(t + 1, R, C, sm, tab);
-                wf_tick<K>(t + 2, R, C, sm, tab);
+            for (int t = 0; t < C.T;) {
+                if (t >= ts0 && t + 3 <= ts1) {
+                    wf_tick_steady<K>(t, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 1, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 2, R, C, sm, tab);
+                    t += 3;
+                    const int rowb = C.st + (t - 1 - g.gys) * C.P;      // row t-1 for the generic tick that may follow
+                    R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
+                } else {
+                    wf_tick<K>(t, R, C, sm, tab);
+                    ++t;
+                }
             }
             // step done: all its stores have left shared memory
             if (wk_elect()) { wk_wait_read<0>(); wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u); }
