@@ -409,10 +409,30 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
     if (L.path == 5) {
         cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
-        const WkArgs a = wave_args(h, L, mask, nullptr, gw);
+        WkArgs a = wave_args(h, L, mask, nullptr, gw);
+#ifdef WK_PROF
+        static unsigned long long* d_prof = nullptr;
+        if (!d_prof) cudaMalloc(&d_prof, 8 * 16 * 8);
+        cudaMemsetAsync(d_prof, 0, 8 * 16 * 8, h->stream);
+        a.J = reinterpret_cast<double*>(d_prof);
+#endif
         if (L.wp.K == 2) wk_adjoint<2><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
         else wk_adjoint<3><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
         ++h->launches;
+#ifdef WK_PROF
+        {
+            unsigned long long hp[8 * 16];
+            cudaStreamSynchronize(h->stream);
+            cudaMemcpy(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost);
+            static int nprint = 0;
+            if (nprint++ < 1)
+                for (int w = 0; w < 8; ++w) {
+                    fprintf(stderr, "[wkprof adj] warp %d:", w);
+                    for (int q = 0; q < 12; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
+                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, prep-wait, loads+row1, A+scatter, elected, obs, stores, gap | init, steps, epilogue, fetch)\n");
+                }
+        }
+#endif
         return;
     }
     if (L.path == 2 || L.path == 4) {

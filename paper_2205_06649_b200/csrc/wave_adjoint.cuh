@@ -3,39 +3,47 @@
 //
 // Warp w of the CTA runs adjoint steps m = w, w + WK_NW, ... (m-th step: lambda^n -> lambda^{n-1},
 // n = W - m; eq (3)-(4) l.91-98: the window adjoint is the product of the step adjoints in reverse).
-// Resident in shared memory, updated IN PLACE row by row: lambda [3][ey][ex] (zero outside the
-// extended tile, so ghost cells are never stored) and u^n [ey][ex] (the step needs u^1 = u^n of the
+// Resident in shared memory, updated IN PLACE row by row: lambda [3][ey][32 K] (zero outside the
+// extended tile, so ghost cells are never stored) and u^n [ey][32 K] (the step needs u^1 = u^n of the
 // forward step it transposes; the warp of step m leaves u^{n-1}, which it reads anyway, for the
 // warp of step m+1).  The linearisation state Z^{n-1} (trajectory store + frozen ghost ring) arrives
 // through TMA bulk copies in a per-warp ring of three padded rows.
 //
-// The step adjoint is the transpose of Phi (model_math.cuh) about Z^{n-1}, evaluated row by row:
-//   tick t:  stage A recomputed on row t-1 (h^a, u^a, v^a and the differences x_N - x_S);
-//            UB, HB, P on row t-1;  A_h, A_u, A_v on row t-2;
-//            L0 in SCATTER form from row t-2: A(row t-2) adds its centre and east/west parts to
-//            row t-2, its southward part to row t-3 (which is then complete and stored) and
-//            starts row t-1 with its northward part.  All coefficients of the scatter are local
-//            to row t-2 (c_u = dtcz u0, c_v = dtcm v0), so only products cross lanes (shuffles).
+// The step adjoint is the transpose of Phi (model_math.cuh) about Z^{n-1}, evaluated row by row.
+// Tick t works on three rows at once (software pipeline inside the warp):
+//   row t-1:  stage A recomputed (h^a, u^a, v^a and the differences x_N - x_S); UB, HB, P; and every
+//             part of A_h, A_u, A_v that does not need row t:
+//               A_u                                   (complete: it only uses row t-1)
+//               e   = 1 - dtcz (u^a_E - u^a_W) + dtcm r- v^a_S        (A_h = HB (e - dtcm r+ v^a_N))
+//               avp = vb + UB (dtf + dtt u^a) + dtcm r+_{j-1} P_S     (A_v = avp - dtcm r-_{j+1} P_N)
+//   row t-2:  A_h, A_v completed with v^a and P of row t-1; L0 in SCATTER form: A(row t-2) adds its
+//             centre and east/west parts to row t-2, its southward part to row t-3 (which is then
+//             complete and stored) and starts row t-1 with its northward part.  All coefficients of
+//             the scatter are local to row t-2 (c_u = dtcz u0, c_v = dtcm v0), so only products
+//             cross lanes (shuffles).
+// Every row history has depth one or two, so a group of six ticks returns every value to the register it
+// started in: the steady loop (rows well inside the tile) is unrolled by six with compile-time slots and
+// has no register moves, no row-kind branches and immediate shared-memory offsets.  The remaining
+// ticks (ghost rows, pole walls, tails) run the same code with the uniform row-kind tests switched on,
+// at slot 0, followed by an explicit rotation.
 // Reflective pole walls (R4): mirrored virtual rows -1 / py as in model_math.cuh; in
 // scatter form the part that would leave through the wall comes back into the edge row with the
 // sign of the mirrored field.
 #pragma once
 #include "wave_common.cuh"
 
-template <int K> struct WaRegs {
-    double z1[3][K], z2[3][K];      // Z^{n-1} rows t-1, t-2 (own columns)
-    double hz2[3][2];               // E/W halo of row t-2
-    double dn2[3][K];               // x_N - x_S on row t-2
-    double ua2[K], va2[K], va3[K], uaL2, uaR2;
-    double vb1[K], vb2[K];          // lambda_v rows t-1, t-2
-    double UB2[K], HB2[K], P2[K], P3[K];
-    double La[3][K], Lb[3][K];      // unfinished L0 of rows t-2 and t-3
-    int pa, pe, pe2;                // row t-1 in the ring: own column 0 of field 0, the two edge-u^a cells
+template <int K> struct WaState {
+    double z[3][3][K];              // [slot][field][column]: Z^{n-1} rows t, t-1, t-2 (period 3)
+    double L[3][3][K];              // unfinished L0 of rows t-1 (started this tick), t-2, t-3 (period 3)
+    double hz[2][3][2];             // E/W halo of rows t-1, t-2 (period 2)
+    double dn[2][3][K];             // x_N - x_S on rows t-1, t-2
+    double va[2][K], P[2][K], e[2][K], HB[2][K], Au[2][K], avp[2][K];   // rows t-1, t-2
 };
 template <int K> struct WaCtx {
     WkGeo g;
-    int lam, FS, u1, I_ZR, ZP, I_EW, I_EDS, I_EDE, T;
+    int lam, FS, u1, I_ZR, ZP, I_EW, I_EDS, I_EDE, T, maxey;
     uint32_t sm32, a_lead, a_mine, b_z, b_ew;
+    uint32_t zl, zu, SL8, ZP8, FS8, la0;     // per-lane ring / lambda base addresses (shared window), strides in bytes
     unsigned gs10, need0;
     bool has_leader, have_obs, injL, injR, lane0, laneL;    // lane0 / laneL: first lane, lane 31
     int c0, lane, nchunk;
@@ -47,6 +55,9 @@ template <int K> struct WaCtx {
     long long qcur, qend;
     int p_pk; double p_r;
     unsigned par;                   // bits 0..2: ring slots, bits 3, 4: E/W chunk slots
+#ifdef WK_PROF
+    long long pf[8], pt;
+#endif
 };
 
 // lane 0: padded row r of Z^{n-1} -> ring slot r % 3 (ghost rows whole, tile rows at columns 3 .. 3+ex)
@@ -56,16 +67,29 @@ __device__ __forceinline__ void wa_issue_row(const WaCtx<K>& C, int r, bool with
     const WkGeo& g = C.g;
     const int slot = r % 3;
     const uint32_t bar = C.b_z + 8u * slot;
-    uint32_t dst = C.sm32 + 8u * (C.I_ZR + slot * 3 * C.ZP);
+    uint32_t dst = C.zu + slot * C.SL8;
     const int lj = r - g.gys;
     const double* src; uint32_t bytes; long long fstride;
     if ((unsigned)lj < (unsigned)g.ey) { src = C.tz + lj * g.ex; bytes = g.ex * 8u; fstride = g.ncell; dst += 32u; }
     else { src = C.gz + (lj < 0 ? r : g.gys + lj - g.ey) * g.px; bytes = g.px * 8u; fstride = g.nring; }
     wk_mbar_expect32(bar, 3u * bytes + (with_edges ? (uint32_t)(g.gys + g.gyn) * 16u : 0u));
 #pragma unroll 1
-    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, bytes, bar); dst += 8u * C.ZP; src += fstride; }
+    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, bytes, bar); dst += C.ZP8; src += fstride; }
     if (with_edges && g.gys) wk_g2s32(C.sm32 + 8u * C.I_EDS, C.ge, g.gys * 16u, bar);
     if (with_edges && g.gyn) wk_g2s32(C.sm32 + 8u * (C.I_EDS + 8), C.ge + g.gys * 2, g.gyn * 16u, bar);
+}
+// the same for a tile row (tile row l2) into the compile-time slot SLOT
+template <int K>
+__device__ __forceinline__ void wa_issue_tile_row(const WaCtx<K>& C, int l2, const int SLOT)
+{
+    const uint32_t bar = C.b_z + 8u * SLOT;
+    const uint32_t bytes = C.g.ex * 8u;
+    const uint32_t dst = C.zu + SLOT * C.SL8 + 32u;
+    const double* src = C.tz + l2 * C.g.ex;
+    wk_mbar_expect32(bar, 3u * bytes);
+    wk_g2s32(dst, src, bytes, bar);
+    wk_g2s32(dst + C.ZP8, src + C.g.ncell, bytes, bar);
+    wk_g2s32(dst + 2u * C.ZP8, src + 2 * C.g.ncell, bytes, bar);
 }
 template <int K>
 __device__ __forceinline__ void wa_issue_chunk(const WaCtx<K>& C, int c)
@@ -96,24 +120,118 @@ __device__ __forceinline__ void wa_prep_row(WaCtx<K>& C, double* __restrict__ sm
         if (C.lane < 20) sm[C.I_ZR + slot * 3 * C.ZP + C.gcp_dst] = sm[C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs];
     }
 }
-
+// the same for a tile row (tile row l) in the compile-time slot SLOT
 template <int K>
-__device__ __forceinline__ void wa_tick(const int t, WaRegs<K>& R, WaCtx<K>& C, double* __restrict__ sm,
+__device__ __forceinline__ void wa_prep_tile_row(WaCtx<K>& C, int l, const int SLOT)
+{
+    wk_mbar_wait32(C.b_z + 8u * SLOT, (C.par >> SLOT) & 1u); C.par ^= 1u << SLOT;
+    const int cs = (l / WK_EWC) & 1, lr = l % WK_EWC;
+    if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * cs, (C.par >> (3 + cs)) & 1u); C.par ^= 8u << cs; }
+    if (C.lane < 20) {
+        const double gv = wk_lds<0>(C.sm32 + 8u * (C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs));
+        wk_sts<0>(C.zu + SLOT * C.SL8 + 8u * C.gcp_dst, gv);
+    }
+}
+
+#define WA_E(arr, i, edge) ((i) < K - 1 ? (arr)[(i) + 1 < K ? (i) + 1 : (i)] : (edge))
+#define WA_W(arr, i, edge) ((i) > 0 ? (arr)[(i) > 0 ? (i) - 1 : 0] : (edge))
+
+// One tick.  P3 / P2: register slots of this tick (t mod 3, t mod 2 counted from the canonical state);
+// EDGE = false: rows t-3 .. t+2 are tile rows, no wall event.
+template <int K, int P3, int P2, bool EDGE>
+__device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C, double* __restrict__ sm,
                                         const double* __restrict__ tab)
 {
+    constexpr int zn = P3, zc = (P3 + 2) % 3, zs = (P3 + 1) % 3, pn = P2, po = 1 - P2;
+    constexpr uint32_t PL8 = 8u * 32u * K;          // lambda row pitch in bytes
     const WkGeo& g = C.g;
     const int lj = t - g.gys;
-    const bool tile = (unsigned)lj < (unsigned)g.ey;
-    const int ci0 = C.c0 - 3;                       // tile column of own column 0
+    const bool tile = EDGE ? (unsigned)lj < (unsigned)g.ey : true;
+    const bool tile1 = EDGE ? (unsigned)(lj - 1) < (unsigned)g.ey : true;
+    double (&zN)[3][K] = S.z[zn];
+    double (&zC)[3][K] = S.z[zc];
+    double (&zS)[3][K] = S.z[zs];
+    WKP(7)
+
+    // ---- (1) Z^{n-1}: own columns of row t, E/W halo and edge u^a of row t-1
+    double eL, eR;
+    {
+        const int s0 = t % 3, s1 = s0 == 0 ? 2 : s0 - 1;             // ring slots of rows t, t-1
+        if (!EDGE || t < g.py) {
+            const uint32_t a0 = C.zl + s0 * C.SL8 + (tile ? 8u : 0u), a1 = a0 + C.ZP8, a2 = a1 + C.ZP8;
+            zN[0][0] = wk_lds<0>(a0); zN[1][0] = wk_lds<0>(a1); zN[2][0] = wk_lds<0>(a2);
+            if (K > 1) { zN[0][K > 1 ? 1 : 0] = wk_lds<8>(a0); zN[1][K > 1 ? 1 : 0] = wk_lds<8>(a1); zN[2][K > 1 ? 1 : 0] = wk_lds<8>(a2); }
+            if (K > 2) { zN[0][K > 2 ? 2 : 0] = wk_lds<16>(a0); zN[1][K > 2 ? 2 : 0] = wk_lds<16>(a1); zN[2][K > 2 ? 2 : 0] = wk_lds<16>(a2); }
+        } else {
+            const double sg = (t == g.py && g.wn) ? -1.0 : 1.0;     // virtual mirrored row py
+#pragma unroll
+            for (int i = 0; i < K; ++i) { zN[0][i] = zC[0][i]; zN[1][i] = zC[1][i]; zN[2][i] = sg * zC[2][i]; }
+        }
+        const uint32_t h0 = C.zl + s1 * C.SL8 + (tile1 ? 8u : 0u), h1 = h0 + C.ZP8, h2 = h1 + C.ZP8;
+        S.hz[pn][0][0] = wk_lds<-8>(h0); S.hz[pn][1][0] = wk_lds<-8>(h1); S.hz[pn][2][0] = wk_lds<-8>(h2);
+        S.hz[pn][0][1] = wk_lds<8 * K>(h0); S.hz[pn][1][1] = wk_lds<8 * K>(h1); S.hz[pn][2][1] = wk_lds<8 * K>(h2);
+        uint32_t ea, eb;
+        if (tile1) { ea = C.zu + s1 * C.SL8; eb = ea + C.ZP8; }
+        else {
+            const int l1 = lj - 1;
+            ea = C.sm32 + 8u * (uint32_t)(C.I_EDS + (l1 >= g.ey ? 8 + (l1 - g.ey) * 2 : (t > 0 ? (t - 1) * 2 : 0)));
+            eb = ea + 8u;
+        }
+        eL = wk_lds<0>(ea); eR = wk_lds<0>(eb);
+    }
+    if (EDGE && g.ws && t == 1) {                   // virtual row -1 (R4)
+#pragma unroll
+        for (int i = 0; i < K; ++i) { zS[0][i] = zC[0][i]; zS[1][i] = zC[1][i]; zS[2][i] = -zC[2][i]; }
+    }
+    const bool stage2 = EDGE ? t <= g.py : true;    // row t-1 is a padded row
+    const bool vrN = EDGE ? (g.wn && t == g.py + 1) : false;     // row t-1 is the virtual row py
+    const double* t1 = tab + t * 8;                 // table entry of row t-1
+    const double* t2 = EDGE ? tab + (t > 0 ? t - 1 : 0) * 8 : t1 - 8;      // row t-2
+
+    // ---- (2a) row t-1: stage A recomputed
+    double ha1[K], ua1[K], uaW, uaE;
+    if (stage2) {
+        const double dtcz1 = t1[WK_T_DTCZ];
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const double cu = dtcz1 * zC[1][i], cv = C.dtcm * zC[2][i];
+            double xa[3];
+#pragma unroll
+            for (int f = 0; f < 3; ++f) {
+                const double xE = WA_E(zC[f], i, S.hz[pn][f][1]);
+                const double xW = WA_W(zC[f], i, S.hz[pn][f][0]);
+                const double dnf = zN[f][i] - zS[f][i];
+                S.dn[pn][f][i] = dnf;
+                xa[f] = zC[f][i] - (cu * (xE - xW) + cv * dnf) + C.kap * (xE + xW + zN[f][i] + zS[f][i] - 4.0 * zC[f][i]);
+            }
+            ha1[i] = xa[0]; ua1[i] = xa[1]; S.va[pn][i] = xa[2];
+        }
+        uaW = wk_up(ua1[K - 1]); uaE = wk_dn(ua1[0]);
+        uaW = C.injL ? eL : uaW; uaE = C.injR ? eR : uaE;     // frozen u^a of the ghost columns 1 and px-2 (xk_edge_ua)
+    } else {
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            ha1[i] = 0.0; ua1[i] = 0.0; S.va[pn][i] = vrN ? -S.va[po][i] : 0.0;     // virtual row py: v^a mirrored
+#pragma unroll
+            for (int f = 0; f < 3; ++f) S.dn[pn][f][i] = 0.0;
+        }
+        uaW = 0.0; uaE = 0.0;
+    }
+    WKP(2)
+
     // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row
-    if (C.has_leader) { const int nd = t + 4 < C.T + 1 ? t + 4 : C.T + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+    if (C.has_leader) {
+        const int nd = EDGE ? (t + 4 < C.T + 1 ? t + 4 : C.T + 1) : t + 4;
+        wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
+    }
+    WKP(0)
     if (tile && C.have_obs) {
         const WkArgs& A = *C.A;
         for (;;) {
             const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == lj);
             const int cnt = __popc(mm);
             if (cnt == 0) break;
-            if (C.lane < cnt) sm[C.lam + ((C.p_pk >> 8) & 3) * C.FS + lj * g.ex + (C.p_pk & 255)] += C.p_r;
+            if (C.lane < cnt) sm[C.lam + ((C.p_pk >> 8) & 3) * C.FS + lj * (32 * K) + 1 + (C.p_pk & 255)] += C.p_r;
             C.qcur += cnt;
             C.p_pk = 0x7fffffff;
             if (C.qcur + C.lane < C.qend) { C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_r = A.obs_r[C.qcur + C.lane]; }
@@ -121,193 +239,168 @@ __device__ __forceinline__ void wa_tick(const int t, WaRegs<K>& R, WaCtx<K>& C, 
         }
         __syncwarp();
     }
-    // ---- (1) loads
-    const int zb = C.I_ZR + (t % 3) * 3 * C.ZP;
-    int ra = 0, re = 0, re2 = 0;
-    if (tile) { ra = zb + 1 + C.c0; re = zb; re2 = zb + C.ZP; }
-    else if (t < g.py) { const bool north = lj >= g.ey; ra = zb + C.c0; re = C.I_EDS + (north ? 8 + (lj - g.ey) * 2 : t * 2); re2 = re + 1; }
-    double z0[3][K], hz1[3][2], vb0[K], hb1[K], ub1[K], u1r[K];
-    if (t < g.py) {
-#pragma unroll
-        for (int f = 0; f < 3; ++f)
-#pragma unroll
-            for (int i = 0; i < K; ++i) z0[f][i] = sm[ra + f * C.ZP + i];
-    } else {
-        const double sg = (t == g.py && g.wn) ? -1.0 : 1.0;     // virtual mirrored row py
-#pragma unroll
-        for (int i = 0; i < K; ++i) { z0[0][i] = R.z1[0][i]; z0[1][i] = R.z1[1][i]; z0[2][i] = sg * R.z1[2][i]; }
-    }
-#pragma unroll
-    for (int f = 0; f < 3; ++f) { hz1[f][0] = sm[R.pa + f * C.ZP - 1]; hz1[f][1] = sm[R.pa + f * C.ZP + K]; }
-    const double eL = sm[R.pe], eR = sm[R.pe2];
-    {
-        const int o0 = C.lam + lj * g.ex + ci0;     // lambda row t (v), row t-1 (h, u), u^n row t-1
-        const bool tile1 = (unsigned)(lj - 1) < (unsigned)g.ey;
-#pragma unroll
-        for (int i = 0; i < K; ++i) {
-            const bool tc = (C.tmask >> i) & 1u;
-            vb0[i] = (tile && tc) ? sm[o0 + 2 * C.FS + i] : 0.0;
-            hb1[i] = (tile1 && tc) ? sm[o0 - g.ex + i] : 0.0;
-            ub1[i] = (tile1 && tc) ? sm[o0 - g.ex + C.FS + i] : 0.0;
-            u1r[i] = (tile1 && tc) ? sm[C.u1 + (lj - 1) * g.ex + ci0 + i] : 0.0;
-        }
-    }
-    if (g.wn && t == g.py) {                        // virtual row py: lambda_v mirrored
-#pragma unroll
-        for (int i = 0; i < K; ++i) vb0[i] = -R.vb1[i];
-    }
-    if (g.ws && t <= 2) {                           // virtual row -1
-        if (t == 1) {
-#pragma unroll
-            for (int i = 0; i < K; ++i) { R.z2[0][i] = R.z1[0][i]; R.z2[1][i] = R.z1[1][i]; R.z2[2][i] = -R.z1[2][i]; R.vb2[i] = -R.vb1[i]; }
-        }
-        if (t == 2) {
-            const double rm0 = tab[8 + WK_T_RM];
-#pragma unroll
-            for (int i = 0; i < K; ++i) { R.va3[i] = -R.va2[i]; R.P3[i] = rm0 * R.P2[i]; }
-        }
-    }
+    WKP(5)
 
-    // ---- (2) row t-1: stage A recomputed, UB, HB, P
-    double ua1[K], va1[K], dn1[3][K], UB1[K], HB1[K], P1[K], uaL1, uaR1;
-    if (t <= g.py) {
-        const double* tb = tab + t * 8;
-        const double dtcz1 = tb[WK_T_DTCZ], gdtcz1 = tb[WK_T_GDTCZ], dtf1 = tb[WK_T_DTF], dtt1 = tb[WK_T_DTT];
-        double ha1[K];
-#pragma unroll
-        for (int i = 0; i < K; ++i) {
-            const double cu = dtcz1 * R.z1[1][i], cv = C.dtcm * R.z1[2][i];
-            double xa[3];
-#pragma unroll
-            for (int f = 0; f < 3; ++f) {
-                const double xE = i < K - 1 ? R.z1[f][i + 1 < K ? i + 1 : i] : hz1[f][1];
-                const double xW = i > 0 ? R.z1[f][i > 0 ? i - 1 : 0] : hz1[f][0];
-                dn1[f][i] = z0[f][i] - R.z2[f][i];
-                xa[f] = R.z1[f][i] - (cu * (xE - xW) + cv * dn1[f][i]) +
-                        C.kap * (xE + xW + z0[f][i] + R.z2[f][i] - 4.0 * R.z1[f][i]);
-            }
-            ha1[i] = xa[0]; ua1[i] = xa[1]; va1[i] = xa[2];
-            UB1[i] = mm_UB(ub1[i], R.vb1[i], u1r[i], dtf1, dtt1);
+    // ---- (2b) lambda^n: v rows t, t-1, t-2; h, u and u^n row t-1.  UB, HB, P and the row-local parts of A on row t-1
+    const uint32_t lrow = C.la0 + (uint32_t)lj * PL8;      // own cell 0 of lambda_h, tile row lj (may be outside: EDGE)
+    double P1[K];
+    if (stage2) {
+        const uint32_t zrow = C.la0 + (uint32_t)C.maxey * PL8;          // the all-zero row
+        const uint32_t ah = tile1 ? lrow - PL8 : zrow, au = ah + C.FS8, a1 = ah + 3u * C.FS8, ac = ah + 2u * C.FS8;
+        const double dtcz1 = t1[WK_T_DTCZ], gdtcz1 = t1[WK_T_GDTCZ], dtf1 = t1[WK_T_DTF], dtt1 = t1[WK_T_DTT];
+        const double cmrm1 = t1[WK_T_CMRM], cmrp2 = t2[WK_T_CMRP];
+        double hb1[K], ub1[K], u1r[K], vbN[K], vbC[K], vbS[K];
+        {
+            // (rows t-1 and t-2 of lambda_v are still in place: row r is overwritten at tick r + 3)
+            const bool tile2 = EDGE ? (unsigned)(lj - 2) < (unsigned)g.ey : true;
+            const uint32_t av = (tile ? lrow : zrow) + 2u * C.FS8, as = (tile2 ? lrow - 2u * PL8 : zrow) + 2u * C.FS8;
+            vbN[0] = wk_lds<0>(av); hb1[0] = wk_lds<0>(ah); ub1[0] = wk_lds<0>(au); u1r[0] = wk_lds<0>(a1);
+            vbC[0] = wk_lds<0>(ac); vbS[0] = wk_lds<0>(as);
+            if (K > 1) { vbN[K > 1 ? 1 : 0] = wk_lds<8>(av); hb1[K > 1 ? 1 : 0] = wk_lds<8>(ah); ub1[K > 1 ? 1 : 0] = wk_lds<8>(au); u1r[K > 1 ? 1 : 0] = wk_lds<8>(a1);
+                         vbC[K > 1 ? 1 : 0] = wk_lds<8>(ac); vbS[K > 1 ? 1 : 0] = wk_lds<8>(as); }
+            if (K > 2) { vbN[K > 2 ? 2 : 0] = wk_lds<16>(av); hb1[K > 2 ? 2 : 0] = wk_lds<16>(ah); ub1[K > 2 ? 2 : 0] = wk_lds<16>(au); u1r[K > 2 ? 2 : 0] = wk_lds<16>(a1);
+                         vbC[K > 2 ? 2 : 0] = wk_lds<16>(ac); vbS[K > 2 ? 2 : 0] = wk_lds<16>(as); }
         }
-        uaL1 = wk_up(ua1[K - 1]); uaR1 = wk_dn(ua1[0]);
-        uaL1 = C.injL ? eL : uaL1; uaR1 = C.injR ? eR : uaR1;
-        double UBL = wk_up(UB1[K - 1]), UBR = wk_dn(UB1[0]);
-        UBL = C.lane0 ? 0.0 : UBL; UBR = C.laneL ? 0.0 : UBR;      // ghost columns: lambda = 0
+        if (EDGE && g.ws && t == 1) {               // virtual row -1: lambda_v mirrored
+#pragma unroll
+            for (int i = 0; i < K; ++i) vbS[i] = -vbC[i];
+        }
+        if (EDGE && g.wn && t == g.py) {            // virtual row py: lambda_v mirrored
+#pragma unroll
+            for (int i = 0; i < K; ++i) vbN[i] = -vbC[i];
+        }
+        double UB1[K];
+#pragma unroll
+        for (int i = 0; i < K; ++i) UB1[i] = mm_UB(ub1[i], vbC[i], u1r[i], dtf1, dtt1);
+        double UBW = wk_up(UB1[K - 1]), UBE = wk_dn(UB1[0]);
+        UBW = C.lane0 ? 0.0 : UBW; UBE = C.laneL ? 0.0 : UBE;          // ghost columns: lambda = 0
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            const double UE = i < K - 1 ? UB1[i + 1 < K ? i + 1 : i] : UBR;
-            const double UW = i > 0 ? UB1[i > 0 ? i - 1 : 0] : UBL;
-            HB1[i] = mm_HB(hb1[i], vb0[i], R.vb2[i], UE, UW, C.gdtcm, gdtcz1);
-            P1[i] = -ha1[i] * HB1[i];
+            const double hb = mm_HB(hb1[i], vbN[i], vbS[i], WA_E(UB1, i, UBE), WA_W(UB1, i, UBW), C.gdtcm, gdtcz1);
+            P1[i] = -ha1[i] * hb;
+            S.HB[pn][i] = hb;                       // (HB of row t-2 sits in the other slot until (3) has read it)
+        }
+        double PW = wk_up(P1[K - 1]), PE = wk_dn(P1[0]);
+        PW = C.lane0 ? 0.0 : PW; PE = C.laneL ? 0.0 : PE;
+        const bool wS1 = EDGE ? (g.ws && t == 1) : false;          // row t-2 is the virtual row -1
+        const double rm0 = EDGE ? tab[8 + WK_T_RM] : 0.0;
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const double vaS = wS1 ? -S.va[pn][i] : S.va[po][i];
+            const double PS = wS1 ? rm0 * P1[i] : S.P[po][i];
+            S.Au[pn][i] = mm_Au(UB1[i], S.va[pn][i], WA_W(P1, i, PW), WA_E(P1, i, PE), dtt1, dtcz1);
+            S.e[pn][i] = 1.0 - dtcz1 * (WA_E(ua1, i, uaE) - WA_W(ua1, i, uaW)) + cmrm1 * vaS;
+            S.avp[pn][i] = vbC[i] + UB1[i] * (dtf1 + dtt1 * ua1[i]) + cmrp2 * PS;
         }
     } else {
-        const bool vr = g.wn && t == g.py + 1;      // virtual row py: v^a mirrored, P carries the metric ratio
         const double rpn = tab[g.py * 8 + WK_T_RP];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            ua1[i] = 0.0; va1[i] = vr ? -R.va2[i] : 0.0; UB1[i] = 0.0; HB1[i] = 0.0; P1[i] = vr ? rpn * R.P2[i] : 0.0;
-#pragma unroll
-            for (int f = 0; f < 3; ++f) dn1[f][i] = 0.0;
+            P1[i] = vrN ? rpn * S.P[po][i] : 0.0;   // virtual row py: P carries the metric ratio
+            S.HB[pn][i] = 0.0; S.Au[pn][i] = 0.0; S.e[pn][i] = 0.0; S.avp[pn][i] = 0.0;
         }
-        uaL1 = 0.0; uaR1 = 0.0;
     }
+    WKP(3)
 
-    // ---- (3) row t-2: A_h, A_u, A_v; (4) scatter into L0 of rows t-1, t-2, t-3
-    double Lc[3][K];
-    if (t >= 2 && t <= g.py + 1) {               // (rows -1 and py are virtual: nothing is scattered from them)
-        const double* tb = tab + t * 8 - 8;
-        const double dtcz2 = tb[WK_T_DTCZ], dtf2 = tb[WK_T_DTF], dtt2 = tb[WK_T_DTT], rp2 = tb[WK_T_RP], rm2 = tb[WK_T_RM];
-        const double rp3 = tb[WK_T_RP - 8], rm1 = tb[WK_T_RM + 8];
-        double PL = wk_up(R.P2[K - 1]), PR = wk_dn(R.P2[0]);
-        PL = C.lane0 ? 0.0 : PL; PR = C.laneL ? 0.0 : PR;
-        double Aa[3][K], mE[3][K], mW[3][K];
-        const bool wallS = g.ws && t == 2, wallN = g.wn && t == g.py + 1;
+    // ---- (3) row t-2: A_h, A_u, A_v completed; (4) scatter into L0 of rows t-1, t-2, t-3
+    double (&Ln)[3][K] = S.L[zn];
+    double (&La)[3][K] = S.L[zc];
+    double (&Lb)[3][K] = S.L[zs];
+    if (!EDGE || (t >= 2 && t <= g.py + 1)) {       // (rows -1 and py are virtual: nothing is scattered from them)
+        const double dtcz2 = t2[WK_T_DTCZ], cmrp2 = t2[WK_T_CMRP], cmrm1 = t1[WK_T_CMRM];
+        const bool wallS = EDGE ? (g.ws && t == 2) : false, wallN = EDGE ? (g.wn && t == g.py + 1) : false;
+        double Aa[3][K], cu[K], cv[K], su[K], sv[K];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            const double uE = i < K - 1 ? R.ua2[i + 1 < K ? i + 1 : i] : R.uaR2;
-            const double uW = i > 0 ? R.ua2[i > 0 ? i - 1 : 0] : R.uaL2;
-            const double PE = i < K - 1 ? R.P2[i + 1 < K ? i + 1 : i] : PR;
-            const double PW = i > 0 ? R.P2[i > 0 ? i - 1 : 0] : PL;
-            const double D = mm_div(uE, uW, va1[i], R.va3[i], dtcz2, C.dtcm, rp2, rm2);
-            Aa[0][i] = mm_Ah(R.HB2[i], D);
-            Aa[1][i] = mm_Au(R.UB2[i], R.va2[i], PW, PE, dtt2, dtcz2);
-            Aa[2][i] = mm_Av(R.vb2[i], R.UB2[i], R.ua2[i], rp3 * R.P3[i], rm1 * P1[i], dtf2, dtt2, C.dtcm);
-            const double cu = dtcz2 * R.z2[1][i], cv = C.dtcm * R.z2[2][i];
-            const double kE = C.kap - cu, kW = C.kap + cu, kS = C.kap + cv, kN = C.kap - cv;
-            double su = 0.0, sv = 0.0;
-#pragma unroll
-            for (int f = 0; f < 3; ++f) {
-                const double a = Aa[f][i];
-                const double xE = i < K - 1 ? R.z2[f][i + 1 < K ? i + 1 : i] : R.hz2[f][1];
-                const double xW = i > 0 ? R.z2[f][i > 0 ? i - 1 : 0] : R.hz2[f][0];
-                mE[f][i] = a * kE; mW[f][i] = a * kW;
-                su += (xE - xW) * a; sv += R.dn2[f][i] * a;
-                const double sgn = f == 2 ? -1.0 : 1.0;
-                const double mS = a * kS, mN = a * kN;
-                double la = R.La[f][i] + a * C.c0k;
-                if (wallS) la += sgn * mS; else R.Lb[f][i] += mS;
-                if (wallN) { la += sgn * mN; Lc[f][i] = 0.0; } else Lc[f][i] = mN;
-                R.La[f][i] = la;
-            }
-            R.La[1][i] -= dtcz2 * su; R.La[2][i] -= C.dtcm * sv;
+            Aa[0][i] = S.HB[po][i] * (S.e[po][i] - cmrp2 * S.va[pn][i]);
+            Aa[1][i] = S.Au[po][i];
+            Aa[2][i] = S.avp[po][i] - cmrm1 * P1[i];
+            cu[i] = dtcz2 * zS[1][i]; cv[i] = C.dtcm * zS[2][i];
+            su[i] = 0.0; sv[i] = 0.0;
         }
 #pragma unroll
         for (int f = 0; f < 3; ++f) {
-            const double fW = wk_up(mE[f][K - 1]), fE = wk_dn(mW[f][0]);
+            double mE[K], mW[K];
+            const double sgn = f == 2 ? -1.0 : 1.0;
 #pragma unroll
-            for (int i = 0; i < K; ++i)
-                R.La[f][i] += (i > 0 ? mE[f][i > 0 ? i - 1 : 0] : fW) + (i < K - 1 ? mW[f][i + 1 < K ? i + 1 : i] : fE);
+            for (int i = 0; i < K; ++i) {
+                const double a = Aa[f][i];
+                const double xE = WA_E(zS[f], i, S.hz[po][f][1]);
+                const double xW = WA_W(zS[f], i, S.hz[po][f][0]);
+                mE[i] = a * (C.kap - cu[i]); mW[i] = a * (C.kap + cu[i]);
+                su[i] += (xE - xW) * a; sv[i] += S.dn[po][f][i] * a;
+                const double mS = a * (C.kap + cv[i]), mN = a * (C.kap - cv[i]);
+                double la = La[f][i] + a * C.c0k;
+                if (wallS) la += sgn * mS; else Lb[f][i] += mS;
+                if (wallN) { la += sgn * mN; Ln[f][i] = 0.0; } else Ln[f][i] = mN;
+                La[f][i] = la;
+            }
+            const double fW = wk_up(mE[K - 1]), fE = wk_dn(mW[0]);
+#pragma unroll
+            for (int i = 0; i < K; ++i) La[f][i] += WA_W(mE, i, fW) + WA_E(mW, i, fE);
         }
+#pragma unroll
+        for (int i = 0; i < K; ++i) { La[1][i] -= dtcz2 * su[i]; La[2][i] -= C.dtcm * sv[i]; }
     } else {
 #pragma unroll
         for (int f = 0; f < 3; ++f)
 #pragma unroll
-            for (int i = 0; i < K; ++i) Lc[f][i] = 0.0;
+            for (int i = 0; i < K; ++i) Ln[f][i] = 0.0;
     }
+#pragma unroll
+    for (int i = 0; i < K; ++i) S.P[pn][i] = P1[i];
+    WKP(6)
 
     // ---- (5) row t-3 of lambda^{n-1} is complete; u^{n-1} of row t-2 replaces u^n
     {
-        const int l3 = lj - 3, l2 = lj - 2;
-        if ((unsigned)l3 < (unsigned)g.ey) {
-            const int o3 = C.lam + l3 * g.ex + ci0;
-#pragma unroll
-            for (int i = 0; i < K; ++i)
-                if ((C.tmask >> i) & 1u) { sm[o3 + i] = R.Lb[0][i]; sm[o3 + C.FS + i] = R.Lb[1][i]; sm[o3 + 2 * C.FS + i] = R.Lb[2][i]; }
+        const bool st3 = EDGE ? (unsigned)(lj - 3) < (unsigned)g.ey : true;
+        const bool st2 = EDGE ? (unsigned)(lj - 2) < (unsigned)g.ey : true;
+        const uint32_t o0 = lrow - 3u * PL8, o1 = o0 + C.FS8, o2 = o1 + C.FS8, o3 = lrow - 2u * PL8 + 3u * C.FS8;
+        if (st3) {
+            if (C.tmask & 1u) { wk_sts<0>(o0, Lb[0][0]); wk_sts<0>(o1, Lb[1][0]); wk_sts<0>(o2, Lb[2][0]); }
+            if (K > 1 && (C.tmask & 2u)) { wk_sts<8>(o0, Lb[0][K > 1 ? 1 : 0]); wk_sts<8>(o1, Lb[1][K > 1 ? 1 : 0]); wk_sts<8>(o2, Lb[2][K > 1 ? 1 : 0]); }
+            if (K > 2 && (C.tmask & 4u)) { wk_sts<16>(o0, Lb[0][K > 2 ? 2 : 0]); wk_sts<16>(o1, Lb[1][K > 2 ? 2 : 0]); wk_sts<16>(o2, Lb[2][K > 2 ? 2 : 0]); }
         }
-        if ((unsigned)l2 < (unsigned)g.ey) {
-            const int o2 = C.u1 + l2 * g.ex + ci0;
-#pragma unroll
-            for (int i = 0; i < K; ++i)
-                if ((C.tmask >> i) & 1u) sm[o2 + i] = R.z2[1][i];
+        if (st2) {
+            if (C.tmask & 1u) wk_sts<0>(o3, zS[1][0]);
+            if (K > 1 && (C.tmask & 2u)) wk_sts<8>(o3, zS[1][K > 1 ? 1 : 0]);
+            if (K > 2 && (C.tmask & 4u)) wk_sts<16>(o3, zS[1][K > 2 ? 2 : 0]);
         }
     }
     // the next row of Z^{n-1} must have landed; its ghost cells go in place
-    if (t + 1 < g.py) wa_prep_row<K>(C, sm, t + 1);
+    if (EDGE) { if (t + 1 < g.py) wa_prep_row<K>(C, sm, t + 1); }
+    else wa_prep_tile_row<K>(C, lj + 1, (t + 1) % 3);
     __syncwarp();
+    WKP(1)
     // ---- (6) one lane: progress word, the row after next, next E/W chunk
     if (wk_elect()) {
-        if (t < C.T) wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
-        if (t + 2 < g.py) wa_issue_row<K>(C, t + 2, false);
+        if (!EDGE || t < C.T) wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
+        if (EDGE) { if (t + 2 < g.py) wa_issue_row<K>(C, t + 2, false); }
+        else wa_issue_tile_row<K>(C, lj + 2, (t + 2) % 3);
         const int l1 = lj + 1;
-        if ((unsigned)l1 < (unsigned)g.ey && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk)
+        if ((!EDGE || (unsigned)l1 < (unsigned)g.ey) && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk)
             wa_issue_chunk<K>(C, l1 / WK_EWC + 2);
     }
-    // ---- (7) rotate
+    WKP(4)
+}
+
+// after a tick run at slot 0: move every history back to the canonical registers
+template <int K>
+__device__ __forceinline__ void wa_rotate(WaState<K>& S)
+{
 #pragma unroll
     for (int i = 0; i < K; ++i) {
 #pragma unroll
         for (int f = 0; f < 3; ++f) {
-            R.z2[f][i] = R.z1[f][i]; R.z1[f][i] = z0[f][i]; R.dn2[f][i] = dn1[f][i];
-            R.Lb[f][i] = R.La[f][i]; R.La[f][i] = Lc[f][i];
+            S.z[1][f][i] = S.z[2][f][i]; S.z[2][f][i] = S.z[0][f][i];
+            S.L[1][f][i] = S.L[2][f][i]; S.L[2][f][i] = S.L[0][f][i];
+            S.dn[1][f][i] = S.dn[0][f][i];
         }
-        R.ua2[i] = ua1[i]; R.va3[i] = R.va2[i]; R.va2[i] = va1[i];
-        R.vb2[i] = R.vb1[i]; R.vb1[i] = vb0[i];
-        R.UB2[i] = UB1[i]; R.HB2[i] = HB1[i]; R.P3[i] = R.P2[i]; R.P2[i] = P1[i];
+        S.va[1][i] = S.va[0][i]; S.P[1][i] = S.P[0][i]; S.e[1][i] = S.e[0][i];
+        S.HB[1][i] = S.HB[0][i]; S.Au[1][i] = S.Au[0][i]; S.avp[1][i] = S.avp[0][i];
     }
 #pragma unroll
-    for (int f = 0; f < 3; ++f) { R.hz2[f][0] = hz1[f][0]; R.hz2[f][1] = hz1[f][1]; }
-    R.uaL2 = uaL1; R.uaR2 = uaR1;
-    if (t < g.py) { R.pa = ra; R.pe = re; R.pe2 = re2; }
+    for (int f = 0; f < 3; ++f) { S.hz[1][f][0] = S.hz[0][f][0]; S.hz[1][f][1] = S.hz[0][f][1]; }
 }
 
 template <int K>
@@ -320,6 +413,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
     int* s_next = reinterpret_cast<int*>(sm + 52);
     double* tab = sm + Ly.tab;
     const int IW = Ly.wbase + w * Ly.wsz;
+    constexpr int PL = 32 * K;
     if (tid == 0) {
         for (int i = 0; i < 41; ++i) wk_mbar_init32(sm32 + 8u * i, 1);
         wk_fence_mbar_init();
@@ -331,14 +425,20 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
     const int lw = (w + WK_NW - 1) % WK_NW;
 
     WaCtx<K> C;
-    C.lam = Ly.st; C.u1 = Ly.u1; C.ZP = Ly.ZP;
+    C.lam = Ly.st; C.u1 = Ly.u1; C.ZP = Ly.ZP; C.FS = Ly.FS; C.maxey = A.maxey;
     C.I_ZR = IW + Ly.zr; C.I_EW = IW + Ly.ew; C.I_EDS = IW + Ly.eds; C.I_EDE = IW + Ly.ede;
     C.sm32 = sm32; C.a_lead = sm32 + 8u * 48u + 4u * lw; C.a_mine = sm32 + 8u * 48u + 4u * w;
     C.b_z = sm32 + 8u * (w * 5); C.b_ew = sm32 + 8u * (w * 5 + 3);
     C.c0 = 2 + K * lane; C.lane = lane; C.lane0 = lane == 0; C.laneL = lane == 31;
+    C.zu = sm32 + 8u * C.I_ZR; C.zl = C.zu + 8u * C.c0; C.SL8 = 8u * 3 * Ly.ZP; C.ZP8 = 8u * Ly.ZP; C.FS8 = 8u * Ly.FS;
+    C.la0 = sm32 + 8u * (Ly.st + K * lane);
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm; C.c0k = 1.0 - 4.0 * A.m.kap; C.mu2 = 2.0 * A.cp.mu;
     C.A = &A; C.par = 0u;
-    const int lam = Ly.st;
+    const int lam = Ly.st, FS = Ly.FS;
+#ifdef WK_PROF
+    for (int q = 0; q < 8; ++q) C.pf[q] = 0;
+    long long ph[4] = {0, 0, 0, 0}, pht = clock64();
+#endif
 
     for (;;) {
         if (tid == 0) *s_next = atomicAdd(A.counter, 1);
@@ -350,26 +450,30 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
         const Sub s = A.subs[k];
         const WkGeo g = wk_geo(s);
         C.g = g;
-        const int FS = g.ncell;                 // lambda and u^n are stored with the tile's own pitch
-        C.FS = FS;
         const long long n3 = 3LL * g.ncell;
+        WKPH(3)
 
         // ---------------- init: lambda^W = successor-window overlap forcing (25c), else zero; u^W
+        // (cells 0 and > ex of every row and the row maxey are zero and stay zero)
         wk_load_tab(tab, A.m, g);
         {
             const bool succ = s.jw < A.geo.q - 1;
             const double* tw = A.traj + s.toff + (long long)g.W * n3;
             const double* xn = succ ? A.xfrozen + A.subs[k + A.geo.p1 * A.geo.p2].coff : nullptr;
-            for (int c = tid; c < g.ncell; c += WK_NT) {
+            for (int q = tid; q < g.ey * PL; q += WK_NT) {
+                const int lj = q / PL, qi = q - lj * PL;
+                const bool in = qi >= 1 && qi <= g.ex;
+                const int c = lj * g.ex + qi - 1;
 #pragma unroll
                 for (int f = 0; f < 3; ++f) {
-                    const double zv = __ldg(tw + (long long)f * g.ncell + c);
-                    sm[lam + f * FS + c] = succ ? C.mu2 * (zv - __ldg(xn + (long long)f * g.ncell + c)) * A.cp.ib[f] : 0.0;
-                    if (f == 1) sm[C.u1 + c] = zv;
+                    const double zv = in ? __ldg(tw + (long long)f * g.ncell + c) : 0.0;
+                    sm[lam + f * FS + q] = (in && succ) ? C.mu2 * (zv - __ldg(xn + (long long)f * g.ncell + c)) * A.cp.ib[f] : 0.0;
+                    if (f == 1) sm[C.u1 + q] = zv;
                 }
             }
         }
         __syncthreads();
+        WKPH(0)
 
         // ---------------- per-lane column map of this tile
         C.tmask = 0u;
@@ -386,6 +490,9 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
         }
         C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
         C.T = g.py + 3;
+        // steady ticks: rows t-3 .. t+2 are tile rows, no wall event; groups of six starting at a multiple of three
+        const int ts0 = g.gys + 3 > 3 ? g.gys + 3 : 3;
+        const int ts1 = g.gys + g.ey - 2;       // a steady tick needs t < ts1
 
         // ---------------- the steps of this warp
         for (int m = w; m < g.W; m += WK_NW) {
@@ -406,23 +513,46 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 wa_issue_chunk<K>(C, 0);
                 if (C.nchunk > 1) wa_issue_chunk<K>(C, 1);
             }
-            WaRegs<K> R;
+            WaState<K> S;
 #pragma unroll
             for (int i = 0; i < K; ++i) {
 #pragma unroll
-                for (int f = 0; f < 3; ++f) { R.z1[f][i] = R.z2[f][i] = R.dn2[f][i] = R.La[f][i] = R.Lb[f][i] = 0.0; }
-                R.ua2[i] = R.va2[i] = R.va3[i] = R.vb1[i] = R.vb2[i] = R.UB2[i] = R.HB2[i] = R.P2[i] = R.P3[i] = 0.0;
+                for (int sl = 0; sl < 3; ++sl) {
+#pragma unroll
+                    for (int f = 0; f < 3; ++f) { S.z[sl][f][i] = 0.0; S.L[sl][f][i] = 0.0; }
+                }
+#pragma unroll
+                for (int sl = 0; sl < 2; ++sl) {
+#pragma unroll
+                    for (int f = 0; f < 3; ++f) S.dn[sl][f][i] = 0.0;
+                    S.va[sl][i] = S.P[sl][i] = S.e[sl][i] = S.HB[sl][i] = S.Au[sl][i] = S.avp[sl][i] = 0.0;
+                }
             }
 #pragma unroll
-            for (int f = 0; f < 3; ++f) { R.hz2[f][0] = 0.0; R.hz2[f][1] = 0.0; }
-            R.uaL2 = R.uaR2 = 0.0; R.pa = C.I_ZR + 1; R.pe = C.I_EDS; R.pe2 = C.I_EDS;
+            for (int sl = 0; sl < 2; ++sl)
+#pragma unroll
+                for (int f = 0; f < 3; ++f) { S.hz[sl][f][0] = 0.0; S.hz[sl][f][1] = 0.0; }
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
+#ifdef WK_PROF
+            C.pt = clock64();
+#endif
 #pragma unroll 1
-            for (int t = 0; t < C.T; ++t) wa_tick<K>(t, R, C, sm, tab);
+            for (int t = 0; t < C.T;) {
+                if (t >= ts0 && t < ts1) {
+                    wa_tick<K, 0, 0, false>(t, S, C, sm, tab);
+                    wa_rotate<K>(S);
+                    ++t;
+                } else {
+                    wa_tick<K, 0, 0, true>(t, S, C, sm, tab);
+                    wa_rotate<K>(S);
+                    ++t;
+                }
+            }
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);
             __syncwarp();
         }
+        WKPH(1)
         __syncthreads();
 
         // ---------------- gradient at the window start: lambda^0 + H^T R^-1 at level 0 (25b)
@@ -431,7 +561,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             const long long a0 = A.obs_start[s.ooff], a1 = A.obs_start[s.ooff + 1];
             for (long long q = a0 + tid; q < a1; q += WK_NT) {
                 const int pk = A.obs_lj[q];
-                sm[lam + ((pk >> 8) & 3) * FS + (pk >> 12) * g.ex + (pk & 255)] += A.obs_r[q];
+                sm[lam + ((pk >> 8) & 3) * FS + (pk >> 12) * PL + 1 + (pk & 255)] += A.obs_r[q];
             }
             __syncthreads();
         }
@@ -442,14 +572,14 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 for (int li = lane; li < g.ex; li += 32) {
                     int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
                     const double wsp2 = 2.0 * (s.jw == 0 ? 1.0 : A.cp.bgw) / (double)(A.geo.ncolcov[gi] * nr);
-                    const int c = lj * g.ex + li;
+                    const int c = lj * g.ex + li, q = lj * PL + 1 + li;
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {
                         const long long o = s.coff + (long long)f * g.ncell + c;
                         const double xv = __ldg(A.x + o);
-                        double gg = sm[lam + f * FS + c] + wsp2 * (xv - __ldg(A.xbs + o)) * A.cp.ib[f];
+                        double gg = sm[lam + f * FS + q] + wsp2 * (xv - __ldg(A.xbs + o)) * A.cp.ib[f];
                         if (pred) gg += C.mu2 * (xv - __ldg(A.pred_end + o)) * A.cp.ib[f];
-                        sm[lam + f * FS + c] = gg;
+                        sm[lam + f * FS + q] = gg;
                     }
                 }
             }
@@ -459,25 +589,36 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 const double* xf = A.xfrozen + nb.coff2 + (long long)nb.nj0 * nb.ex2 + nb.ni0;
                 for (int dj = w; dj < nb.h; dj += WK_NW)
                     for (int di = lane; di < nb.w; di += 32) {
-                        const int c = (nb.j0 + dj) * g.ex + nb.i0 + di;
+                        const int c = (nb.j0 + dj) * g.ex + nb.i0 + di, q = (nb.j0 + dj) * PL + 1 + nb.i0 + di;
 #pragma unroll
                         for (int f = 0; f < 3; ++f) {
                             const double xv = __ldg(A.x + s.coff + (long long)f * g.ncell + c);
-                            sm[lam + f * FS + c] += C.mu2 * (xv - __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di)) * A.cp.ib[f];
+                            sm[lam + f * FS + q] += C.mu2 * (xv - __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di)) * A.cp.ib[f];
                         }
                     }
             }
             __syncthreads();
-            for (int c = tid; c < g.ncell; c += WK_NT) {
+            for (int lj = w; lj < g.ey; lj += WK_NW)
+                for (int li = lane; li < g.ex; li += 32) {
+                    const int c = lj * g.ex + li, q = lj * PL + 1 + li;
 #pragma unroll
-                for (int f = 0; f < 3; ++f) {
-                    const long long o = s.coff + (long long)f * g.ncell + c;
-                    const double gg = sm[lam + f * FS + c];
-                    A.gx[o] = gg;
-                    if (A.gw) A.gw[o] = A.cp.sb[f] * gg;
+                    for (int f = 0; f < 3; ++f) {
+                        const long long o = s.coff + (long long)f * g.ncell + c;
+                        const double gg = sm[lam + f * FS + q];
+                        A.gx[o] = gg;
+                        if (A.gw) A.gw[o] = A.cp.sb[f] * gg;
+                    }
                 }
-            }
         }
+        __syncthreads();                        // the next subdomain's init overwrites lambda
         gbase += (unsigned)g.W + 1u;
+        WKPH(2)
     }
+#ifdef WK_PROF
+    if (lane == 0 && A.J) {
+        unsigned long long* pr = reinterpret_cast<unsigned long long*>(A.J);
+        for (int q = 0; q < 8; ++q) atomicAdd(pr + w * 16 + q, (unsigned long long)C.pf[q]);
+        for (int q = 0; q < 4; ++q) atomicAdd(pr + w * 16 + 8 + q, (unsigned long long)ph[q]);
+    }
+#endif
 }

@@ -48,8 +48,9 @@ struct WkArgs {
 // forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
 //   [tile ex][E ghosts 3][pad 2][W ghosts of the NEXT row 3], so that padded column c of tile row
 //   lj is at  st + f*FS + lj*P + (c - 3)  for every c (W ghosts sit in the previous row's tail).
-// adjoint resident state: lambda [3][maxey*maxex] and u1 [maxey*maxex], tile only (lambda is zero
-//   outside the extended tile).
+// adjoint resident state: lambda [3][maxey+1][32 K] and u1 [maxey+1][32 K]: lambda is zero outside
+//   the extended tile, so only the columns the lanes own are kept; the cells of ghost columns and
+//   the extra row stay zero and serve every read that falls outside the tile.
 struct WkLayout {
     int tab, st, P, FS, u1, wbase, wsz, sn, zr, ZP, ew, eds, ede, total;
 };
@@ -63,9 +64,11 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
         L.st = o + 8; o += 8 + 3 * L.FS + 64;       // 64 doubles of slack: lanes beyond px read past a row
         L.u1 = 0;
     } else {
-        L.P = maxex; L.FS = maxey * maxex;
-        L.st = o; o += 3 * L.FS; o = (o + 1) & ~1;
-        L.u1 = o; o += L.FS; o = (o + 1) & ~1;
+        // row pitch = 32 K cells (one cell per lane and owned column: cell q <-> padded column q + 2, so
+        // q = 0 and q > ex are permanently zero), plus one all-zero row (index maxey) per field
+        L.P = maxpx - 4 <= 64 ? 64 : 96; L.FS = (maxey + 1) * L.P;
+        L.st = o; o += 3 * L.FS;
+        L.u1 = o; o += L.FS;
     }
     L.wbase = o;
     int p = 0;
@@ -189,7 +192,7 @@ __device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const 
         t[0] = m.dtcz[cj]; t[1] = m.gdtcz[cj]; t[2] = m.dtf[cj]; t[3] = m.dtt[cj];
         t[4] = gj < 0 ? 1.0 : m.rp[cj];
         t[5] = gj >= m.nlat ? 1.0 : m.rm[cj];
-        t[6] = 0.0; t[7] = 0.0;
+        t[6] = m.dtcm * t[4]; t[7] = m.dtcm * t[5];
     }
 }
 #define WK_T_DTCZ 0
@@ -198,6 +201,8 @@ __device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const 
 #define WK_T_DTT 3
 #define WK_T_RP 4
 #define WK_T_RM 5
+#define WK_T_CMRP 6             // dtcm * r+
+#define WK_T_CMRM 7             // dtcm * r-
 
 // one elected lane of the (converged) warp; tells the compiler the region is single-threaded
 __device__ __forceinline__ bool wk_elect()
