@@ -401,6 +401,8 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
     a.obs_y = L.obs_y; a.obs_c = L.obs_c; a.obs_r = L.obs_r;
     a.parts = L.parts; a.J = Jout; a.gx = L.gx; a.gw = gw;
     a.maxex = L.wp.maxex; a.maxey = L.wp.maxey; a.maxpx = L.wp.maxpx; a.maxpy = L.wp.maxpy;
+    a.Lf = wk_layout(false, a.maxex, a.maxey, a.maxpx, a.maxpy);
+    a.La = wk_layout(true, a.maxex, a.maxey, a.maxpx, a.maxpy);
     return a;
 }
 

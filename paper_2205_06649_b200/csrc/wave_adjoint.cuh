@@ -32,12 +32,13 @@
 #pragma once
 #include "wave_common.cuh"
 
-template <int K> struct WaState {
-    double z[3][3][K];              // [slot][field][column]: Z^{n-1} rows t, t-1, t-2 (period 3)
-    double L[3][3][K];              // unfinished L0 of rows t-1 (started this tick), t-2, t-3 (period 3)
-    double hz[2][3][2];             // E/W halo of rows t-1, t-2 (period 2)
+template <int K> struct WaState {     // every history has depth one: slot [t & 1] is written at tick t and read at tick t + 1
+    double zc[2][3][K];             // [slot][field][column]: Z^{n-1} row t-1 (own columns), kept for one tick as row t-2
+    double hz[2][3][2];             // E/W halo of rows t-1, t-2
     double dn[2][3][K];             // x_N - x_S on rows t-1, t-2
     double va[2][K], P[2][K], e[2][K], HB[2][K], Au[2][K], avp[2][K];   // rows t-1, t-2
+    double mN[2][3][K];             // northward part of the scatter from row t-2: starts L0 of row t-1
+    double La[2][3][K];             // L0 of row t-2 without the southward part of row t-1
 };
 template <int K> struct WaCtx {
     WkGeo g;
@@ -138,25 +139,34 @@ __device__ __forceinline__ void wa_prep_tile_row(WaCtx<K>& C, int l, const int S
 
 // One tick.  P3 / P2: register slots of this tick (t mod 3, t mod 2 counted from the canonical state);
 // EDGE = false: rows t-3 .. t+2 are tile rows, no wall event.
-template <int K, int P3, int P2, bool EDGE>
+template <int K, int P2, bool EDGE>
 __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C, double* __restrict__ sm,
                                         const double* __restrict__ tab)
 {
-    constexpr int zn = P3, zc = (P3 + 2) % 3, zs = (P3 + 1) % 3, pn = P2, po = 1 - P2;
+    constexpr int pn = P2, po = 1 - P2;
     constexpr uint32_t PL8 = 8u * 32u * K;          // lambda row pitch in bytes
     const WkGeo& g = C.g;
     const int lj = t - g.gys;
     const bool tile = EDGE ? (unsigned)lj < (unsigned)g.ey : true;
     const bool tile1 = EDGE ? (unsigned)(lj - 1) < (unsigned)g.ey : true;
-    double (&zN)[3][K] = S.z[zn];
-    double (&zC)[3][K] = S.z[zc];
-    double (&zS)[3][K] = S.z[zs];
+    double zN[3][K];                                // row t (re-read as row t-1 by the next tick: the ring still holds it)
+    double (&zC)[3][K] = S.zc[pn];
+    double (&zS)[3][K] = S.zc[po];
     WKP(7)
 
     // ---- (1) Z^{n-1}: own columns of row t, E/W halo and edge u^a of row t-1
     double eL, eR;
     {
         const int s0 = t % 3, s1 = s0 == 0 ? 2 : s0 - 1;             // ring slots of rows t, t-1
+        const uint32_t h0 = C.zl + s1 * C.SL8 + (tile1 ? 8u : 0u), h1 = h0 + C.ZP8, h2 = h1 + C.ZP8;
+        if (!EDGE || t <= g.py) {                   // row t-1 is a padded row (at t = 0: stale but finite data)
+            zC[0][0] = wk_lds<0>(h0); zC[1][0] = wk_lds<0>(h1); zC[2][0] = wk_lds<0>(h2);
+            if (K > 1) { zC[0][K > 1 ? 1 : 0] = wk_lds<8>(h0); zC[1][K > 1 ? 1 : 0] = wk_lds<8>(h1); zC[2][K > 1 ? 1 : 0] = wk_lds<8>(h2); }
+            if (K > 2) { zC[0][K > 2 ? 2 : 0] = wk_lds<16>(h0); zC[1][K > 2 ? 2 : 0] = wk_lds<16>(h1); zC[2][K > 2 ? 2 : 0] = wk_lds<16>(h2); }
+        } else {
+#pragma unroll
+            for (int i = 0; i < K; ++i) { zC[0][i] = zS[0][i]; zC[1][i] = zS[1][i]; zC[2][i] = zS[2][i]; }
+        }
         if (!EDGE || t < g.py) {
             const uint32_t a0 = C.zl + s0 * C.SL8 + (tile ? 8u : 0u), a1 = a0 + C.ZP8, a2 = a1 + C.ZP8;
             zN[0][0] = wk_lds<0>(a0); zN[1][0] = wk_lds<0>(a1); zN[2][0] = wk_lds<0>(a2);
@@ -167,7 +177,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 #pragma unroll
             for (int i = 0; i < K; ++i) { zN[0][i] = zC[0][i]; zN[1][i] = zC[1][i]; zN[2][i] = sg * zC[2][i]; }
         }
-        const uint32_t h0 = C.zl + s1 * C.SL8 + (tile1 ? 8u : 0u), h1 = h0 + C.ZP8, h2 = h1 + C.ZP8;
         S.hz[pn][0][0] = wk_lds<-8>(h0); S.hz[pn][1][0] = wk_lds<-8>(h1); S.hz[pn][2][0] = wk_lds<-8>(h2);
         S.hz[pn][0][1] = wk_lds<8 * K>(h0); S.hz[pn][1][1] = wk_lds<8 * K>(h1); S.hz[pn][2][1] = wk_lds<8 * K>(h2);
         uint32_t ea, eb;
@@ -303,9 +312,9 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     WKP(3)
 
     // ---- (3) row t-2: A_h, A_u, A_v completed; (4) scatter into L0 of rows t-1, t-2, t-3
-    double (&Ln)[3][K] = S.L[zn];
-    double (&La)[3][K] = S.L[zc];
-    double (&Lb)[3][K] = S.L[zs];
+    double (&Ln)[3][K] = S.mN[pn];                  // L0 of row t-1: northward part of the scatter from row t-2
+    double (&La)[3][K] = S.La[pn];                  // L0 of row t-2 (its southward part arrives at the next tick)
+    double Lb[3][K];                                // L0 of row t-3: complete
     if (!EDGE || (t >= 2 && t <= g.py + 1)) {       // (rows -1 and py are virtual: nothing is scattered from them)
         const double dtcz2 = t2[WK_T_DTCZ], cmrp2 = t2[WK_T_CMRP], cmrm1 = t1[WK_T_CMRM];
         const bool wallS = EDGE ? (g.ws && t == 2) : false, wallN = EDGE ? (g.wn && t == g.py + 1) : false;
@@ -330,8 +339,8 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
                 mE[i] = a * (C.kap - cu[i]); mW[i] = a * (C.kap + cu[i]);
                 su[i] += (xE - xW) * a; sv[i] += S.dn[po][f][i] * a;
                 const double mS = a * (C.kap + cv[i]), mN = a * (C.kap - cv[i]);
-                double la = La[f][i] + a * C.c0k;
-                if (wallS) la += sgn * mS; else Lb[f][i] += mS;
+                double la = S.mN[po][f][i] + a * C.c0k;
+                if (wallS) { la += sgn * mS; Lb[f][i] = S.La[po][f][i]; } else Lb[f][i] = S.La[po][f][i] + mS;
                 if (wallN) { la += sgn * mN; Ln[f][i] = 0.0; } else Ln[f][i] = mN;
                 La[f][i] = la;
             }
@@ -345,7 +354,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 #pragma unroll
         for (int f = 0; f < 3; ++f)
 #pragma unroll
-            for (int i = 0; i < K; ++i) Ln[f][i] = 0.0;
+            for (int i = 0; i < K; ++i) { Ln[f][i] = 0.0; La[f][i] = S.mN[po][f][i]; Lb[f][i] = S.La[po][f][i]; }
     }
 #pragma unroll
     for (int i = 0; i < K; ++i) S.P[pn][i] = P1[i];
@@ -384,7 +393,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     WKP(4)
 }
 
-// after a tick run at slot 0: move every history back to the canonical registers
+// after a single tick run at slot 0: move every history to slot 1, where the next tick at slot 0 reads it
 template <int K>
 __device__ __forceinline__ void wa_rotate(WaState<K>& S)
 {
@@ -392,9 +401,8 @@ __device__ __forceinline__ void wa_rotate(WaState<K>& S)
     for (int i = 0; i < K; ++i) {
 #pragma unroll
         for (int f = 0; f < 3; ++f) {
-            S.z[1][f][i] = S.z[2][f][i]; S.z[2][f][i] = S.z[0][f][i];
-            S.L[1][f][i] = S.L[2][f][i]; S.L[2][f][i] = S.L[0][f][i];
-            S.dn[1][f][i] = S.dn[0][f][i];
+            S.zc[1][f][i] = S.zc[0][f][i]; S.dn[1][f][i] = S.dn[0][f][i];
+            S.mN[1][f][i] = S.mN[0][f][i]; S.La[1][f][i] = S.La[0][f][i];
         }
         S.va[1][i] = S.va[0][i]; S.P[1][i] = S.P[0][i]; S.e[1][i] = S.e[0][i];
         S.HB[1][i] = S.HB[0][i]; S.Au[1][i] = S.Au[0][i]; S.avp[1][i] = S.avp[0][i];
@@ -408,7 +416,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
 {
     extern __shared__ __align__(128) double sm[];
     const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(tid >> 5);
-    const WkLayout Ly = wk_layout(true, A.maxex, A.maxey, A.maxpx, A.maxpy);
+    const WkLayout& Ly = A.La;
     const uint32_t sm32 = wk_s32(sm);
     int* s_next = reinterpret_cast<int*>(sm + 52);
     double* tab = sm + Ly.tab;
@@ -460,15 +468,30 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             const bool succ = s.jw < A.geo.q - 1;
             const double* tw = A.traj + s.toff + (long long)g.W * n3;
             const double* xn = succ ? A.xfrozen + A.subs[k + A.geo.p1 * A.geo.p2].coff : nullptr;
-            for (int q = tid; q < g.ey * PL; q += WK_NT) {
-                const int lj = q / PL, qi = q - lj * PL;
-                const bool in = qi >= 1 && qi <= g.ex;
-                const int c = lj * g.ex + qi - 1;
+            // (four cells per thread and pass: all loads are issued before the first use)
+            const int nq = g.ey * PL;
+            for (int q0 = tid; q0 < nq; q0 += 4 * WK_NT) {
+                double zv[4][3], xv[4][3];
 #pragma unroll
-                for (int f = 0; f < 3; ++f) {
-                    const double zv = in ? __ldg(tw + (long long)f * g.ncell + c) : 0.0;
-                    sm[lam + f * FS + q] = (in && succ) ? C.mu2 * (zv - __ldg(xn + (long long)f * g.ncell + c)) * A.cp.ib[f] : 0.0;
-                    if (f == 1) sm[C.u1 + q] = zv;
+                for (int u = 0; u < 4; ++u) {
+                    const int q = q0 + u * WK_NT;
+                    const int lj = q / PL, qi = q - lj * PL;
+                    const bool in = q < nq && qi >= 1 && qi <= g.ex;
+                    const int c = lj * g.ex + qi - 1;
+#pragma unroll
+                    for (int f = 0; f < 3; ++f) {
+                        zv[u][f] = in ? __ldg(tw + (long long)f * g.ncell + c) : 0.0;
+                        xv[u][f] = (in && succ) ? __ldg(xn + (long long)f * g.ncell + c) : zv[u][f];
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int q = q0 + u * WK_NT;
+                    if (q < nq) {
+#pragma unroll
+                        for (int f = 0; f < 3; ++f) sm[lam + f * FS + q] = C.mu2 * (zv[u][f] - xv[u][f]) * A.cp.ib[f];
+                        sm[C.u1 + q] = zv[u][1];
+                    }
                 }
             }
         }
@@ -515,23 +538,16 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             }
             WaState<K> S;
 #pragma unroll
-            for (int i = 0; i < K; ++i) {
+            for (int sl = 0; sl < 2; ++sl) {
 #pragma unroll
-                for (int sl = 0; sl < 3; ++sl) {
+                for (int i = 0; i < K; ++i) {
 #pragma unroll
-                    for (int f = 0; f < 3; ++f) { S.z[sl][f][i] = 0.0; S.L[sl][f][i] = 0.0; }
-                }
-#pragma unroll
-                for (int sl = 0; sl < 2; ++sl) {
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) S.dn[sl][f][i] = 0.0;
+                    for (int f = 0; f < 3; ++f) { S.zc[sl][f][i] = 0.0; S.dn[sl][f][i] = 0.0; S.mN[sl][f][i] = 0.0; S.La[sl][f][i] = 0.0; }
                     S.va[sl][i] = S.P[sl][i] = S.e[sl][i] = S.HB[sl][i] = S.Au[sl][i] = S.avp[sl][i] = 0.0;
                 }
-            }
-#pragma unroll
-            for (int sl = 0; sl < 2; ++sl)
 #pragma unroll
                 for (int f = 0; f < 3; ++f) { S.hz[sl][f][0] = 0.0; S.hz[sl][f][1] = 0.0; }
+            }
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
 #ifdef WK_PROF
@@ -539,12 +555,12 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
 #endif
 #pragma unroll 1
             for (int t = 0; t < C.T;) {
-                if (t >= ts0 && t < ts1) {
-                    wa_tick<K, 0, 0, false>(t, S, C, sm, tab);
-                    wa_rotate<K>(S);
-                    ++t;
+                if (t >= ts0 && t + 2 <= ts1) {
+                    wa_tick<K, 0, false>(t, S, C, sm, tab);
+                    wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
+                    t += 2;
                 } else {
-                    wa_tick<K, 0, 0, true>(t, S, C, sm, tab);
+                    wa_tick<K, 0, true>(t, S, C, sm, tab);
                     wa_rotate<K>(S);
                     ++t;
                 }
@@ -566,49 +582,72 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             __syncthreads();
         }
         {
-            const bool pred = s.jw > 0;
-            for (int lj = w; lj < g.ey; lj += WK_NW) {
-                const int nr = A.geo.nrowcov[s.ej0 + lj];
-                for (int li = lane; li < g.ex; li += 32) {
-                    int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
-                    const double wsp2 = 2.0 * (s.jw == 0 ? 1.0 : A.cp.bgw) / (double)(A.geo.ncolcov[gi] * nr);
-                    const int c = lj * g.ex + li, q = lj * PL + 1 + li;
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) {
-                        const long long o = s.coff + (long long)f * g.ncell + c;
-                        const double xv = __ldg(A.x + o);
-                        double gg = sm[lam + f * FS + q] + wsp2 * (xv - __ldg(A.xbs + o)) * A.cp.ib[f];
-                        if (pred) gg += C.mu2 * (xv - __ldg(A.pred_end + o)) * A.cp.ib[f];
-                        sm[lam + f * FS + q] = gg;
-                    }
-                }
-            }
             for (int r = 0; r < s.nnb; ++r) {   // (25c) case 1, one rectangle at a time (a cell may lie in several)
-                __syncthreads();
                 const NbRect nb = A.nbr[s.nb0 + r];
                 const double* xf = A.xfrozen + nb.coff2 + (long long)nb.nj0 * nb.ex2 + nb.ni0;
-                for (int dj = w; dj < nb.h; dj += WK_NW)
-                    for (int di = lane; di < nb.w; di += 32) {
-                        const int c = (nb.j0 + dj) * g.ex + nb.i0 + di, q = (nb.j0 + dj) * PL + 1 + nb.i0 + di;
+                const int ncr = nb.w * nb.h;
+                for (int e0 = tid; e0 < ncr; e0 += 2 * WK_NT) {
+                    double xv[2][3], fv[2][3];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int e = e0 + u * WK_NT;
+                        const int dj = e / nb.w, di = e - dj * nb.w;
+                        const int c = (nb.j0 + dj) * g.ex + nb.i0 + di;
 #pragma unroll
                         for (int f = 0; f < 3; ++f) {
-                            const double xv = __ldg(A.x + s.coff + (long long)f * g.ncell + c);
-                            sm[lam + f * FS + q] += C.mu2 * (xv - __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di)) * A.cp.ib[f];
+                            xv[u][f] = e < ncr ? __ldg(A.x + s.coff + (long long)f * g.ncell + c) : 0.0;
+                            fv[u][f] = e < ncr ? __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di) : 0.0;
                         }
                     }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int e = e0 + u * WK_NT;
+                        if (e < ncr) {
+                            const int dj = e / nb.w, di = e - dj * nb.w;
+                            const int q = (nb.j0 + dj) * PL + 1 + nb.i0 + di;
+#pragma unroll
+                            for (int f = 0; f < 3; ++f) sm[lam + f * FS + q] += C.mu2 * (xv[u][f] - fv[u][f]) * A.cp.ib[f];
+                        }
+                    }
+                }
+                __syncthreads();
             }
-            __syncthreads();
-            for (int lj = w; lj < g.ey; lj += WK_NW)
-                for (int li = lane; li < g.ex; li += 32) {
-                    const int c = lj * g.ex + li, q = lj * PL + 1 + li;
+            const bool pred = s.jw > 0;
+            const double bw2 = 2.0 * (s.jw == 0 ? 1.0 : A.cp.bgw);
+            for (int c0 = tid; c0 < g.ncell; c0 += 2 * WK_NT) {
+                double xv[2][3], bv[2][3], pv[2][3], wsp2[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int c = c0 + u * WK_NT;
+                    const bool in = c < g.ncell;
+                    const int lj = c / g.ex, li = c - lj * g.ex;
+                    int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
+                    wsp2[u] = in ? bw2 / (double)(A.geo.ncolcov[gi] * A.geo.nrowcov[s.ej0 + lj]) : 0.0;
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {
                         const long long o = s.coff + (long long)f * g.ncell + c;
-                        const double gg = sm[lam + f * FS + q];
-                        A.gx[o] = gg;
-                        if (A.gw) A.gw[o] = A.cp.sb[f] * gg;
+                        xv[u][f] = in ? __ldg(A.x + o) : 0.0;
+                        bv[u][f] = in ? __ldg(A.xbs + o) : 0.0;
+                        pv[u][f] = (in && pred) ? __ldg(A.pred_end + o) : xv[u][f];
                     }
                 }
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int c = c0 + u * WK_NT;
+                    if (c < g.ncell) {
+                        const int lj = c / g.ex, li = c - lj * g.ex;
+                        const int q = lj * PL + 1 + li;
+#pragma unroll
+                        for (int f = 0; f < 3; ++f) {
+                            const long long o = s.coff + (long long)f * g.ncell + c;
+                            const double gg = sm[lam + f * FS + q] + wsp2[u] * (xv[u][f] - bv[u][f]) * A.cp.ib[f] +
+                                              C.mu2 * (xv[u][f] - pv[u][f]) * A.cp.ib[f];
+                            A.gx[o] = gg;
+                            if (A.gw) A.gw[o] = A.cp.sb[f] * gg;
+                        }
+                    }
+                }
+            }
         }
         __syncthreads();                        // the next subdomain's init overwrites lambda
         gbase += (unsigned)g.W + 1u;

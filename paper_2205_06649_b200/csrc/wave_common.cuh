@@ -30,19 +30,6 @@
 #define WK_HDR 128              // doubles reserved at the start of shared memory (barriers, flags)
 #define WK_SMEM_MAX 232448      // 227 KB: largest opt-in dynamic shared memory of one CTA on sm_100a
 
-// Kernel arguments (by value; everything the two kernels need).
-struct WkArgs {
-    const Sub* subs; const NbRect* nbr; const int* mask; int nsub; int* counter;
-    ModelP m; CostP cp; GeoP geo;
-    const double *x, *xbs, *xfrozen, *pred_end;
-    double* traj; const double* ghost; const double* gedge;
-    const long long* obs_start; const int* obs_idx; const int* obs_lj;
-    const double *obs_y, *obs_c; double* obs_r;
-    double *parts, *J;          // forward outputs: [nsub][5], [nsub]
-    double *gx, *gw;            // adjoint outputs
-    int maxex, maxey, maxpx, maxpy;
-};
-
 // Shared-memory layout in doubles (same function on host and device).
 //   header | row tables [(maxpy+2)][8] | resident state | per-warp staging
 // forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
@@ -82,6 +69,20 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
     L.total = L.wbase + WK_NW * L.wsz + 64;
     return L;
 }
+
+// Kernel arguments (by value; everything the two kernels need).
+struct WkArgs {
+    const Sub* subs; const NbRect* nbr; const int* mask; int nsub; int* counter;
+    ModelP m; CostP cp; GeoP geo;
+    const double *x, *xbs, *xfrozen, *pred_end;
+    double* traj; const double* ghost; const double* gedge;
+    const long long* obs_start; const int* obs_idx; const int* obs_lj;
+    const double *obs_y, *obs_c; double* obs_r;
+    double *parts, *J;          // forward outputs: [nsub][5], [nsub]
+    double *gx, *gw;            // adjoint outputs
+    int maxex, maxey, maxpx, maxpy;
+    WkLayout Lf, La;            // shared-memory layouts (forward, adjoint), computed on the host: constant-bank operands
+};
 
 // ------------------------------------------------------------------------------------------
 // PTX wrappers: mbarrier, TMA bulk copies (cp.async.bulk), proxy fence, release/acquire flags.

@@ -404,7 +404,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
 {
     extern __shared__ __align__(128) double sm[];
     const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(tid >> 5);
-    const WkLayout Ly = wk_layout(false, A.maxex, A.maxey, A.maxpx, A.maxpy);
+    const WkLayout& Ly = A.Lf;
     const uint32_t sm32 = wk_s32(sm);
     const uint32_t b_init = sm32 + 8u * 40u;
     int* s_next = reinterpret_cast<int*>(sm + 52);
@@ -472,19 +472,37 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
         // Rows over warps, columns over lanes; plain sums in a fixed order.
         double bg = 0.0, sp = 0.0, pr = 0.0, ob = 0.0;
         {
+            // (two cells per thread and pass: all loads are issued before the first use)
             const bool pred = s.jw > 0;
-            for (int lj = w; lj < g.ey; lj += WK_NW) {
-                const int nr = A.geo.nrowcov[s.ej0 + lj];
-                for (int li = lane; li < g.ex; li += 32) {
+            const double bw = s.jw == 0 ? 1.0 : A.cp.bgw;
+            for (int c0 = tid; c0 < g.ncell; c0 += 2 * WK_NT) {
+                double bv[2][3], pv[2][3], wsp[2];
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int c = c0 + u * WK_NT;
+                    const bool in = c < g.ncell;
+                    const int lj = c / g.ex, li = c - lj * g.ex;
                     int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
-                    const double wsp = (s.jw == 0 ? 1.0 : A.cp.bgw) / (double)(A.geo.ncolcov[gi] * nr);
-                    const long long cg = s.coff + (long long)lj * g.ex + li;
+                    wsp[u] = in ? bw / (double)(A.geo.ncolcov[gi] * A.geo.nrowcov[s.ej0 + lj]) : 0.0;
 #pragma unroll
                     for (int f = 0; f < 3; ++f) {
-                        const double xv = sm[st + f * FS + lj * P + li];
-                        const double db = xv - __ldg(A.xbs + cg + (long long)f * g.ncell);
-                        bg += wsp * db * db * A.cp.ib[f];
-                        if (pred) { const double dv = xv - __ldg(A.pred_end + cg + (long long)f * g.ncell); pr += dv * dv * A.cp.ib[f]; }
+                        const long long o = s.coff + (long long)f * g.ncell + c;
+                        bv[u][f] = in ? __ldg(A.xbs + o) : 0.0;
+                        pv[u][f] = (in && pred) ? __ldg(A.pred_end + o) : 0.0;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int c = c0 + u * WK_NT;
+                    if (c < g.ncell) {
+                        const int lj = c / g.ex, li = c - lj * g.ex;
+#pragma unroll
+                        for (int f = 0; f < 3; ++f) {
+                            const double xv = sm[st + f * FS + lj * P + li];
+                            const double db = xv - bv[u][f];
+                            bg += wsp[u] * db * db * A.cp.ib[f];
+                            if (pred) { const double dv = xv - pv[u][f]; pr += dv * dv * A.cp.ib[f]; }
+                        }
                     }
                 }
             }
@@ -492,15 +510,29 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             for (int r = 0; r < s.nnb; ++r) {
                 const NbRect nb = A.nbr[s.nb0 + r];
                 const double* xf = A.xfrozen + nb.coff2 + (long long)nb.nj0 * nb.ex2 + nb.ni0;
-                for (int dj = w; dj < nb.h; dj += WK_NW)
-                    for (int di = lane; di < nb.w; di += 32) {
+                const int ncr = nb.w * nb.h;
+                for (int e0 = tid; e0 < ncr; e0 += 2 * WK_NT) {
+                    double fv[2][3];
 #pragma unroll
-                        for (int f = 0; f < 3; ++f) {
-                            const double dv = sm[st + f * FS + (nb.j0 + dj) * P + nb.i0 + di] -
-                                              __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di);
-                            sp += dv * dv * A.cp.ib[f];
+                    for (int u = 0; u < 2; ++u) {
+                        const int e = e0 + u * WK_NT;
+                        const int dj = e / nb.w, di = e - dj * nb.w;
+#pragma unroll
+                        for (int f = 0; f < 3; ++f) fv[u][f] = e < ncr ? __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di) : 0.0;
+                    }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int e = e0 + u * WK_NT;
+                        if (e < ncr) {
+                            const int dj = e / nb.w, di = e - dj * nb.w;
+#pragma unroll
+                            for (int f = 0; f < 3; ++f) {
+                                const double dv = sm[st + f * FS + (nb.j0 + dj) * P + nb.i0 + di] - fv[u][f];
+                                sp += dv * dv * A.cp.ib[f];
+                            }
                         }
                     }
+                }
             }
             if (A.obs_start) {
                 const long long a0 = A.obs_start[s.ooff], a1 = A.obs_start[s.ooff + 1];
@@ -603,14 +635,27 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
         double su = 0.0;
         if (s.jw < A.geo.q - 1) {               // (25c) successor window: Z^W against its frozen control
             const double* xn = A.xfrozen + A.subs[k + A.geo.p1 * A.geo.p2].coff;
-            for (int lj = w; lj < g.ey; lj += WK_NW)
-                for (int li = lane; li < g.ex; li += 32) {
+            for (int c0 = tid; c0 < g.ncell; c0 += 4 * WK_NT) {
+                double nv[4][3];
 #pragma unroll
-                    for (int f = 0; f < 3; ++f) {
-                        const double dv = sm[st + f * FS + lj * P + li] - __ldg(xn + (long long)f * g.ncell + lj * g.ex + li);
-                        su += dv * dv * A.cp.ib[f];
+                for (int u = 0; u < 4; ++u) {
+                    const int c = c0 + u * WK_NT;
+#pragma unroll
+                    for (int f = 0; f < 3; ++f) nv[u][f] = c < g.ncell ? __ldg(xn + (long long)f * g.ncell + c) : 0.0;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int c = c0 + u * WK_NT;
+                    if (c < g.ncell) {
+                        const int lj = c / g.ex, li = c - lj * g.ex;
+#pragma unroll
+                        for (int f = 0; f < 3; ++f) {
+                            const double dv = sm[st + f * FS + lj * P + li] - nv[u][f];
+                            su += dv * dv * A.cp.ib[f];
+                        }
                     }
                 }
+            }
         }
         su = block_sum<WK_NT>(su, red);
         if (tid == 0) {
