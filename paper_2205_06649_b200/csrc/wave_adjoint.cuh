@@ -137,9 +137,10 @@ __device__ __forceinline__ void wa_prep_tile_row(WaCtx<K>& C, int l, const int S
 #define WA_E(arr, i, edge) ((i) < K - 1 ? (arr)[(i) + 1 < K ? (i) + 1 : (i)] : (edge))
 #define WA_W(arr, i, edge) ((i) > 0 ? (arr)[(i) > 0 ? (i) - 1 : 0] : (edge))
 
-// One tick.  P3 / P2: register slots of this tick (t mod 3, t mod 2 counted from the canonical state);
-// EDGE = false: rows t-3 .. t+2 are tile rows, no wall event.
-template <int K, int P2, bool EDGE>
+// One tick.  P2: register slot written by this tick (the other one holds the values of the last tick).
+// WALL = false: no pole-wall event falls on this tick (every tick of a tile without walls; on such
+// ticks whatever is computed on rows outside the padded tile is finite and multiplies lambda = 0).
+template <int K, int P2, bool WALL>
 __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C, double* __restrict__ sm,
                                         const double* __restrict__ tab)
 {
@@ -147,8 +148,8 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     constexpr uint32_t PL8 = 8u * 32u * K;          // lambda row pitch in bytes
     const WkGeo& g = C.g;
     const int lj = t - g.gys;
-    const bool tile = EDGE ? (unsigned)lj < (unsigned)g.ey : true;
-    const bool tile1 = EDGE ? (unsigned)(lj - 1) < (unsigned)g.ey : true;
+    const bool tile = (unsigned)lj < (unsigned)g.ey;
+    const bool tile1 = (unsigned)(lj - 1) < (unsigned)g.ey;
     double zN[3][K];                                // row t (re-read as row t-1 by the next tick: the ring still holds it)
     double (&zC)[3][K] = S.zc[pn];
     double (&zS)[3][K] = S.zc[po];
@@ -159,7 +160,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     {
         const int s0 = t % 3, s1 = s0 == 0 ? 2 : s0 - 1;             // ring slots of rows t, t-1
         const uint32_t h0 = C.zl + s1 * C.SL8 + (tile1 ? 8u : 0u), h1 = h0 + C.ZP8, h2 = h1 + C.ZP8;
-        if (!EDGE || t <= g.py) {                   // row t-1 is a padded row (at t = 0: stale but finite data)
+        if (!WALL || t <= g.py) {                   // row t-1 is a padded row (at t = 0: stale but finite data)
             zC[0][0] = wk_lds<0>(h0); zC[1][0] = wk_lds<0>(h1); zC[2][0] = wk_lds<0>(h2);
             if (K > 1) { zC[0][K > 1 ? 1 : 0] = wk_lds<8>(h0); zC[1][K > 1 ? 1 : 0] = wk_lds<8>(h1); zC[2][K > 1 ? 1 : 0] = wk_lds<8>(h2); }
             if (K > 2) { zC[0][K > 2 ? 2 : 0] = wk_lds<16>(h0); zC[1][K > 2 ? 2 : 0] = wk_lds<16>(h1); zC[2][K > 2 ? 2 : 0] = wk_lds<16>(h2); }
@@ -167,7 +168,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 #pragma unroll
             for (int i = 0; i < K; ++i) { zC[0][i] = zS[0][i]; zC[1][i] = zS[1][i]; zC[2][i] = zS[2][i]; }
         }
-        if (!EDGE || t < g.py) {
+        if (!WALL || t < g.py) {
             const uint32_t a0 = C.zl + s0 * C.SL8 + (tile ? 8u : 0u), a1 = a0 + C.ZP8, a2 = a1 + C.ZP8;
             zN[0][0] = wk_lds<0>(a0); zN[1][0] = wk_lds<0>(a1); zN[2][0] = wk_lds<0>(a2);
             if (K > 1) { zN[0][K > 1 ? 1 : 0] = wk_lds<8>(a0); zN[1][K > 1 ? 1 : 0] = wk_lds<8>(a1); zN[2][K > 1 ? 1 : 0] = wk_lds<8>(a2); }
@@ -188,14 +189,14 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         }
         eL = wk_lds<0>(ea); eR = wk_lds<0>(eb);
     }
-    if (EDGE && g.ws && t == 1) {                   // virtual row -1 (R4)
+    if (WALL && g.ws && t == 1) {                   // virtual row -1 (R4)
 #pragma unroll
         for (int i = 0; i < K; ++i) { zS[0][i] = zC[0][i]; zS[1][i] = zC[1][i]; zS[2][i] = -zC[2][i]; }
     }
-    const bool stage2 = EDGE ? t <= g.py : true;    // row t-1 is a padded row
-    const bool vrN = EDGE ? (g.wn && t == g.py + 1) : false;     // row t-1 is the virtual row py
+    const bool stage2 = WALL ? t <= g.py : true;    // row t-1 is a padded row
+    const bool vrN = WALL ? (g.wn && t == g.py + 1) : false;     // row t-1 is the virtual row py
     const double* t1 = tab + t * 8;                 // table entry of row t-1
-    const double* t2 = EDGE ? tab + (t > 0 ? t - 1 : 0) * 8 : t1 - 8;      // row t-2
+    const double* t2 = tab + (t > 0 ? t - 1 : 0) * 8;      // row t-2
 
     // ---- (2a) row t-1: stage A recomputed
     double ha1[K], ua1[K], uaW, uaE;
@@ -230,7 +231,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 
     // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row
     if (C.has_leader) {
-        const int nd = EDGE ? (t + 4 < C.T + 1 ? t + 4 : C.T + 1) : t + 4;
+        const int nd = t + 4 < C.T + 1 ? t + 4 : C.T + 1;
         wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
     }
     WKP(0)
@@ -251,7 +252,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     WKP(5)
 
     // ---- (2b) lambda^n: v rows t, t-1, t-2; h, u and u^n row t-1.  UB, HB, P and the row-local parts of A on row t-1
-    const uint32_t lrow = C.la0 + (uint32_t)lj * PL8;      // own cell 0 of lambda_h, tile row lj (may be outside: EDGE)
+    const uint32_t lrow = C.la0 + (uint32_t)lj * PL8;      // own cell 0 of lambda_h, tile row lj (may lie outside the tile)
     double P1[K];
     if (stage2) {
         const uint32_t zrow = C.la0 + (uint32_t)C.maxey * PL8;          // the all-zero row
@@ -261,7 +262,7 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         double hb1[K], ub1[K], u1r[K], vbN[K], vbC[K], vbS[K];
         {
             // (rows t-1 and t-2 of lambda_v are still in place: row r is overwritten at tick r + 3)
-            const bool tile2 = EDGE ? (unsigned)(lj - 2) < (unsigned)g.ey : true;
+            const bool tile2 = (unsigned)(lj - 2) < (unsigned)g.ey;
             const uint32_t av = (tile ? lrow : zrow) + 2u * C.FS8, as = (tile2 ? lrow - 2u * PL8 : zrow) + 2u * C.FS8;
             vbN[0] = wk_lds<0>(av); hb1[0] = wk_lds<0>(ah); ub1[0] = wk_lds<0>(au); u1r[0] = wk_lds<0>(a1);
             vbC[0] = wk_lds<0>(ac); vbS[0] = wk_lds<0>(as);
@@ -270,11 +271,11 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
             if (K > 2) { vbN[K > 2 ? 2 : 0] = wk_lds<16>(av); hb1[K > 2 ? 2 : 0] = wk_lds<16>(ah); ub1[K > 2 ? 2 : 0] = wk_lds<16>(au); u1r[K > 2 ? 2 : 0] = wk_lds<16>(a1);
                          vbC[K > 2 ? 2 : 0] = wk_lds<16>(ac); vbS[K > 2 ? 2 : 0] = wk_lds<16>(as); }
         }
-        if (EDGE && g.ws && t == 1) {               // virtual row -1: lambda_v mirrored
+        if (WALL && g.ws && t == 1) {               // virtual row -1: lambda_v mirrored
 #pragma unroll
             for (int i = 0; i < K; ++i) vbS[i] = -vbC[i];
         }
-        if (EDGE && g.wn && t == g.py) {            // virtual row py: lambda_v mirrored
+        if (WALL && g.wn && t == g.py) {            // virtual row py: lambda_v mirrored
 #pragma unroll
             for (int i = 0; i < K; ++i) vbN[i] = -vbC[i];
         }
@@ -291,8 +292,8 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         }
         double PW = wk_up(P1[K - 1]), PE = wk_dn(P1[0]);
         PW = C.lane0 ? 0.0 : PW; PE = C.laneL ? 0.0 : PE;
-        const bool wS1 = EDGE ? (g.ws && t == 1) : false;          // row t-2 is the virtual row -1
-        const double rm0 = EDGE ? tab[8 + WK_T_RM] : 0.0;
+        const bool wS1 = WALL ? (g.ws && t == 1) : false;          // row t-2 is the virtual row -1
+        const double rm0 = WALL ? tab[8 + WK_T_RM] : 0.0;
 #pragma unroll
         for (int i = 0; i < K; ++i) {
             const double vaS = wS1 ? -S.va[pn][i] : S.va[po][i];
@@ -315,9 +316,9 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     double (&Ln)[3][K] = S.mN[pn];                  // L0 of row t-1: northward part of the scatter from row t-2
     double (&La)[3][K] = S.La[pn];                  // L0 of row t-2 (its southward part arrives at the next tick)
     double Lb[3][K];                                // L0 of row t-3: complete
-    if (!EDGE || (t >= 2 && t <= g.py + 1)) {       // (rows -1 and py are virtual: nothing is scattered from them)
+    if (!WALL || (t >= 2 && t <= g.py + 1)) {       // (rows -1 and py are virtual: nothing is scattered from them)
         const double dtcz2 = t2[WK_T_DTCZ], cmrp2 = t2[WK_T_CMRP], cmrm1 = t1[WK_T_CMRM];
-        const bool wallS = EDGE ? (g.ws && t == 2) : false, wallN = EDGE ? (g.wn && t == g.py + 1) : false;
+        const bool wallS = WALL ? (g.ws && t == 2) : false, wallN = WALL ? (g.wn && t == g.py + 1) : false;
         double Aa[3][K], cu[K], cv[K], su[K], sv[K];
 #pragma unroll
         for (int i = 0; i < K; ++i) {
@@ -362,8 +363,8 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 
     // ---- (5) row t-3 of lambda^{n-1} is complete; u^{n-1} of row t-2 replaces u^n
     {
-        const bool st3 = EDGE ? (unsigned)(lj - 3) < (unsigned)g.ey : true;
-        const bool st2 = EDGE ? (unsigned)(lj - 2) < (unsigned)g.ey : true;
+        const bool st3 = (unsigned)(lj - 3) < (unsigned)g.ey;
+        const bool st2 = (unsigned)(lj - 2) < (unsigned)g.ey;
         const uint32_t o0 = lrow - 3u * PL8, o1 = o0 + C.FS8, o2 = o1 + C.FS8, o3 = lrow - 2u * PL8 + 3u * C.FS8;
         if (st3) {
             if (C.tmask & 1u) { wk_sts<0>(o0, Lb[0][0]); wk_sts<0>(o1, Lb[1][0]); wk_sts<0>(o2, Lb[2][0]); }
@@ -377,17 +378,15 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         }
     }
     // the next row of Z^{n-1} must have landed; its ghost cells go in place
-    if (EDGE) { if (t + 1 < g.py) wa_prep_row<K>(C, sm, t + 1); }
-    else wa_prep_tile_row<K>(C, lj + 1, (t + 1) % 3);
+    if (t + 1 < g.py) wa_prep_row<K>(C, sm, t + 1);
     __syncwarp();
     WKP(1)
     // ---- (6) one lane: progress word, the row after next, next E/W chunk
     if (wk_elect()) {
-        if (!EDGE || t < C.T) wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
-        if (EDGE) { if (t + 2 < g.py) wa_issue_row<K>(C, t + 2, false); }
-        else wa_issue_tile_row<K>(C, lj + 2, (t + 2) % 3);
+        wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
+        if (t + 2 < g.py) wa_issue_row<K>(C, t + 2, false);
         const int l1 = lj + 1;
-        if ((!EDGE || (unsigned)l1 < (unsigned)g.ey) && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk)
+        if ((unsigned)l1 < (unsigned)g.ey && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk)
             wa_issue_chunk<K>(C, l1 / WK_EWC + 2);
     }
     WKP(4)
@@ -513,9 +512,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
         }
         C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
         C.T = g.py + 3;
-        // steady ticks: rows t-3 .. t+2 are tile rows, no wall event; groups of six starting at a multiple of three
-        const int ts0 = g.gys + 3 > 3 ? g.gys + 3 : 3;
-        const int ts1 = g.gys + g.ey - 2;       // a steady tick needs t < ts1
 
         // ---------------- the steps of this warp
         for (int m = w; m < g.W; m += WK_NW) {
@@ -555,12 +551,15 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
 #endif
 #pragma unroll 1
             for (int t = 0; t < C.T;) {
-                if (t >= ts0 && t + 2 <= ts1) {
+                const bool wall0 = (g.ws && t <= 2) || (g.wn && t >= g.py);
+                const bool wall1 = (g.ws && t + 1 <= 2) || (g.wn && t + 1 >= g.py);
+                if (!wall0 && !wall1 && t + 2 <= C.T) {
                     wa_tick<K, 0, false>(t, S, C, sm, tab);
                     wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
                     t += 2;
                 } else {
-                    wa_tick<K, 0, true>(t, S, C, sm, tab);
+                    if (wall0) wa_tick<K, 0, true>(t, S, C, sm, tab);
+                    else wa_tick<K, 0, false>(t, S, C, sm, tab);
                     wa_rotate<K>(S);
                     ++t;
                 }
