@@ -549,19 +549,27 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
 #ifdef WK_PROF
             C.pt = clock64();
 #endif
+            // ticks [0, tp0) and [tp1, T): one at a time (pole-wall events, odd remainder); ticks [tp0, tp1): in
+            // pairs (a pair returns every history to the register slot it started in: no register moves)
+            const int tp0 = g.ws ? 3 : 0;
+            int tp1 = g.wn ? g.py : C.T;
+            tp1 -= (tp1 - tp0) & 1;
+            int t = 0;
 #pragma unroll 1
-            for (int t = 0; t < C.T;) {
-                const bool wall0 = (g.ws && t <= 2) || (g.wn && t >= g.py);
-                const bool wall1 = (g.ws && t + 1 <= 2) || (g.wn && t + 1 >= g.py);
-                if (!wall0 && !wall1 && t + 2 <= C.T) {
-                    wa_tick<K, 0, false>(t, S, C, sm, tab);
-                    wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
-                    t += 2;
-                } else {
-                    if (wall0) wa_tick<K, 0, true>(t, S, C, sm, tab);
+            for (int ph = 0; ph < 2; ++ph) {
+                const int tend = ph == 0 ? tp0 : C.T;
+#pragma unroll 1
+                for (; t < tend; ++t) {
+                    if ((g.ws && t <= 2) || (g.wn && t >= g.py)) wa_tick<K, 0, true>(t, S, C, sm, tab);
                     else wa_tick<K, 0, false>(t, S, C, sm, tab);
                     wa_rotate<K>(S);
-                    ++t;
+                }
+                if (ph == 0) {
+#pragma unroll 1
+                    for (; t < tp1; t += 2) {
+                        wa_tick<K, 0, false>(t, S, C, sm, tab);
+                        wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
+                    }
                 }
             }
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);
