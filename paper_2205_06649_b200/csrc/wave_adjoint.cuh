@@ -511,7 +511,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             C.gcp_dst = (lane - 18) * C.ZP;
         }
         C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
-        C.T = g.py + 3;
+        C.T = g.py + 3 - g.gyn;             // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
 
         // ---------------- the steps of this warp
         for (int m = w; m < g.W; m += WK_NW) {

@@ -566,7 +566,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             C.gcp_dst = g.ex + 3 + (lane - 18);
         }
         C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
-        C.T = g.py + 3;
+        C.T = g.py + 3 - g.gyn;             // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
         C.obw = 0.0;                            // this lane's share of H (25b) over this warp's steps
 
         // ---------------- the steps of this warp
