@@ -589,7 +589,7 @@ int dd4dvar_create(const dd4dvar_grid* grid, const dd4dvar_decomp* decomp, const
     if (h->opt.path == 2 && !fits) { delete h; return -2; }
     if ((h->opt.path == 4 || h->opt.path == 5) && !wave) { delete h; return -2; }
     if (h->opt.path < 0 || h->opt.path > 5) { delete h; return -1; }
-    if (h->opt.path == 0) h->L.path = wave ? 4 : (fits ? 2 : 1);
+    if (h->opt.path == 0) h->L.path = wave ? 5 : (fits ? 2 : 1);
     else h->L.path = h->opt.path;
     if (h->L.path != 4 && h->L.path != 5) h->L.wp = WavePlan();
     fused_plan_init(h->G.fp, nullptr, 0, 0);
