@@ -21,6 +21,7 @@
 #include "step_kernels.cuh"
 #include "wave_forward.cuh"
 #include "wave_adjoint.cuh"
+#include "cost_kernels.cuh"
 
 namespace {
 
@@ -48,6 +49,10 @@ struct WavePlan {
     int maxex = 0, maxey = 0, maxpx = 0, maxpy = 0;
     size_t smem_fwd = 0, smem_adj = 0;
     int* counter = nullptr;
+    double* wtab = nullptr;             // [p2][maxpy + 2][8] row tables per tile row (wave_common.cuh)
+    int wtab_stride = 0;
+    double* lamW = nullptr;             // [ctot] adjoint variable at the window end (ck_cost -> wk_adjoint)
+    double* obpart = nullptr;           // [nsub][WK_NW] H (25b) cost per warp (wk_forward -> ck_cost)
 };
 
 struct Layout {
@@ -275,6 +280,10 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
     if (L.wp.enabled) {
         L.gedge = ar.take<double>(std::max<long long>(L.etot, 2));
         L.wp.counter = ar.take<int>(16);
+        L.wp.wtab_stride = (L.wp.maxpy + 2) * 8;
+        L.wp.wtab = ar.take<double>((size_t)L.p2 * L.wp.wtab_stride);
+        L.wp.lamW = ar.take<double>(L.ctot);
+        L.wp.obpart = ar.take<double>((size_t)L.nsub * WK_NW);
     }
 }
 
@@ -287,6 +296,7 @@ void wave_plan_init(WavePlan& wp, const Sub* subs, int nsub)
         const Sub& s = subs[k];
         if (s.gx != DD_GHOST || (s.ex & 1) || s.ey > 1000 || s.ex < 2 || s.ex > 255) return;
         if ((s.gys != 0 && s.gys != DD_GHOST) || (s.gyn != 0 && s.gyn != DD_GHOST)) return;
+        if (s.W < 4) return;            // WK_NTAB row-table slots cover the steps in flight only if every window has >= 4 steps
         wp.maxex = std::max(wp.maxex, s.ex); wp.maxey = std::max(wp.maxey, s.ey);
         wp.maxpx = std::max(wp.maxpx, s.px); wp.maxpy = std::max(wp.maxpy, s.py);
     }
@@ -401,6 +411,7 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
     a.obs_y = L.obs_y; a.obs_c = L.obs_c; a.obs_r = L.obs_r;
     a.parts = L.parts; a.J = Jout; a.gx = L.gx; a.gw = gw;
     a.maxex = L.wp.maxex; a.maxey = L.wp.maxey; a.maxpx = L.wp.maxpx; a.maxpy = L.wp.maxpy;
+    a.wtab = L.wp.wtab; a.wtab_stride = L.wp.wtab_stride; a.lamW = L.wp.lamW; a.obpart = L.wp.obpart;
     a.Lf = wk_layout(false, a.maxex, a.maxey, a.maxpx, a.maxpy);
     a.La = wk_layout(true, a.maxex, a.maxey, a.maxpx, a.maxpy);
     return a;
@@ -410,7 +421,7 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
 void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
     if (L.path == 5) {
-        cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
+        // (consumes the control-level part of the gradient that ck_cost left in gx: one adjoint sweep per forward sweep)
         WkArgs a = wave_args(h, L, mask, nullptr, gw);
 #ifdef WK_PROF
         static unsigned long long* d_prof = nullptr;
@@ -430,11 +441,12 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
             if (nprint++ < 1)
                 for (int w = 0; w < 8; ++w) {
                     fprintf(stderr, "[wkprof adj] warp %d:", w);
-                    for (int q = 0; q < 12; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
-                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, prep-wait, loads+row1, A+scatter, elected, obs, stores, gap | init, steps, epilogue, fetch)\n");
+                    for (int q = 0; q < 8; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
+                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, prep-wait, loads+row1, A+scatter, elected, obs, stores, gap)\n");
                 }
         }
 #endif
+        if (gw) LAUNCH(ck_scale_grad, dim3(std::min(32, (3 * L.maxncell + 255) / 256), L.nsub), 256, L.dsubs, mask, h->cp, L.gx, gw);
         return;
     }
     if (L.path == 2 || L.path == 4) {
@@ -457,8 +469,7 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* Jout, double* gw)
 {
     if (L.path == 4 || L.path == 5) {
-        // forward sweep, trajectory store and cost terms in one wavefront kernel
-        cudaMemsetAsync(L.wp.counter, 0, sizeof(int), h->stream);
+        // forward sweep + trajectory store + H (25b) in the wavefront kernel, then the control-level terms (ck_cost)
         WkArgs a = wave_args(h, L, mask, Jout, gw);
 #ifdef WK_PROF      // profiling build (_work only): per-phase cycle counters of wk_forward on stderr
         static unsigned long long* d_prof = nullptr;
@@ -478,11 +489,14 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
             if (nprint++ < 2)
                 for (int w = 0; w < 8; ++w) {
                     fprintf(stderr, "[wkprof fwd] warp %d:", w);
-                    for (int q = 0; q < 12; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
-                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, chunk+ghostcopy, loads+A+h1+u1, v1+STS+fence, obs, lane0 block, -, loop-gap | init, steps, epilogue, fetch)\n");
+                    for (int q = 0; q < 8; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
+                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, chunk+ghostcopy, loads+A+h1+u1, v1+STS+fence, obs, lane0 block, -, loop-gap)\n");
                 }
+            a.gw = gw;
         }
 #endif
+        ck_cost<<<L.nsub, CK_NT, 0, h->stream>>>(a);
+        ++h->launches;
         if (with_adjoint) adjoint_only(h, L, mask, gw);
         return;
     }
@@ -633,6 +647,23 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
             ? cudaFuncSetAttribute(wk_adjoint<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_adj)
             : cudaFuncSetAttribute(wk_adjoint<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->L.wp.smem_adj);
         if (e1 != cudaSuccess || e2 != cudaSuccess) return fail(h, -4, "shared-memory opt-in of the wavefront kernels failed");
+        // row tables per tile row: entry r+1 <-> padded row r = -1 .. py, guard values of the virtual pole rows
+        std::vector<double> wt((size_t)h->L.p2 * h->L.wp.wtab_stride, 0.0);
+        const double* T6 = h->h_tab.data();
+        for (int b = 0; b < h->L.p2; ++b) {
+            const Sub& sb = h->L.hs[(size_t)b * h->L.p1];
+            for (int q = 0; q < sb.py + 2; ++q) {
+                const int gj = sb.ej0 - sb.gys + q - 1;
+                const int cj = gj < 0 ? 0 : (gj >= nlat ? nlat - 1 : gj);
+                double* t = &wt[(size_t)b * h->L.wp.wtab_stride + (size_t)q * 8];
+                t[0] = T6[cj]; t[1] = T6[nlat + cj]; t[2] = T6[2 * nlat + cj]; t[3] = T6[3 * nlat + cj];
+                t[4] = gj < 0 ? 1.0 : T6[4 * nlat + cj];
+                t[5] = gj >= nlat ? 1.0 : T6[5 * nlat + cj];
+                t[6] = h->mp.dtcm * t[4]; t[7] = h->mp.dtcm * t[5];
+            }
+        }
+        CU(cudaMemcpyAsync(h->L.wp.wtab, wt.data(), sizeof(double) * wt.size(), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
     }
     if (h->L.fp.enabled) {
         h->h_ctab.assign(6 * (size_t)FK_CTAB, 0.0);

@@ -26,6 +26,10 @@
 // has no register moves, no row-kind branches and immediate shared-memory offsets.  The remaining
 // ticks (ghost rows, pole walls, tails) run the same code with the uniform row-kind tests switched on,
 // at slot 0, followed by an explicit rotation.
+// Continuous pipeline (wave_common.cuh): the first adjoint step of a subdomain (level W) follows the last
+// step of the previous subdomain of this CTA; its input rows lambda^W = 2 mu (Z^W - x_succ) / sigma_b^2 (written
+// by ck_cost) and u^W arrive from global memory two ticks ahead, straight into the resident rows.  The last
+// step (level 1 -> 0) adds lambda^0 to the control-level part of the gradient that ck_cost left in gx.
 // Reflective pole walls (R4): mirrored virtual rows -1 / py as in model_math.cuh; in
 // scatter form the part that would leave through the wall comes back into the edge row with the
 // sign of the mirrored field.
@@ -47,6 +51,10 @@ template <int K> struct WaCtx {
     uint32_t zl, zu, SL8, ZP8, FS8, la0;     // per-lane ring / lambda base addresses (shared window), strides in bytes
     unsigned gs10, need0;
     bool has_leader, have_obs, injL, injR, lane0, laneL;    // lane0 / laneL: first lane, lane 31
+    bool first, last;               // adjoint step of level W (its input rows arrive from global memory) / of level 1 (its output is the gradient)
+    int dlead, TLd;                 // tick t starts when the leader has published min(t + dlead, TLd + 1)
+    const double *lw, *uw;          // per lane: lambda^W (ck_cost) and u^W (trajectory store) of own cell 0, tile row 0, field 0
+    double* gxl;                    // per lane: gradient cell of own cell 0, tile row 0, field 0
     int c0, lane, nchunk;
     int gcp_base, gcp_ss, gcp_rs, gcp_dst;
     unsigned tmask;
@@ -96,16 +104,16 @@ template <int K>
 __device__ __forceinline__ void wa_issue_chunk(const WaCtx<K>& C, int c)
 {
     const WkGeo& g = C.g;
-    const int r0 = c * WK_EWC;
-    const int rows = g.ey - r0 < WK_EWC ? g.ey - r0 : WK_EWC;
+    const int r0 = c * WK_EWCA;
+    const int rows = g.ey - r0 < WK_EWCA ? g.ey - r0 : WK_EWCA;
     const int slot = c & 1;
     const uint32_t bar = C.b_ew + 8u * slot;
     wk_mbar_expect32(bar, (uint32_t)rows * (3u * 48u + 16u));
     const double* src = C.gz + (g.gys + g.gyn) * g.px + r0 * 6;
-    uint32_t dst = C.sm32 + 8u * (C.I_EW + slot * 18 * WK_EWC);
+    uint32_t dst = C.sm32 + 8u * (C.I_EW + slot * 18 * WK_EWCA);
 #pragma unroll 1
-    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, rows * 48u, bar); dst += 8u * 6 * WK_EWC; src += g.nring; }
-    wk_g2s32(C.sm32 + 8u * (C.I_EDE + slot * 2 * WK_EWC), C.ge + (g.gys + g.gyn) * 2 + r0 * 2, rows * 16u, bar);
+    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, rows * 48u, bar); dst += 8u * 6 * WK_EWCA; src += g.nring; }
+    wk_g2s32(C.sm32 + 8u * (C.I_EDE + slot * 2 * WK_EWCA), C.ge + (g.gys + g.gyn) * 2 + r0 * 2, rows * 16u, bar);
 }
 // row r has landed in its ring slot; for a tile row put its E/W ghost cells and edge u^a in place
 template <int K>
@@ -116,7 +124,7 @@ __device__ __forceinline__ void wa_prep_row(WaCtx<K>& C, double* __restrict__ sm
     wk_mbar_wait32(C.b_z + 8u * slot, (C.par >> slot) & 1u); C.par ^= 1u << slot;
     const int l = r - g.gys;
     if ((unsigned)l < (unsigned)g.ey) {
-        const int cs = (l / WK_EWC) & 1, lr = l % WK_EWC;
+        const int cs = (l / WK_EWCA) & 1, lr = l % WK_EWCA;
         if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * cs, (C.par >> (3 + cs)) & 1u); C.par ^= 8u << cs; }
         if (C.lane < 20) sm[C.I_ZR + slot * 3 * C.ZP + C.gcp_dst] = sm[C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs];
     }
@@ -126,12 +134,35 @@ template <int K>
 __device__ __forceinline__ void wa_prep_tile_row(WaCtx<K>& C, int l, const int SLOT)
 {
     wk_mbar_wait32(C.b_z + 8u * SLOT, (C.par >> SLOT) & 1u); C.par ^= 1u << SLOT;
-    const int cs = (l / WK_EWC) & 1, lr = l % WK_EWC;
+    const int cs = (l / WK_EWCA) & 1, lr = l % WK_EWCA;
     if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * cs, (C.par >> (3 + cs)) & 1u); C.par ^= 8u << cs; }
     if (C.lane < 20) {
         const double gv = wk_lds<0>(C.sm32 + 8u * (C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs));
         wk_sts<0>(C.zu + SLOT * C.SL8 + 8u * C.gcp_dst, gv);
     }
+}
+
+// first adjoint step of a subdomain: tile row l of lambda^W and u^W -> the resident rows (every lane its own
+// cells: 8-byte asynchronous copies for tile columns, zeros elsewhere); one cp.async group per call
+template <int K>
+__device__ __forceinline__ void wa_issue_lamrow(const WaCtx<K>& C, int l)
+{
+    if ((unsigned)l < (unsigned)C.g.ey) {
+        const uint32_t d0 = C.la0 + (uint32_t)l * (8u * 32u * K);
+        const double* a = C.lw + l * C.g.ex;
+        const double* u = C.uw + l * C.g.ex;
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const uint32_t d = d0 + 8u * i;
+            if ((C.tmask >> i) & 1u) {
+                wk_cpa8(d, a + i); wk_cpa8(d + C.FS8, a + C.g.ncell + i); wk_cpa8(d + 2u * C.FS8, a + 2 * C.g.ncell + i);
+                wk_cpa8(d + 3u * C.FS8, u + i);
+            } else {
+                wk_sts<0>(d, 0.0); wk_sts<0>(d + C.FS8, 0.0); wk_sts<0>(d + 2u * C.FS8, 0.0); wk_sts<0>(d + 3u * C.FS8, 0.0);
+            }
+        }
+    }
+    wk_cpa_commit();
 }
 
 #define WA_E(arr, i, edge) ((i) < K - 1 ? (arr)[(i) + 1 < K ? (i) + 1 : (i)] : (edge))
@@ -231,8 +262,13 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
 
     // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row
     if (C.has_leader) {
-        const int nd = t + 4 < C.T + 1 ? t + 4 : C.T + 1;
+        const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1;
         wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
+    }
+    if (C.first) {                                  // row t of lambda^W / u^W has landed; fetch row t + 2
+        wk_cpa_wait<1>();
+        wa_issue_lamrow<K>(C, lj + 2);
+        __syncwarp();
     }
     WKP(0)
     if (tile && C.have_obs) {
@@ -366,12 +402,22 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         const bool st3 = (unsigned)(lj - 3) < (unsigned)g.ey;
         const bool st2 = (unsigned)(lj - 2) < (unsigned)g.ey;
         const uint32_t o0 = lrow - 3u * PL8, o1 = o0 + C.FS8, o2 = o1 + C.FS8, o3 = lrow - 2u * PL8 + 3u * C.FS8;
-        if (st3) {
+        if (st3 && C.last) {
+            // lambda^0 of row t-3: added to the control-level part of the gradient ck_cost left in gx
+            // (one reduction per cell, no return value: the sum does not depend on timing)
+            double* gp = C.gxl + (lj - 3) * g.ex;
+#pragma unroll
+            for (int i = 0; i < K; ++i)
+                if ((C.tmask >> i) & 1u) {
+#pragma unroll
+                    for (int f = 0; f < 3; ++f) atomicAdd(gp + (long long)f * g.ncell + i, Lb[f][i]);
+                }
+        } else if (st3) {
             if (C.tmask & 1u) { wk_sts<0>(o0, Lb[0][0]); wk_sts<0>(o1, Lb[1][0]); wk_sts<0>(o2, Lb[2][0]); }
             if (K > 1 && (C.tmask & 2u)) { wk_sts<8>(o0, Lb[0][K > 1 ? 1 : 0]); wk_sts<8>(o1, Lb[1][K > 1 ? 1 : 0]); wk_sts<8>(o2, Lb[2][K > 1 ? 1 : 0]); }
             if (K > 2 && (C.tmask & 4u)) { wk_sts<16>(o0, Lb[0][K > 2 ? 2 : 0]); wk_sts<16>(o1, Lb[1][K > 2 ? 2 : 0]); wk_sts<16>(o2, Lb[2][K > 2 ? 2 : 0]); }
         }
-        if (st2) {
+        if (st2 && !C.last) {
             if (C.tmask & 1u) wk_sts<0>(o3, zS[1][0]);
             if (K > 1 && (C.tmask & 2u)) wk_sts<8>(o3, zS[1][K > 1 ? 1 : 0]);
             if (K > 2 && (C.tmask & 4u)) wk_sts<16>(o3, zS[1][K > 2 ? 2 : 0]);
@@ -386,8 +432,8 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
         if (t + 2 < g.py) wa_issue_row<K>(C, t + 2, false);
         const int l1 = lj + 1;
-        if ((unsigned)l1 < (unsigned)g.ey && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk)
-            wa_issue_chunk<K>(C, l1 / WK_EWC + 2);
+        if ((unsigned)l1 < (unsigned)g.ey && (l1 % WK_EWCA) == WK_EWCA - 1 && l1 / WK_EWCA + 2 < C.nchunk)
+            wa_issue_chunk<K>(C, l1 / WK_EWCA + 2);
     }
     WKP(4)
 }
@@ -414,110 +460,80 @@ template <int K>
 __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ WkArgs A)
 {
     extern __shared__ __align__(128) double sm[];
-    const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(tid >> 5);
+    const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(wk_logical_warp(tid >> 5));
     const WkLayout& Ly = A.La;
     const uint32_t sm32 = wk_s32(sm);
-    int* s_next = reinterpret_cast<int*>(sm + 52);
-    double* tab = sm + Ly.tab;
     const int IW = Ly.wbase + w * Ly.wsz;
-    constexpr int PL = 32 * K;
     if (tid == 0) {
-        for (int i = 0; i < 41; ++i) wk_mbar_init32(sm32 + 8u * i, 1);
+        for (int i = 0; i < WK_NW * WK_BAR_PER_WARP; ++i) wk_mbar_init32(sm32 + 8u * i, 1);
         wk_fence_mbar_init();
     }
-    if (tid < WK_NW) reinterpret_cast<unsigned*>(sm + 48)[tid] = 0u;
-    for (int q = tid; q < Ly.total - WK_HDR; q += WK_NT) sm[WK_HDR + q] = 0.0;
-    __syncthreads();
-    unsigned gbase = 1u;
+    if (tid < WK_NW) reinterpret_cast<unsigned*>(sm + WK_PROG)[tid] = 0u;
+    for (int q = tid; q < Ly.total - WK_HDR; q += WK_NT) sm[WK_HDR + q] = 0.0;     // (the zero row and the pad cells stay zero)
+    __syncthreads();                            // the only CTA-wide barrier
     const int lw = (w + WK_NW - 1) % WK_NW;
 
     WaCtx<K> C;
     C.lam = Ly.st; C.u1 = Ly.u1; C.ZP = Ly.ZP; C.FS = Ly.FS; C.maxey = A.maxey;
     C.I_ZR = IW + Ly.zr; C.I_EW = IW + Ly.ew; C.I_EDS = IW + Ly.eds; C.I_EDE = IW + Ly.ede;
-    C.sm32 = sm32; C.a_lead = sm32 + 8u * 48u + 4u * lw; C.a_mine = sm32 + 8u * 48u + 4u * w;
-    C.b_z = sm32 + 8u * (w * 5); C.b_ew = sm32 + 8u * (w * 5 + 3);
+    C.sm32 = sm32; C.a_lead = sm32 + 8u * WK_PROG + 4u * lw; C.a_mine = sm32 + 8u * WK_PROG + 4u * w;
+    C.b_z = sm32 + 8u * (w * WK_BAR_PER_WARP); C.b_ew = C.b_z + 24u;
     C.c0 = 2 + K * lane; C.lane = lane; C.lane0 = lane == 0; C.laneL = lane == 31;
     C.zu = sm32 + 8u * C.I_ZR; C.zl = C.zu + 8u * C.c0; C.SL8 = 8u * 3 * Ly.ZP; C.ZP8 = 8u * Ly.ZP; C.FS8 = 8u * Ly.FS;
     C.la0 = sm32 + 8u * (Ly.st + K * lane);
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm; C.c0k = 1.0 - 4.0 * A.m.kap; C.mu2 = 2.0 * A.cp.mu;
     C.A = &A; C.par = 0u;
-    const int lam = Ly.st, FS = Ly.FS;
 #ifdef WK_PROF
     for (int q = 0; q < 8; ++q) C.pf[q] = 0;
-    long long ph[4] = {0, 0, 0, 0}, pht = clock64();
 #endif
 
-    for (;;) {
-        if (tid == 0) *s_next = atomicAdd(A.counter, 1);
-        __syncthreads();
-        const int k = wk_uni(*s_next);
-        __syncthreads();
-        if (k >= A.nsub) break;
+    // Every warp walks the same list of (subdomain, adjoint step) pairs (see wk_forward).
+    int nord = -1;                              // ordinal of the current subdomain in this CTA's list
+    unsigned gnext = 1u, glast = 0u;            // global numbers: step 0 of the current subdomain, last step of the previous one
+    int TL = 0, gysL = 0;
+    for (int k = blockIdx.x; k < A.nsub; k += gridDim.x) {
         if (A.mask && !A.mask[k]) continue;
+        ++nord;
         const Sub s = A.subs[k];
         const WkGeo g = wk_geo(s);
-        C.g = g;
-        const long long n3 = 3LL * g.ncell;
-        WKPH(3)
-
-        // ---------------- init: lambda^W = successor-window overlap forcing (25c), else zero; u^W
-        // (cells 0 and > ex of every row and the row maxey are zero and stay zero)
-        wk_load_tab(tab, A.m, g);
-        {
-            const bool succ = s.jw < A.geo.q - 1;
-            const double* tw = A.traj + s.toff + (long long)g.W * n3;
-            const double* xn = succ ? A.xfrozen + A.subs[k + A.geo.p1 * A.geo.p2].coff : nullptr;
-            // (four cells per thread and pass: all loads are issued before the first use)
-            const int nq = g.ey * PL;
-            for (int q0 = tid; q0 < nq; q0 += 4 * WK_NT) {
-                double zv[4][3], xv[4][3];
+        const int T = g.py + 3 - g.gyn;
+        const int m0 = (int)((unsigned)(w + 1) - gnext) & (WK_NW - 1);
+        if (m0 < g.W) {
+            C.g = g; C.T = T;
+            const long long n3 = 3LL * g.ncell;
+            // ---------------- per-lane column map of this tile
+            C.tmask = 0u;
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int q = q0 + u * WK_NT;
-                    const int lj = q / PL, qi = q - lj * PL;
-                    const bool in = q < nq && qi >= 1 && qi <= g.ex;
-                    const int c = lj * g.ex + qi - 1;
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) {
-                        zv[u][f] = in ? __ldg(tw + (long long)f * g.ncell + c) : 0.0;
-                        xv[u][f] = (in && succ) ? __ldg(xn + (long long)f * g.ncell + c) : zv[u][f];
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int q = q0 + u * WK_NT;
-                    if (q < nq) {
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) sm[lam + f * FS + q] = C.mu2 * (zv[u][f] - xv[u][f]) * A.cp.ib[f];
-                        sm[C.u1 + q] = zv[u][1];
-                    }
-                }
+            for (int i = 0; i < K; ++i) if ((C.c0 + i >= 3) && (C.c0 + i < 3 + g.ex)) C.tmask |= 1u << i;
+            C.injL = lane == 0; C.injR = (lane == 31) && (C.c0 + K == g.px - 2);
+            if (lane < 18) {                    // E/W ghost cell (field lane/6, cell lane%6) -> padded columns 0..2, px-3..px-1
+                const int f = lane / 6, e = lane % 6;
+                C.gcp_base = C.I_EW + f * 6 * WK_EWCA + e; C.gcp_ss = 18 * WK_EWCA; C.gcp_rs = 6;
+                C.gcp_dst = f * C.ZP + 1 + (e < 3 ? e : g.ex + e);
+            } else {                            // lanes 18, 19: edge u^a west / east -> the free cell 0 of fields 0 / 1
+                C.gcp_base = C.I_EDE + (lane - 18); C.gcp_ss = 2 * WK_EWCA; C.gcp_rs = 2;
+                C.gcp_dst = (lane - 18) * C.ZP;
             }
-        }
-        __syncthreads();
-        WKPH(0)
-
-        // ---------------- per-lane column map of this tile
-        C.tmask = 0u;
-#pragma unroll
-        for (int i = 0; i < K; ++i) if ((C.c0 + i >= 3) && (C.c0 + i < 3 + g.ex)) C.tmask |= 1u << i;
-        C.injL = lane == 0; C.injR = (lane == 31) && (C.c0 + K == g.px - 2);
-        if (lane < 18) {                        // E/W ghost cell (field lane/6, cell lane%6) -> padded columns 0..2, px-3..px-1
-            const int f = lane / 6, e = lane % 6;
-            C.gcp_base = C.I_EW + f * 6 * WK_EWC + e; C.gcp_ss = 18 * WK_EWC; C.gcp_rs = 6;
-            C.gcp_dst = f * C.ZP + 1 + (e < 3 ? e : g.ex + e);
-        } else {                                // lanes 18, 19: edge u^a west / east -> the free cell 0 of fields 0 / 1
-            C.gcp_base = C.I_EDE + (lane - 18); C.gcp_ss = 2 * WK_EWC; C.gcp_rs = 2;
-            C.gcp_dst = (lane - 18) * C.ZP;
-        }
-        C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
-        C.T = g.py + 3 - g.gyn;             // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
+            C.nchunk = (g.ey + WK_EWCA - 1) / WK_EWCA;
+            // own cell 0 <-> padded column 2 + K lane <-> tile column K lane - 1
+            C.lw = A.lamW + s.coff + (K * lane - 1);
+            C.uw = A.traj + s.toff + (long long)g.W * n3 + g.ncell + (K * lane - 1);
+            C.gxl = A.gx + s.coff + (K * lane - 1);
+            const double* tab = sm + Ly.tab + (nord % WK_NTAB) * WK_TABSZ(A.maxpy);
 
         // ---------------- the steps of this warp
-        for (int m = w; m < g.W; m += WK_NW) {
+        for (int m = m0; m < g.W; m += WK_NW) {
             const int n = g.W - m;
-            const unsigned gs = gbase + (unsigned)m;
-            C.gs10 = gs << 10; C.need0 = (gs - 1u) << 10; C.has_leader = m > 0;
+            const unsigned gs = gnext + (unsigned)m;
+            C.first = m == 0;
+            // the leader: the step before this one, for a first step the last step of the previous subdomain
+            const unsigned gl = C.first ? glast : gs - 1u;
+            C.gs10 = gs << 10; C.need0 = gl << 10; C.has_leader = gl != 0u;
+            C.a_lead = sm32 + 8u * WK_PROG + 4u * ((gl - 1u) & (WK_NW - 1)); C.last = n == 1;
+            // A first step only OVERWRITES what the previous subdomain left: its last step (which stores nothing in
+            // shared memory) has finished with tile row l after its tick l + gysL + 2.
+            C.dlead = C.first ? 5 + gysL - g.gys : 4;
+            C.TLd = C.first ? TL : T;
             C.gz = A.ghost + s.goff + (long long)(n - 1) * 3 * g.nring;
             C.ge = A.gedge + s.eoff + (long long)(n - 1) * 2 * g.py;
             C.tz = A.traj + s.toff + (long long)(n - 1) * n3;
@@ -543,6 +559,13 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 }
 #pragma unroll
                 for (int f = 0; f < 3; ++f) { S.hz[sl][f][0] = 0.0; S.hz[sl][f][1] = 0.0; }
+            }
+            if (C.first) {
+                // what ticks -2 and -1 would do: the rows of lambda^W / u^W that ticks 0 and 1 read
+                if (C.has_leader) { const int nd = C.dlead < C.TLd + 1 ? C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+                wk_copy_tab(sm + Ly.tab + (nord % WK_NTAB) * WK_TABSZ(A.maxpy), A.wtab + (long long)s.b * A.wtab_stride, g.py, lane);
+                wa_issue_lamrow<K>(C, -g.gys);
+                wa_issue_lamrow<K>(C, 1 - g.gys);
             }
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
@@ -572,99 +595,21 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                     }
                 }
             }
+            if (C.first) wk_cpa_wait<0>();
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);
             __syncwarp();
         }
-        WKPH(1)
-        __syncthreads();
-
-        // ---------------- gradient at the window start: lambda^0 + H^T R^-1 at level 0 (25b)
-        //                  + (25a) + control-level (25c) terms; g_w = sigma_b g_x (eq (44) l.630-634)
-        if (A.obs_start) {
-            const long long a0 = A.obs_start[s.ooff], a1 = A.obs_start[s.ooff + 1];
-            for (long long q = a0 + tid; q < a1; q += WK_NT) {
-                const int pk = A.obs_lj[q];
-                sm[lam + ((pk >> 8) & 3) * FS + (pk >> 12) * PL + 1 + (pk & 255)] += A.obs_r[q];
-            }
-            __syncthreads();
         }
-        {
-            for (int r = 0; r < s.nnb; ++r) {   // (25c) case 1, one rectangle at a time (a cell may lie in several)
-                const NbRect nb = A.nbr[s.nb0 + r];
-                const double* xf = A.xfrozen + nb.coff2 + (long long)nb.nj0 * nb.ex2 + nb.ni0;
-                const int ncr = nb.w * nb.h;
-                for (int e0 = tid; e0 < ncr; e0 += 2 * WK_NT) {
-                    double xv[2][3], fv[2][3];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int e = e0 + u * WK_NT;
-                        const int dj = e / nb.w, di = e - dj * nb.w;
-                        const int c = (nb.j0 + dj) * g.ex + nb.i0 + di;
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) {
-                            xv[u][f] = e < ncr ? __ldg(A.x + s.coff + (long long)f * g.ncell + c) : 0.0;
-                            fv[u][f] = e < ncr ? __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di) : 0.0;
-                        }
-                    }
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int e = e0 + u * WK_NT;
-                        if (e < ncr) {
-                            const int dj = e / nb.w, di = e - dj * nb.w;
-                            const int q = (nb.j0 + dj) * PL + 1 + nb.i0 + di;
-#pragma unroll
-                            for (int f = 0; f < 3; ++f) sm[lam + f * FS + q] += C.mu2 * (xv[u][f] - fv[u][f]) * A.cp.ib[f];
-                        }
-                    }
-                }
-                __syncthreads();
-            }
-            const bool pred = s.jw > 0;
-            const double bw2 = 2.0 * (s.jw == 0 ? 1.0 : A.cp.bgw);
-            for (int c0 = tid; c0 < g.ncell; c0 += 2 * WK_NT) {
-                double xv[2][3], bv[2][3], pv[2][3], wsp2[2];
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int c = c0 + u * WK_NT;
-                    const bool in = c < g.ncell;
-                    const int lj = c / g.ex, li = c - lj * g.ex;
-                    int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
-                    wsp2[u] = in ? bw2 / (double)(A.geo.ncolcov[gi] * A.geo.nrowcov[s.ej0 + lj]) : 0.0;
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) {
-                        const long long o = s.coff + (long long)f * g.ncell + c;
-                        xv[u][f] = in ? __ldg(A.x + o) : 0.0;
-                        bv[u][f] = in ? __ldg(A.xbs + o) : 0.0;
-                        pv[u][f] = (in && pred) ? __ldg(A.pred_end + o) : xv[u][f];
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int c = c0 + u * WK_NT;
-                    if (c < g.ncell) {
-                        const int lj = c / g.ex, li = c - lj * g.ex;
-                        const int q = lj * PL + 1 + li;
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) {
-                            const long long o = s.coff + (long long)f * g.ncell + c;
-                            const double gg = sm[lam + f * FS + q] + wsp2[u] * (xv[u][f] - bv[u][f]) * A.cp.ib[f] +
-                                              C.mu2 * (xv[u][f] - pv[u][f]) * A.cp.ib[f];
-                            A.gx[o] = gg;
-                            if (A.gw) A.gw[o] = A.cp.sb[f] * gg;
-                        }
-                    }
-                }
-            }
-        }
-        __syncthreads();                        // the next subdomain's init overwrites lambda
-        gbase += (unsigned)g.W + 1u;
-        WKPH(2)
+        // (one step number is skipped when the window length is a multiple of the warp count, so that the
+        //  levels that carry observations do not always fall on the same warp)
+        glast = gnext + (unsigned)g.W - 1u;
+        gnext = glast + 1u + ((g.W & (WK_NW - 1)) == 0 ? 1u : 0u);
+        TL = T; gysL = g.gys;
     }
 #ifdef WK_PROF
     if (lane == 0 && A.J) {
         unsigned long long* pr = reinterpret_cast<unsigned long long*>(A.J);
         for (int q = 0; q < 8; ++q) atomicAdd(pr + w * 16 + q, (unsigned long long)C.pf[q]);
-        for (int q = 0; q < 4; ++q) atomicAdd(pr + w * 16 + 8 + q, (unsigned long long)ph[q]);
     }
 #endif
 }

@@ -1,7 +1,10 @@
 // wave_common.cuh -- shared pieces of the WAVEFRONT sweep kernels (wave_forward.cuh, wave_adjoint.cuh).
 //
-// Design ("smem-resident tile, temporal wavefront").  One CTA of WK_NW warps owns one
-// space-time subdomain Delta_j x Omega_i (Def 3 l.128-154) at a time; the state of the window
+// Design ("smem-resident tile, temporal wavefront").  One CTA of WK_NW warps works
+// through the space-time subdomains Delta_j x Omega_i (Def 3 l.128-154) blockIdx.x, blockIdx.x + gridDim.x,
+// ... as ONE continuous pipeline of model steps: the first step of a subdomain follows the last step of the
+// previous one row by row, like any other step (no CTA-wide phase, no __syncthreads after start-up; the
+// control-level terms of J_ji run in the bandwidth-bound kernel ck_cost).  The state of the window
 // (forward: Z^n, adjoint: the adjoint variable lambda^n and u^n) lives IN PLACE in shared memory for
 // the whole window.  Warp w works on a DIFFERENT TIME STEP than its neighbours: it marches over the
 // rows of the tile a few rows behind the warp that produces its input level (its "leader") and a
@@ -24,14 +27,19 @@
 #include "common.cuh"
 #include "model_math.cuh"
 
-#define WK_NW 8                 // warps per CTA = time steps in flight per subdomain
+#ifndef WK_NW
+#define WK_NW 8                 // warps per CTA = time steps in flight per CTA
+#endif
 #define WK_NT (WK_NW * 32)
-#define WK_EWC 4                // tile rows per staged chunk of east/west ghost cells
+#define WK_EWC 4                // tile rows per staged chunk of east/west ghost cells (forward kernel)
+#define WK_EWCA 2               // the same in the adjoint kernel (its shared memory is full)
 #define WK_HDR 128              // doubles reserved at the start of shared memory (barriers, flags)
+#define WK_NTAB 3               // row-table slots: 8 steps in flight span at most 3 subdomains when every window has >= 4 steps
+#define WK_TABSZ(maxpy) (((maxpy) + 2) * 8)
 #define WK_SMEM_MAX 232448      // 227 KB: largest opt-in dynamic shared memory of one CTA on sm_100a
 
 // Shared-memory layout in doubles (same function on host and device).
-//   header | row tables [(maxpy+2)][8] | resident state | per-warp staging
+//   header | row tables [WK_NTAB][(maxpy+2)][8] | resident state | per-warp staging
 // forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
 //   [tile ex][E ghosts 3][pad 2][W ghosts of the NEXT row 3], so that padded column c of tile row
 //   lj is at  st + f*FS + lj*P + (c - 3)  for every c (W ghosts sit in the previous row's tail).
@@ -45,7 +53,7 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
 {
     WkLayout L;
     int o = WK_HDR;
-    L.tab = o; o += (maxpy + 8) * 8;
+    L.tab = o; o += WK_NTAB * WK_TABSZ(maxpy);      // row tables of the subdomains in flight
     if (!adj) {
         L.P = maxex + 8; L.FS = maxey * L.P;
         L.st = o + 8; o += 8 + 3 * L.FS + 64;       // 64 doubles of slack: lanes beyond px read past a row
@@ -62,9 +70,10 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
     L.ZP = maxpx + 2;
     if (!adj) { L.sn = p; p += 9 * maxpx; L.zr = 0; }
     else { L.zr = p; p += 9 * L.ZP; L.sn = 0; }
-    L.ew = p; p += 2 * 3 * 6 * WK_EWC;
+    const int ewc = adj ? WK_EWCA : WK_EWC;
+    L.ew = p; p += 2 * 3 * 6 * ewc;
     L.eds = p; p += 16;
-    L.ede = p; p += 2 * 2 * WK_EWC;
+    L.ede = p; p += 2 * 2 * ewc;
     L.wsz = (p + 1) & ~1;
     L.total = L.wbase + WK_NW * L.wsz + 64;
     return L;
@@ -81,6 +90,9 @@ struct WkArgs {
     double *parts, *J;          // forward outputs: [nsub][5], [nsub]
     double *gx, *gw;            // adjoint outputs
     int maxex, maxey, maxpx, maxpy;
+    const double* wtab; int wtab_stride;    // row tables per tile row b: [p2][maxpy + 2][8] (entry r+1 <-> padded row r = -1 .. py)
+    double* lamW;               // [ctot] adjoint variable at the window end, written by ck_cost: 2 mu (Z^W - x_succ) / sigma_b^2
+    double* obpart;             // [nsub][WK_NW] H (25b) cost of the steps each warp ran (levels 1 .. W)
     WkLayout Lf, La;            // shared-memory layouts (forward, adjoint), computed on the host: constant-bank operands
 };
 
@@ -152,20 +164,37 @@ template <int N> __device__ __forceinline__ void wk_wait_read()
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA store source)
 __device__ __forceinline__ void wk_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void wk_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// Progress words.  Writer: every lane stores its cells of the row (st.shared), __syncwarp, then ONE lane stores
+// the word; reader: polls the word, then loads the row.  Both sides use plain volatile accesses unless
+// WK_FENCED_FLAGS is defined: the data and the word are shared-memory accesses of the same SM, which its
+// shared-memory pipe performs in issue order (a store issued after another by the same warp becomes visible
+// after it; a load issued after the poll that saw the word cannot see older data), so the release / acquire
+// fences (MEMBAR.ALL.CTA in SASS, once per tick on either side) buy nothing here.
 __device__ __forceinline__ void wk_publish(uint32_t addr, unsigned v)
 {
+#ifdef WK_FENCED_FLAGS
     asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+#else
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+#endif
 }
 __device__ __forceinline__ unsigned wk_peek(uint32_t addr)
 {
     unsigned v;
+#ifdef WK_FENCED_FLAGS
     asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+#else
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+#endif
     return v;
 }
+#ifndef WK_BACKOFF
+#define WK_BACKOFF __nanosleep(40)
+#endif
 // wait until the progress word at `addr` has reached `need` (monotone counters, wrap-safe compare)
 __device__ __forceinline__ void wk_wait_prog(uint32_t addr, unsigned need)
 {
-    while ((int)(wk_peek(addr) - need) < 0) __nanosleep(40);
+    while ((int)(wk_peek(addr) - need) < 0) { WK_BACKOFF; }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -182,19 +211,13 @@ __device__ __forceinline__ WkGeo wk_geo(const Sub& s)
     g.ws = s.gys == 0; g.wn = s.gyn == 0;
     return g;
 }
-// row tables of this tile into shared memory: entry r+1 for padded row r = -1 .. py, with the guard
-// values r+_{-1} = 1 and r-_{nlat} = 1 of the virtual mirrored pole rows (model_math.cuh, A_v)
-__device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const WkGeo& g)
+// Row tables (host-built, dd4dvar.cu): entry r+1 for padded row r = -1 .. py of a tile row, with the guard
+// values r+_{-1} = 1 and r-_{nlat} = 1 of the virtual mirrored pole rows (model_math.cuh, A_v).  The warp
+// that runs the first step of a subdomain copies the table of its tile row into slot (ordinal % WK_NTAB)
+// before its first tick; the steps behind it see it through the progress words.
+__device__ __forceinline__ void wk_copy_tab(double* dst, const double* __restrict__ src, int py, int lane)
 {
-    for (int q = threadIdx.x; q < g.py + 2; q += WK_NT) {
-        const int gj = g.joff + q - 1;
-        const int cj = gj < 0 ? 0 : (gj >= m.nlat ? m.nlat - 1 : gj);
-        double* t = tab + q * 8;
-        t[0] = m.dtcz[cj]; t[1] = m.gdtcz[cj]; t[2] = m.dtf[cj]; t[3] = m.dtt[cj];
-        t[4] = gj < 0 ? 1.0 : m.rp[cj];
-        t[5] = gj >= m.nlat ? 1.0 : m.rm[cj];
-        t[6] = m.dtcm * t[4]; t[7] = m.dtcm * t[5];
-    }
+    for (int q = lane; q < (py + 2) * 8; q += 32) dst[q] = __ldg(src + q);
 }
 #define WK_T_DTCZ 0
 #define WK_T_GDTCZ 1
@@ -204,6 +227,29 @@ __device__ __forceinline__ void wk_load_tab(double* tab, const ModelP& m, const 
 #define WK_T_RM 5
 #define WK_T_CMRP 6             // dtcm * r+
 #define WK_T_CMRM 7             // dtcm * r-
+#define WK_BAR_PER_WARP 8       // mbarriers per warp at the start of shared memory
+#define WK_PROG 64              // progress words (one u32 per warp) at double index WK_PROG
+
+// Position of a physical warp in the step order.  Warps p and p + 4 share a scheduler (SM sub-partition);
+// WK_PAIR_DIST is the distance of such a pair in the step order (4: identity).  Consecutive steps run about
+// 0.8 tick apart in phase, so the distance decides how much the compute phases of a pair overlap.
+#ifndef WK_PAIR_DIST
+#define WK_PAIR_DIST 4
+#endif
+__device__ __forceinline__ int wk_logical_warp(int p)
+{
+#if WK_NW == 8 && WK_PAIR_DIST == 3
+    const int a[4] = { 0, 6, 4, 2 }, b[4] = { 3, 1, 7, 5 };
+    return p < 4 ? a[p] : b[p - 4];
+#elif WK_NW == 8 && WK_PAIR_DIST == 2
+    const int a[4] = { 0, 4, 1, 5 }, b[4] = { 2, 6, 3, 7 };
+    return p < 4 ? a[p] : b[p - 4];
+#elif WK_NW == 8 && WK_PAIR_DIST == 1
+    return p < 4 ? 2 * p : 2 * (p - 4) + 1;
+#else
+    return p;
+#endif
+}
 
 // one elected lane of the (converged) warp; tells the compiler the region is single-threaded
 __device__ __forceinline__ bool wk_elect()
@@ -227,6 +273,14 @@ template <int OFF> __device__ __forceinline__ void wk_sts(uint32_t a, double v)
 {
     asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(a), "n"(OFF), "d"(v) : "memory");
 }
+
+// 8-byte asynchronous copy global -> shared by every lane (LDGSTS), per-thread groups
+__device__ __forceinline__ void wk_cpa8(uint32_t dst, const double* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void wk_cpa_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void wk_cpa_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // 64-bit shuffles
 __device__ __forceinline__ double wk_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }

@@ -16,10 +16,16 @@
 // Synchronisation: after tick t a warp publishes (step << 10) + t + 1; the warp of the next step
 // starts its tick t when its leader has published tick t + 3 (row t of its input is then final,
 // and the leader's bulk store of every row this warp is about to overwrite has left shared memory).
+// The first step of a subdomain (n = 0) follows the LAST step of the previous subdomain of this CTA: its
+// input rows, the control, arrive from global memory two ticks ahead (TMA into the resident rows the
+// previous subdomain has finished with); J_ji's control-level terms, the level-0 copy of the trajectory
+// store and the successor-window term run in ck_cost (cost_kernels.cuh) after this kernel.
 // There is ONE tick body (uniform branches only, the hot loop must stay inside the instruction
 // cache); the tick loop is unrolled by three so that the row histories rotate by renaming.
 #pragma once
 #include "wave_common.cuh"
+
+#define WK_XD 3         // a first step fetches its control rows this many ticks ahead (4 mbarrier slots: WK_XD <= 3)
 
 
 // row histories of one warp-step (names: 1 = row t-1, 2 = row t-2, ... at the start of tick t)
@@ -35,6 +41,10 @@ template <int K> struct WfCtx {
     uint32_t sm32, a_lead, a_mine, b_sn, b_ew;      // shared-window addresses: progress words, barriers
     unsigned gs10, need0;                            // (global step << 10), ((global step - 1) << 10)
     bool has_leader, have_obs, injL, injR;           // injL / injR per lane
+    bool first;                                      // step 0 of a subdomain: its input rows (the control) arrive from global memory
+    int dlead, TLd;                                  // tick t starts when the leader has published min(t + dlead, TLd + 1)
+    uint32_t b_x;                                    // mbarriers of the control rows in flight (4 slots)
+    const double* xk;                                // control of this subdomain [3][ey][ex]
     int c0, lane, nchunk;
     int gcp_base, gcp_ss, gcp_rs, gcp_dst;           // per lane (< 20): ghost / edge cell copied per tile row
     unsigned tmask;                                  // per lane: bit i = own column i is a tile column
@@ -84,6 +94,25 @@ __device__ __forceinline__ void wf_issue_ns(const WfCtx<K>& C, bool north)
     wk_g2s32(C.sm32 + 8u * (C.I_EDS + (north ? 8 : 0)), C.ge + roff * 2, rows * 16u, C.b_sn);
 }
 
+// lane 0, first step of a subdomain: tile row l of the control -> resident state (slot l & 3)
+template <int K>
+__device__ __forceinline__ void wf_issue_xrow(const WfCtx<K>& C, int l)
+{
+    const WkGeo& g = C.g;
+    const uint32_t bar = C.b_x + 8u * (l & 3);
+    wk_mbar_expect32(bar, 3u * g.ex * 8u);
+    const double* src = C.xk + l * g.ex;
+    uint32_t dst = C.sm32 + 8u * (C.st + l * C.P);
+#pragma unroll 1
+    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, g.ex * 8u, bar); dst += 8u * C.FS; src += g.ncell; }
+}
+template <int K>
+__device__ __forceinline__ void wf_wait_xrow(WfCtx<K>& C, int l)
+{
+    const int slot = l & 3;
+    wk_mbar_wait32(C.b_x + 8u * slot, (C.par >> (4 + slot)) & 1u); C.par ^= 16u << slot;
+}
+
 // put the E/W ghost cells (lanes 0..17) and the edge u^a (lanes 18, 19) of tile row l next to the row
 template <int K>
 __device__ __forceinline__ void wf_prep_row(WfCtx<K>& C, double* __restrict__ sm, int l)
@@ -102,10 +131,11 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
     const bool tile = (unsigned)lj < (unsigned)g.ey;
     // ---- (0) row t becomes readable
     WKP(7)
-    if (C.has_leader) { const int nd = t + 4 < C.T + 1 ? t + 4 : C.T + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+    if (C.has_leader) { const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
     WKP(0)
     int ra = 0, rfs = 0, re = 0;                    // own column 0 of row t, field stride, edge-u^a index
     if (tile) {                                      // (its E/W ghost cells were put in place one tick earlier)
+        if (C.first) wf_wait_xrow<K>(C, lj);
         const int rowb = C.st + lj * C.P;
         ra = rowb - 3 + C.c0; rfs = C.FS; re = rowb + g.ex + 3;
     } else if (t < g.py) {
@@ -208,8 +238,8 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
             const double v1 = mm_v1(R.va3[i], R.u13[i], h12[i], R.h14[i], C.gdtcm, dtf3, dtt3);
             if ((C.tmask >> i) & 1u) { sm[ob0 + i] = R.h13[i]; sm[ob0 + C.FS + i] = R.u13[i]; sm[ob0 + 2 * C.FS + i] = v1; }
         }
-        wk_fence_async();
     }
+    wk_fence_async();
     WKP(3)
     // E/W ghost cells and edge u^a of the NEXT row go next to its tile row (the leader read them two ticks ago)
     const int l1 = lj + 1;
@@ -230,6 +260,7 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
             wk_commit();
         }
         if (g.gys && g.gyn && t == g.gys) wf_issue_ns(C, true);               // S rows consumed (halo of row gys-1 read)
+        if (C.first && (unsigned)(lj + WK_XD) < (unsigned)g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
         if (prep && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
     }
     WKP(4)
@@ -276,7 +307,8 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
     const int lj = t - g.gys;
     const uint32_t P8 = 8u * C.P, FS8 = 8u * C.FS;
     WKP(7)
-    if (C.has_leader) wk_wait_prog(C.a_lead, C.need0 + (unsigned)t + 4u);
+    if (C.has_leader) { const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+    if (C.first) wf_wait_xrow<K>(C, lj);
     WKP(0)
     // ---- loads: own columns of row t, E/W halo and edge u^a of row t-1
     const uint32_t urow = C.sm32 + 8u * (C.st + lj * C.P);          // tile row lj, tile column 0, field 0
@@ -365,6 +397,7 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
         for (int f = 0; f < 3; ++f) { wk_s2g32(dst, src, g.ex * 8u); dst += g.ncell; src += FS8; }
         wk_commit();
         if ((l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
+        if (C.first && lj + WK_XD < g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
     }
     WKP(4)
     // ---- H (25b) at level n+1 on row t-3
@@ -403,176 +436,75 @@ template <int K>
 __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ WkArgs A)
 {
     extern __shared__ __align__(128) double sm[];
-    const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(tid >> 5);
+    const int tid = threadIdx.x, lane = tid & 31, w = wk_uni(wk_logical_warp(tid >> 5));
     const WkLayout& Ly = A.Lf;
     const uint32_t sm32 = wk_s32(sm);
-    const uint32_t b_init = sm32 + 8u * 40u;
-    int* s_next = reinterpret_cast<int*>(sm + 52);
-    double* red = sm + 64;                      // [32] block reduction scratch
-    double* wpart = sm + 96;                    // [WK_NW] observation cost of each warp's steps
-    double* tab = sm + Ly.tab;
     const int IW = Ly.wbase + w * Ly.wsz;
     if (tid == 0) {
-        for (int i = 0; i < 41; ++i) wk_mbar_init32(sm32 + 8u * i, 1);
+        for (int i = 0; i < WK_NW * WK_BAR_PER_WARP; ++i) wk_mbar_init32(sm32 + 8u * i, 1);
         wk_fence_mbar_init();
     }
-    if (tid < WK_NW) reinterpret_cast<unsigned*>(sm + 48)[tid] = 0u;
+    if (tid < WK_NW) reinterpret_cast<unsigned*>(sm + WK_PROG)[tid] = 0u;
     for (int q = tid; q < Ly.total - WK_HDR; q += WK_NT) sm[WK_HDR + q] = 0.0;      // no stale NaN patterns
-    __syncthreads();
-    unsigned par_init = 0u;
-    unsigned gbase = 1u;                        // CTA-wide step counter (progress words only grow)
+    __syncthreads();                            // the only CTA-wide barrier
     const int lw = (w + WK_NW - 1) % WK_NW;     // the warp that runs the previous step
 
     WfCtx<K> C;
     C.st = Ly.st; C.P = Ly.P; C.FS = Ly.FS;
     C.I_SN = IW + Ly.sn; C.I_EW = IW + Ly.ew; C.I_EDS = IW + Ly.eds; C.I_EDE = IW + Ly.ede;
-    C.sm32 = sm32; C.a_lead = sm32 + 8u * 48u + 4u * lw; C.a_mine = sm32 + 8u * 48u + 4u * w;
-    C.b_sn = sm32 + 8u * (w * 5); C.b_ew = sm32 + 8u * (w * 5 + 1);
+    C.sm32 = sm32; C.a_lead = sm32 + 8u * WK_PROG + 4u * lw; C.a_mine = sm32 + 8u * WK_PROG + 4u * w;
+    C.b_sn = sm32 + 8u * (w * WK_BAR_PER_WARP); C.b_ew = C.b_sn + 8u; C.b_x = C.b_sn + 32u;
     C.c0 = 2 + K * lane; C.lane = lane;
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm;
     C.A = &A; C.par = 0u;
-    const int st = Ly.st, P = Ly.P, FS = Ly.FS;
+    const int FS = Ly.FS;
 #ifdef WK_PROF
     for (int q = 0; q < 8; ++q) C.pf[q] = 0;
-    long long ph[4] = {0, 0, 0, 0}, pht = clock64();
-#define WKPH(i) { const long long c_ = clock64(); ph[i] += c_ - pht; pht = c_; }
-#else
-#define WKPH(i)
 #endif
 
-    for (;;) {
-        if (tid == 0) *s_next = atomicAdd(A.counter, 1);
-        __syncthreads();
-        const int k = wk_uni(*s_next);
-        __syncthreads();
-        if (k >= A.nsub) break;
+    // Every warp walks the same list of (subdomain, step) pairs; global step number gs (1, 2, ...) belongs
+    // to warp (gs - 1) % WK_NW, and the step gs - 1 is its leader whatever subdomain it belongs to.
+    int nord = -1;                              // ordinal of the current subdomain in this CTA's list
+    unsigned gnext = 1u, glast = 0u;            // global numbers: step 0 of the current subdomain, last step of the previous one                        // global number of step 0 of the current subdomain
+    int TL = 0, gysL = 0;                       // ticks and south ghost rows of the previous subdomain of this CTA
+    for (int k = blockIdx.x; k < A.nsub; k += gridDim.x) {
         if (A.mask && !A.mask[k]) continue;
+        ++nord;
         const Sub s = A.subs[k];
         const WkGeo g = wk_geo(s);
-        C.g = g;
-        WKPH(3)
-        // ---------------- init: control -> resident state (TMA), row tables, level 0 of the store
-        if (tid == 0) wk_mbar_expect32(b_init, 3u * g.ncell * 8u);
-        wk_load_tab(tab, A.m, g);
-        __syncthreads();
-        for (int q = tid; q < 3 * g.ey; q += WK_NT) {
-            const int f = q / g.ey, lj = q - f * g.ey;
-            wk_g2s32(sm32 + 8u * (st + f * FS + lj * P), A.x + s.coff + (long long)f * g.ncell + lj * g.ex, g.ex * 8u, b_init);
-        }
-        wk_mbar_wait32(b_init, par_init); par_init ^= 1u;
-        __syncthreads();
-        for (int q = tid; q < 3 * g.ey; q += WK_NT) {
-            const int f = q / g.ey, lj = q - f * g.ey;
-            wk_s2g32(A.traj + s.toff + (long long)f * g.ncell + lj * g.ex, sm32 + 8u * (st + f * FS + lj * P), g.ex * 8u);
-        }
-        wk_commit();
-
-        // ---------------- control-level cost terms: (25a) background, (25c) spatial overlap and
-        // predecessor window, and H (25b) at level 0; the successor term follows the sweep.
-        // Rows over warps, columns over lanes; plain sums in a fixed order.
-        double bg = 0.0, sp = 0.0, pr = 0.0, ob = 0.0;
-        {
-            // (two cells per thread and pass: all loads are issued before the first use)
-            const bool pred = s.jw > 0;
-            const double bw = s.jw == 0 ? 1.0 : A.cp.bgw;
-            for (int c0 = tid; c0 < g.ncell; c0 += 2 * WK_NT) {
-                double bv[2][3], pv[2][3], wsp[2];
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int c = c0 + u * WK_NT;
-                    const bool in = c < g.ncell;
-                    const int lj = c / g.ex, li = c - lj * g.ex;
-                    int gi = s.ei0 + li; gi = gi < 0 ? gi + A.geo.nlon : (gi >= A.geo.nlon ? gi - A.geo.nlon : gi);
-                    wsp[u] = in ? bw / (double)(A.geo.ncolcov[gi] * A.geo.nrowcov[s.ej0 + lj]) : 0.0;
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) {
-                        const long long o = s.coff + (long long)f * g.ncell + c;
-                        bv[u][f] = in ? __ldg(A.xbs + o) : 0.0;
-                        pv[u][f] = (in && pred) ? __ldg(A.pred_end + o) : 0.0;
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int c = c0 + u * WK_NT;
-                    if (c < g.ncell) {
-                        const int lj = c / g.ex, li = c - lj * g.ex;
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) {
-                            const double xv = sm[st + f * FS + lj * P + li];
-                            const double db = xv - bv[u][f];
-                            bg += wsp[u] * db * db * A.cp.ib[f];
-                            if (pred) { const double dv = xv - pv[u][f]; pr += dv * dv * A.cp.ib[f]; }
-                        }
-                    }
-                }
-            }
-            // (25c) case 1: one rectangle per (neighbour tile, periodic image) of the same window
-            for (int r = 0; r < s.nnb; ++r) {
-                const NbRect nb = A.nbr[s.nb0 + r];
-                const double* xf = A.xfrozen + nb.coff2 + (long long)nb.nj0 * nb.ex2 + nb.ni0;
-                const int ncr = nb.w * nb.h;
-                for (int e0 = tid; e0 < ncr; e0 += 2 * WK_NT) {
-                    double fv[2][3];
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int e = e0 + u * WK_NT;
-                        const int dj = e / nb.w, di = e - dj * nb.w;
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) fv[u][f] = e < ncr ? __ldg(xf + (long long)f * nb.ncell2 + dj * nb.ex2 + di) : 0.0;
-                    }
-#pragma unroll
-                    for (int u = 0; u < 2; ++u) {
-                        const int e = e0 + u * WK_NT;
-                        if (e < ncr) {
-                            const int dj = e / nb.w, di = e - dj * nb.w;
-#pragma unroll
-                            for (int f = 0; f < 3; ++f) {
-                                const double dv = sm[st + f * FS + (nb.j0 + dj) * P + nb.i0 + di] - fv[u][f];
-                                sp += dv * dv * A.cp.ib[f];
-                            }
-                        }
-                    }
-                }
-            }
-            if (A.obs_start) {
-                const long long a0 = A.obs_start[s.ooff], a1 = A.obs_start[s.ooff + 1];
-                for (long long q = a0 + tid; q < a1; q += WK_NT) {
-                    const int pk = A.obs_lj[q];
-                    const double rr = sm[st + ((pk >> 8) & 3) * FS + (pk >> 12) * P + (pk & 255)] - A.obs_y[q];
-                    const double cq = A.obs_c[q];
-                    ob += cq * rr * rr;
-                    A.obs_r[q] = 2.0 * cq * rr;
-                }
-            }
-        }
-        wk_wait_read<0>();                      // level-0 stores have left shared memory
-        bg = block_sum<WK_NT>(bg, red);
-        sp = block_sum<WK_NT>(sp, red);
-        pr = block_sum<WK_NT>(pr, red);
-        ob = block_sum<WK_NT>(ob, red);         // (ends with a __syncthreads)
-        WKPH(0)
-
-        // ---------------- per-lane column map of this tile
-        C.tmask = 0u;
-#pragma unroll
-        for (int i = 0; i < K; ++i) if ((C.c0 + i >= 3) && (C.c0 + i < 3 + g.ex)) C.tmask |= 1u << i;
-        C.injL = lane == 0; C.injR = (lane == 31) && (C.c0 + K == g.px - 2);
-        if (lane < 18) {                        // E/W ghost cell (field lane/6, cell lane%6) of a tile row
-            const int f = lane / 6, e = lane % 6;
-            C.gcp_base = C.I_EW + f * 6 * WK_EWC + e; C.gcp_ss = 18 * WK_EWC; C.gcp_rs = 6;
-            C.gcp_dst = f * FS + (e < 3 ? e - 3 : g.ex + e - 3);
-        } else {                                // lanes 18, 19: edge u^a west / east -> the row's two pad cells
-            C.gcp_base = C.I_EDE + (lane - 18); C.gcp_ss = 2 * WK_EWC; C.gcp_rs = 2;
-            C.gcp_dst = g.ex + 3 + (lane - 18);
-        }
-        C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
-        C.T = g.py + 3 - g.gyn;             // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
+        const int T = g.py + 3 - g.gyn;         // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
+        const int n0 = (int)((unsigned)(w + 1) - gnext) & (WK_NW - 1);      // my first step in this subdomain
         C.obw = 0.0;                            // this lane's share of H (25b) over this warp's steps
-
+        if (n0 < g.W) {
+            C.g = g; C.T = T;
+            // ---------------- per-lane column map of this tile
+            C.tmask = 0u;
+#pragma unroll
+            for (int i = 0; i < K; ++i) if ((C.c0 + i >= 3) && (C.c0 + i < 3 + g.ex)) C.tmask |= 1u << i;
+            C.injL = lane == 0; C.injR = (lane == 31) && (C.c0 + K == g.px - 2);
+            if (lane < 18) {                    // E/W ghost cell (field lane/6, cell lane%6) of a tile row
+                const int f = lane / 6, e = lane % 6;
+                C.gcp_base = C.I_EW + f * 6 * WK_EWC + e; C.gcp_ss = 18 * WK_EWC; C.gcp_rs = 6;
+                C.gcp_dst = f * FS + (e < 3 ? e - 3 : g.ex + e - 3);
+            } else {                            // lanes 18, 19: edge u^a west / east -> the row's two pad cells
+                C.gcp_base = C.I_EDE + (lane - 18); C.gcp_ss = 2 * WK_EWC; C.gcp_rs = 2;
+                C.gcp_dst = g.ex + 3 + (lane - 18);
+            }
+            C.nchunk = (g.ey + WK_EWC - 1) / WK_EWC;
+            C.xk = A.x + s.coff;
+            const double* tab = sm + Ly.tab + (nord % WK_NTAB) * WK_TABSZ(A.maxpy);
         // ---------------- the steps of this warp
-        for (int n = w; n < g.W; n += WK_NW) {
-            const unsigned gs = gbase + (unsigned)n;
-            C.gs10 = gs << 10; C.need0 = (gs - 1u) << 10; C.has_leader = n > 0;
+        for (int n = n0; n < g.W; n += WK_NW) {
+            const unsigned gs = gnext + (unsigned)n;
+            C.first = n == 0;
+            // the leader: the step before this one, for a first step the last step of the previous subdomain
+            const unsigned gl = C.first ? glast : gs - 1u;
+            C.gs10 = gs << 10; C.need0 = gl << 10; C.has_leader = gl != 0u;
+            C.a_lead = sm32 + 8u * WK_PROG + 4u * ((gl - 1u) & (WK_NW - 1));
+            // A first step only OVERWRITES what the previous subdomain left: tile row l is free once that
+            // subdomain's last step has stored it and the store has left shared memory (its tick l + gysL + 6).
+            C.dlead = C.first ? 7 + WK_XD + gysL - g.gys : 4;
+            C.TLd = C.first ? TL : T;
             C.gz = A.ghost + s.goff + (long long)n * 3 * g.nring;
             C.ge = A.gedge + s.eoff + (long long)n * 2 * g.py;
             C.tout = A.traj + s.toff + (long long)(n + 1) * 3 * g.ncell;
@@ -600,9 +532,16 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
 #ifdef WK_PROF
             C.pt = clock64();
 #endif
-            if (g.gys == 0) {                   // first tile row: no tick before it to prepare its ghost cells
-                if (C.has_leader) wk_wait_prog(C.a_lead, C.need0 + 4u);
-                wf_prep_row<K>(C, sm, 0);
+            if (C.first || g.gys == 0) {
+                // what tick -1 would do: the control rows that ticks 0 and 1 read, the ghost cells of tile row 0
+                if (C.has_leader) { const int nd = C.dlead - 1 < C.TLd + 1 ? C.dlead - 1 : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+                if (C.first) {
+                    wk_copy_tab(sm + Ly.tab + (nord % WK_NTAB) * WK_TABSZ(A.maxpy), A.wtab + (long long)s.b * A.wtab_stride, g.py, lane);
+                    wk_fence_async();
+                    if (wk_elect())
+                        for (int l = 0; l <= WK_XD - 1 - g.gys && l < g.ey; ++l) wf_issue_xrow<K>(C, l);
+                }
+                if (g.gys == 0) wf_prep_row<K>(C, sm, 0);
                 __syncwarp();
             }
             // steady ticks: rows t-3 .. t+1 are tile rows and no wall event falls on the tick
@@ -626,54 +565,21 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             if (wk_elect()) { wk_wait_read<0>(); wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u); }
             __syncwarp();
         }
-        WKPH(1)
-        // ---------------- reduction of the cost terms (fixed order: lanes, then warps)
+        }
+        // ---------------- H (25b) over the steps this warp ran (fixed order: lanes, then warps in ck_cost)
         double obw = C.obw;
         for (int o = 16; o > 0; o >>= 1) obw += __shfl_down_sync(0xffffffffu, obw, o);
-        if (lane == 0) wpart[w] = obw;
-        __syncthreads();
-        double su = 0.0;
-        if (s.jw < A.geo.q - 1) {               // (25c) successor window: Z^W against its frozen control
-            const double* xn = A.xfrozen + A.subs[k + A.geo.p1 * A.geo.p2].coff;
-            for (int c0 = tid; c0 < g.ncell; c0 += 4 * WK_NT) {
-                double nv[4][3];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int c = c0 + u * WK_NT;
-#pragma unroll
-                    for (int f = 0; f < 3; ++f) nv[u][f] = c < g.ncell ? __ldg(xn + (long long)f * g.ncell + c) : 0.0;
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int c = c0 + u * WK_NT;
-                    if (c < g.ncell) {
-                        const int lj = c / g.ex, li = c - lj * g.ex;
-#pragma unroll
-                        for (int f = 0; f < 3; ++f) {
-                            const double dv = sm[st + f * FS + lj * P + li] - nv[u][f];
-                            su += dv * dv * A.cp.ib[f];
-                        }
-                    }
-                }
-            }
-        }
-        su = block_sum<WK_NT>(su, red);
-        if (tid == 0) {
-            double obt = ob;
-            for (int q = 0; q < WK_NW; ++q) obt += wpart[q];
-            const double v[5] = { bg, obt, A.cp.mu * sp, A.cp.mu * pr, A.cp.mu * su };
-            double tot = 0.0;
-            for (int q = 0; q < 5; ++q) { A.parts[k * 5 + q] = v[q]; tot += v[q]; }
-            A.J[k] = tot;
-        }
-        gbase += (unsigned)g.W + 1u;
-        WKPH(2)
+        if (lane == 0) A.obpart[(long long)k * WK_NW + w] = obw;
+        // (one step number is skipped when the window length is a multiple of the warp count, so that the
+        //  levels that carry observations do not always fall on the same warp)
+        glast = gnext + (unsigned)g.W - 1u;
+        gnext = glast + 1u + ((g.W & (WK_NW - 1)) == 0 ? 1u : 0u);
+        TL = T; gysL = g.gys;
     }
 #ifdef WK_PROF
     if (lane == 0 && A.gw) {
         unsigned long long* pr = reinterpret_cast<unsigned long long*>(A.gw);
         for (int q = 0; q < 8; ++q) atomicAdd(pr + w * 16 + q, (unsigned long long)C.pf[q]);
-        for (int q = 0; q < 4; ++q) atomicAdd(pr + w * 16 + 8 + q, (unsigned long long)ph[q]);
     }
 #endif
 }

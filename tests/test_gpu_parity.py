@@ -31,7 +31,7 @@ LAYOUTS = {
     "wave_px76": dict(nlon=132, nlat=27, dt=300.0, nsteps=19, p_lon=2, p_lat=3, q_time=2, overlap=2,
                       obs_frac=0.3, obs_every=1),
     # K = 2 (px = 38), many short windows
-    "wave_k2": dict(nlon=56, nlat=20, nsteps=12, p_lon=2, p_lat=2, q_time=4, overlap=2),
+    "wave_k2": dict(nlon=56, nlat=20, nsteps=17, p_lon=2, p_lat=2, q_time=4, overlap=2),
 }
 PATHS = [1, 2, 3, 4, 5]
 
