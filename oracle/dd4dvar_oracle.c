@@ -1050,7 +1050,9 @@ static void gather_analysis(const DD* d, double* out)
 }
 /* O9: Algorithm 1 l.443-472, additive (Jacobi) outer iteration (R16), exactly outer_iters
  * iterations (R17).  history[(outer_iters+1)][3] = J(gathered analysis), sum_ji J_ji, delta_l. */
-int orc_run(void* h, int outer_iters, double* analysis, double* history)
+static double gn_run(const DD* d, int k, int n_gn, int n_cg, double* w, double* x, double* gx, double* traj,
+                     double* J0);
+static int run_impl(void* h, int outer_iters, double* analysis, double* history, int gn, int n_gn, int n_cg)
 {
     DD* d = h; if (!d->have_bg) return -3;
     size_t n3 = (size_t)NF * d->m.nlon * d->m.nlat;
@@ -1078,7 +1080,8 @@ int orc_run(void* h, int outer_iters, double* analysis, double* history)
             if (d->w_prev[k]) memcpy(d->w_cur[k], d->w_prev[k], sizeof(double) * n);
             else memset(d->w_cur[k], 0, sizeof(double) * n);
             LocCtx c = { d, k, malloc(sizeof(double) * n), malloc(sizeof(double) * n), d->traj_cur[k] };
-            Jlast[k] = lbfgs_run(n, d->lbfgs_m, d->n_inner, d->max_bt, d->c1, local_fn, &c, d->w_cur[k], &Jfirst[k]);
+            if (gn) Jlast[k] = gn_run(d, k, n_gn, n_cg, d->w_cur[k], c.x, c.gx, d->traj_cur[k], &Jfirst[k]);
+            else Jlast[k] = lbfgs_run(n, d->lbfgs_m, d->n_inner, d->max_bt, d->c1, local_fn, &c, d->w_cur[k], &Jfirst[k]);
             /* one more forward sweep so that the stored trajectory belongs to the accepted iterate */
             CostParts cp;
             w_to_x(d, k, d->w_cur[k], d->x_cur[k]);
@@ -1103,6 +1106,182 @@ int orc_run(void* h, int outer_iters, double* analysis, double* history)
     gather_analysis(d, xa);
     memcpy(analysis, xa, sizeof(double) * n3);
     free(Jfirst); free(Jlast); free(dmax); free(xa);
+    return 0;
+}
+int orc_run(void* h, int outer_iters, double* analysis, double* history)
+{
+    return run_impl(h, outer_iters, analysis, history, 0, 0, 0);
+}
+
+/* ------------------------------------------------------------------ O11: Gauss-Newton ------
+ * The paper's own local minimiser: incremental Gauss-Newton, Algorithm 5 l.568-589 and
+ * Algorithm 6 l.655-685.  J_ji = |F_ji|^2 with F_ji the stacked residuals of eq (25) l.338-344 (R5: no 1/2);
+ * one Gauss-Newton iteration linearises the model about the current trajectory (TLM, Alg 6 l.14-16) and solves
+ * the normal equations (42)-(43) l.620-626
+ *        (grad F^T grad F) dw = - grad F^T F             <=>   H_GN dw = - grad J,   H_GN = 2 grad F^T grad F
+ * in the variable w = V^+ (u - u^b), V = diag(sigma_b) (eq (44)-(46) l.630-649: the "B-preconditioned" system
+ * I + (G V)^T R^-1 G V of Algorithm 7 l.688-696; here with the weights and the overlap terms of eq (25)),
+ * by n_cg iterations of conjugate gradients from dw = 0 (READING, R21: Algorithm 7 names the Lanczos
+ * form of [24]; CG builds the same Krylov iterates; the iteration count is fixed, no residual test), then
+ * u <- u + V dw (Alg 5 l.8: full step, no line search).
+ *
+ * H_GN p for p in w-space: dx = V p; TLM sweep dZ^{n+1} = M_n dZ^n over the window (ghost ring frozen: zero
+ * perturbation); adjoint sweep (ADJ, Alg 6 l.17-19) of the weighted TLM misfits; control-level terms. */
+static void local_gn_hessvec(const DD* d, int k, const double* traj, const double* p, double* out)
+{
+    const Sub* s = &d->sub[k];
+    const int nlon = d->m.nlon, W = s->e - s->s;
+    const long nc = s->ncell;
+    Region r;
+    size_t np = (size_t)(s->ex + 2 * s->gx) * (s->ey + s->gys + s->gyn);
+    double* Zp = malloc(sizeof(double) * NF * np);
+    double* Za = calloc(NF * np, sizeof(double));
+    double* Z1 = calloc(NF * np, sizeof(double));
+    double* dZp = malloc(sizeof(double) * NF * np);
+    double* dZa = calloc(NF * np, sizeof(double));
+    double* dZ1 = calloc(NF * np, sizeof(double));
+    double* dtr = malloc(sizeof(double) * NF * nc * (W + 1));          /* TLM trajectory */
+    for (int fl = 0; fl < NF; ++fl)
+        for (long c = 0; c < nc; ++c) dtr[(size_t)fl * nc + c] = d->sig_b[fl] * p[(size_t)fl * nc + c];
+    for (int n = 0; n < W; ++n) {
+        fill_padded(d, k, s->s + n, traj + (size_t)n * NF * nc, Zp, &r);
+        region_forward(&d->m, &r, Zp, Za, Z1);
+        interior_to_padded(s, &r, dtr + (size_t)n * NF * nc, dZp);      /* frozen ghost ring: dZ = 0 */
+        memset(dZa, 0, sizeof(double) * NF * np); memset(dZ1, 0, sizeof(double) * NF * np);
+        region_tlm(&d->m, &r, Zp, Za, Z1, dZp, dZa, dZ1);
+        padded_to_interior(s, &r, dZ1, dtr + (size_t)(n + 1) * NF * nc);
+    }
+    double* lam = calloc(NF * nc, sizeof(double));
+    double* L1 = malloc(sizeof(double) * NF * np);
+    double* L0 = malloc(sizeof(double) * NF * np);
+    double* A = malloc(sizeof(double) * NF * np);
+    double* HB = malloc(sizeof(double) * np);
+    double* UB = malloc(sizeof(double) * np);
+    if (s->jw < d->q - 1)                                 /* (25c) successor window: 2 mu dZ^W / sigma_b^2 */
+        for (int fl = 0; fl < NF; ++fl) {
+            double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
+            for (long c = 0; c < nc; ++c)
+                lam[(size_t)fl * nc + c] += 2.0 * d->mu * dtr[((size_t)W * NF + fl) * nc + c] * ib;
+        }
+    for (int n = W; n >= 0; --n) {
+        int level = s->s + n;
+        if (d->have_obs)
+            for (long q = 0; q < d->nlocobs[k]; ++q) {    /* (25b): 2 lambda w H^T R^-1 H dZ^n */
+                const LocObs* ob = &d->locobs[k][q];
+                if (d->olev[ob->tidx] != level) continue;
+                int lj = (int)(ob->cell / s->ex), li = (int)(ob->cell % s->ex);
+                int gi = imod(s->ei0 + li, nlon), gj = s->ej0 + lj;
+                double wt = w_space(d, gi, gj) / (double)mult_time(d, level);
+                double dz = dtr[((size_t)n * NF + ob->fld) * nc + ob->cell];
+                lam[(size_t)ob->fld * nc + ob->cell] +=
+                    2.0 * d->lambda * wt * dz / (d->sig_o[ob->fld] * d->sig_o[ob->fld]);
+            }
+        if (n > 0) {
+            fill_padded(d, k, level - 1, traj + (size_t)(n - 1) * NF * nc, Zp, &r);
+            region_forward(&d->m, &r, Zp, Za, Z1);
+            interior_to_padded(s, &r, lam, L1);
+            region_adjoint(&d->m, &r, Zp, Za, Z1, L1, A, HB, UB, L0);
+            padded_to_interior(s, &r, L0, lam);
+        }
+    }
+    for (int fl = 0; fl < NF; ++fl) {
+        double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
+        for (int lj = 0; lj < s->ey; ++lj)
+            for (int li = 0; li < s->ex; ++li) {
+                int gi = imod(s->ei0 + li, nlon), gj = s->ej0 + lj;
+                long c = (long)lj * s->ex + li;
+                double dx = dtr[(size_t)fl * nc + c];
+                double gsum = lam[(size_t)fl * nc + c];
+                gsum += 2.0 * (s->jw == 0 ? 1.0 : d->bgw) * w_space(d, gi, gj) * dx * ib;       /* (25a) */
+                for (int cb = 0; cb < d->nrowcov[gj]; ++cb)                                     /* (25c) case 1 */
+                    for (int ca = 0; ca < d->ncolcov[gi]; ++ca) {
+                        int a2 = d->colcov[4 * gi + ca], b2 = d->rowcov[4 * gj + cb];
+                        if (a2 == s->a && b2 == s->b) continue;
+                        gsum += 2.0 * d->mu * dx * ib;
+                    }
+                if (s->jw > 0) gsum += 2.0 * d->mu * dx * ib;                                   /* predecessor */
+                out[(size_t)fl * nc + c] = d->sig_b[fl] * gsum;
+            }
+    }
+    free(Zp); free(Za); free(Z1); free(dZp); free(dZa); free(dZ1); free(dtr);
+    free(lam); free(L1); free(L0); free(A); free(HB); free(UB);
+}
+
+/* n_gn Gauss-Newton iterations on J_ji from w (updated in place); returns J_ji at the final w (one more
+ * forward sweep, which also leaves the final trajectory in traj); *J0 = J_ji at the initial w. */
+static double gn_run(const DD* d, int k, int n_gn, int n_cg, double* w, double* x, double* gx, double* traj,
+                     double* J0)
+{
+    const Sub* s = &d->sub[k];
+    const long n = NF * s->ncell;
+    double* g = malloc(sizeof(double) * n); double* dw = malloc(sizeof(double) * n);
+    double* rv = malloc(sizeof(double) * n); double* pv = malloc(sizeof(double) * n);
+    double* Hp = malloc(sizeof(double) * n);
+    CostParts cp;
+    for (int it = 0; it < n_gn; ++it) {
+        w_to_x(d, k, w, x);
+        local_eval(d, k, x, &cp, gx, traj);
+        if (it == 0 && J0) *J0 = cp.total;
+        for (int fl = 0; fl < NF; ++fl)
+            for (long q = 0; q < s->ncell; ++q) g[fl * s->ncell + q] = d->sig_b[fl] * gx[fl * s->ncell + q];
+        for (long q = 0; q < n; ++q) { dw[q] = 0.0; rv[q] = -g[q]; pv[q] = rv[q]; }
+        double rr = (double)ldot(rv, rv, n);
+        for (int c = 0; c < n_cg && rr > 0.0; ++c) {
+            local_gn_hessvec(d, k, traj, pv, Hp);
+            double pHp = (double)ldot(pv, Hp, n);
+            if (!(pHp > 0.0)) break;
+            double al = rr / pHp;
+            for (long q = 0; q < n; ++q) { dw[q] += al * pv[q]; rv[q] -= al * Hp[q]; }
+            double rr2 = (double)ldot(rv, rv, n), be = rr2 / rr;
+            for (long q = 0; q < n; ++q) pv[q] = rv[q] + be * pv[q];
+            rr = rr2;
+        }
+        for (long q = 0; q < n; ++q) w[q] += dw[q];
+    }
+    w_to_x(d, k, w, x);
+    local_eval(d, k, x, &cp, NULL, traj);
+    if (n_gn == 0 && J0) *J0 = cp.total;
+    free(g); free(dw); free(rv); free(pv); free(Hp);
+    return cp.total;
+}
+/* Algorithm 1 with the Gauss-Newton local solver; same history layout as orc_run */
+int orc_run_gn(void* h, int outer_iters, int n_gn, int n_cg, double* analysis, double* history)
+{
+    if (n_gn < 0 || n_cg < 0) return -1;
+    return run_impl(h, outer_iters, analysis, history, 1, n_gn, n_cg);
+}
+/* test hook: H_GN p of subdomain k about the control x (p, out in w-space, [3][ncell]) */
+int orc_gn_hessvec(void* h, int k, const double* x, const double* p, double* out)
+{
+    DD* d = h; if (!d->have_bg) return -3;
+    if (k < 0 || k >= d->nsub) return -1;
+    const Sub* s = &d->sub[k];
+    CostParts cp;
+    double* traj = malloc(sizeof(double) * NF * s->ncell * (s->e - s->s + 1));
+    local_eval(d, k, x, &cp, NULL, traj);
+    local_gn_hessvec(d, k, traj, p, out);
+    free(traj);
+    return 0;
+}
+/* test hook: n_gn Gauss-Newton iterations on subdomain k from the control x (in / out), n_cg CG iterations each */
+int orc_gn_local(void* h, int k, int n_gn, int n_cg, double* x, double* J_first_last)
+{
+    DD* d = h; if (!d->have_bg) return -3;
+    if (k < 0 || k >= d->nsub) return -1;
+    const Sub* s = &d->sub[k]; const long n = NF * s->ncell;
+    const double* ubs = ub_level(d, s->s);
+    double* w = malloc(sizeof(double) * n); double* xx = malloc(sizeof(double) * n); double* gx = malloc(sizeof(double) * n);
+    double* traj = malloc(sizeof(double) * n * (s->e - s->s + 1));
+    for (int fl = 0; fl < NF; ++fl)
+        for (int lj = 0; lj < s->ey; ++lj)
+            for (int li = 0; li < s->ex; ++li) {
+                int gi = imod(s->ei0 + li, d->m.nlon), gj = s->ej0 + lj;
+                size_t c = (size_t)fl * s->ncell + (size_t)lj * s->ex + li;
+                w[c] = (x[c] - ubs[gidx(d, fl, gj, gi)]) / d->sig_b[fl];
+            }
+    J_first_last[1] = gn_run(d, k, n_gn, n_cg, w, xx, gx, traj, &J_first_last[0]);
+    memcpy(x, xx, sizeof(double) * n);
+    free(w); free(xx); free(gx); free(traj);
     return 0;
 }
 

@@ -45,6 +45,9 @@ def _load():
     lib.orc_get_trajectory.argtypes = [C.c_void_p, C.c_int, dp]
     lib.orc_run.argtypes = [C.c_void_p, C.c_int, dp, dp]
     lib.orc_global_4dvar.argtypes = [C.c_void_p, C.c_int, dp, dp]
+    lib.orc_run_gn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp, dp]
+    lib.orc_gn_hessvec.argtypes = [C.c_void_p, C.c_int, dp, dp, dp]
+    lib.orc_gn_local.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp, dp]
     lib.orc_lbfgs.restype = C.c_double
     lib.orc_lbfgs.argtypes = [C.c_long, C.c_int, C.c_int, C.c_int, C.c_double, _EVALFN, C.c_void_p, dp]
     lib.orc_sweep_range.restype = C.c_double
@@ -214,6 +217,31 @@ class Oracle:
         if rc:
             raise RuntimeError(f"orc_run -> {rc}")
         return an, hist
+
+    def run_gn(self, outer_iters, n_gn=2, n_cg=5):
+        """Algorithm 1 with the paper's own local minimiser: incremental Gauss-Newton (Alg 5-6),
+        normal equations solved by n_cg CG iterations in w-space (eq (42)-(46))."""
+        an = np.empty(self.shape); hist = np.zeros((outer_iters + 1, 3))
+        rc = self.lib.orc_run_gn(self._h, outer_iters, n_gn, n_cg, _dp(an), _dp(hist))
+        if rc:
+            raise RuntimeError(f"orc_run_gn -> {rc}")
+        return an, hist
+
+    def gn_hessvec(self, k, x, p):
+        """H_GN p of subdomain k about the control x (p and the result in w-space)."""
+        x = _c(x); p = _c(p); out = np.empty_like(p)
+        rc = self.lib.orc_gn_hessvec(self._h, k, _dp(x), _dp(p), _dp(out))
+        if rc:
+            raise RuntimeError(f"orc_gn_hessvec -> {rc}")
+        return out
+
+    def gn_local(self, k, x, n_gn, n_cg):
+        """n_gn Gauss-Newton iterations on subdomain k from the control x; returns (x_new, J_first, J_last)."""
+        x = np.array(_c(x), copy=True); jj = np.zeros(2)
+        rc = self.lib.orc_gn_local(self._h, k, n_gn, n_cg, _dp(x), _dp(jj))
+        if rc:
+            raise RuntimeError(f"orc_gn_local -> {rc}")
+        return x, jj[0], jj[1]
 
     def global_4dvar(self, rounds):
         an = np.empty(self.shape); hist = np.zeros(rounds + 1)

@@ -18,7 +18,7 @@
 
 #define CK_NT 256
 
-__global__ void __launch_bounds__(CK_NT) ck_cost(const WkArgs A)
+__global__ void __launch_bounds__(CK_NT, 5) ck_cost(const WkArgs A)
 {
     __shared__ double red[32];
     const int k = blockIdx.x, tid = threadIdx.x;
