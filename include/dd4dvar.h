@@ -128,6 +128,20 @@ int dd4dvar_set_observations(dd4dvar_t h, int n_times, const int* h_levels,
  * delta_l = max_ji ||u_ji^l - u_ji^(l-1)||_inf (l.466; row 0: 0). */
 int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_history);
 
+/* Algorithm 1 with the paper's own local minimiser (Algorithms 5-7, l.568-696): n_gn incremental Gauss-Newton
+ * iterations per outer iteration; each linearises the model about the current local trajectory (TLM, Alg 6
+ * l.14-16) and solves the normal equations (42)-(43) l.620-626 in w = V^+ (u - u^b), V = diag(sigma_b)
+ * (eq (44)-(46) l.630-649, "B-preconditioned") by exactly n_cg conjugate-gradient iterations from dw = 0, then
+ * takes the full step (Alg 5 l.8).  One CG iteration = one tangent-linear sweep + one adjoint sweep (ADJ, Alg 6
+ * l.17-19) on every subdomain.  Arguments and history as dd4dvar_run.  Needs a layout the wavefront kernels
+ * serve (dd4dvar_active_path == 5), else -2. */
+int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_analysis, double* h_history);
+
+/* Test hook: the Gauss-Newton operator H_GN = 2 grad F^T grad F of every J_ji (F = stacked residuals of eq (25)
+ * l.338-344) about the given controls, applied to d_p; d_controls, d_p, d_out in the "all subdomains" control
+ * layout, d_p and d_out in w-space.  Runs a forward sweep at d_controls first (uses the current frozen data). */
+int dd4dvar_gn_hessvec(dd4dvar_t h, const double* d_controls, const double* d_p, double* d_out);
+
 /* eq (6) l.111 and its gradient by one forward + one adjoint sweep over the whole grid.
  * d_x0 [3][nlat][nlon]; h_cost[1]; d_grad [3][nlat][nlon] or NULL. */
 int dd4dvar_eval_global(dd4dvar_t h, const double* d_x0, double* h_cost, double* d_grad);

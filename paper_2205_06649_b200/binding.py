@@ -51,7 +51,7 @@ EXPORTS = [
     "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
-    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight",
+    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec",
     "dd4dvar_last_error", "dd4dvar_destroy",
 ]
 
@@ -76,6 +76,8 @@ def load_library():
     lib.dd4dvar_obs_workspace_bytes.argtypes = [vp, C.c_longlong]
     lib.dd4dvar_set_observations.argtypes = [vp, C.c_int, ip, C.POINTER(C.c_longlong), dp, dp, hd, dp, C.c_size_t]
     lib.dd4dvar_run.argtypes = [vp, C.c_int, dp, hd]
+    lib.dd4dvar_run_gn.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, hd]
+    lib.dd4dvar_gn_hessvec.argtypes = [vp, dp, dp, dp]
     lib.dd4dvar_eval_global.argtypes = [vp, dp, hd, dp]
     lib.dd4dvar_eval_local.argtypes = [vp, dp, hd, hd, dp]
     lib.dd4dvar_eval_local_host.argtypes = [vp, C.c_void_p, hd, C.c_void_p]
@@ -291,6 +293,24 @@ class DD4DVar:
         hist = np.zeros((outer_iters + 1, 3))
         self._check("dd4dvar_run", self.lib.dd4dvar_run(self._h, outer_iters, an.data_ptr(), _hd(hist)))
         return an, hist
+
+    def run_gn(self, outer_iters, n_gn=2, n_cg=5):
+        """Algorithm 1 with the Gauss-Newton + CG local minimiser (Alg 5-7)."""
+        torch = self.torch
+        an = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        hist = np.zeros((outer_iters + 1, 3))
+        self._check("dd4dvar_run_gn", self.lib.dd4dvar_run_gn(self._h, outer_iters, int(n_gn), int(n_cg),
+                                                              an.data_ptr(), _hd(hist)))
+        return an, hist
+
+    def gn_hessvec(self, controls, p):
+        """H_GN p of every subdomain about `controls` (flat control layout; p and the result in w-space)."""
+        torch = self.torch
+        controls = self._dev(controls); p = self._dev(p)
+        out = torch.empty(self.ctot, dtype=torch.float64, device=self.device)
+        self._check("dd4dvar_gn_hessvec", self.lib.dd4dvar_gn_hessvec(self._h, controls.data_ptr(), p.data_ptr(),
+                                                                      out.data_ptr()))
+        return out
 
     def get_controls(self):
         torch = self.torch

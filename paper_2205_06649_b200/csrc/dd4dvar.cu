@@ -22,6 +22,7 @@
 #include "wave_forward.cuh"
 #include "wave_adjoint.cuh"
 #include "cost_kernels.cuh"
+#include "gn_kernels.cuh"
 
 namespace {
 
@@ -84,6 +85,8 @@ struct Layout {
     int* obs_idx = nullptr;
     int* obs_lj = nullptr;
     double *obs_y = nullptr, *obs_c = nullptr, *obs_r = nullptr;
+    double* obs_rt = nullptr;           // Gauss-Newton: forcing 2 c H dZ of the tangent-linear sweep
+    double *gn_lamW = nullptr, *gn_gx = nullptr, *gn_Hp = nullptr;     // Gauss-Newton: [ctot] each (wavefront layouts)
     FusedPlan fp{};
     WavePlan wp{};
 };
@@ -284,6 +287,7 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
         L.wp.wtab = ar.take<double>((size_t)L.p2 * L.wp.wtab_stride);
         L.wp.lamW = ar.take<double>(L.ctot);
         L.wp.obpart = ar.take<double>((size_t)L.nsub * WK_NW);
+        if (L.lbfgs) { L.gn_lamW = ar.take<double>(L.ctot); L.gn_gx = ar.take<double>(L.ctot); L.gn_Hp = ar.take<double>(L.ctot); }
     }
 }
 
@@ -635,6 +639,9 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
     if (cudaFuncSetAttribute(sk_adjoint_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(sizeof(double) * SK_ADJ_SMEM_DOUBLES)) != cudaSuccess)
         return fail(h, -4, "shared-memory opt-in of sk_adjoint_step failed");
+    if (cudaFuncSetAttribute(tk_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(sizeof(double) * TK_SMEM_DOUBLES)) != cudaSuccess)
+        return fail(h, -4, "shared-memory opt-in of tk_step failed");
     if (h->L.wp.enabled) {
         int dev = 0, nsm = 0;
         CU(cudaGetDevice(&dev));
@@ -704,7 +711,7 @@ int dd4dvar_set_background(dd4dvar_t h, const double* d_xb, const double h_sigma
 size_t dd4dvar_obs_workspace_bytes(dd4dvar_t h, long long n_obs_total)
 {
     if (!h || n_obs_total < 0) return 0;
-    const size_t per = 4 + 4 + 8 + 8 + 8;
+    const size_t per = 4 + 4 + 8 + 8 + 8 + 8;
     size_t nb = (size_t)n_obs_total * (1 + 2 * (size_t)h->L.maxcov);
     return nb * per + (size_t)(h->G.otot + h->L.otot + 8) * 8 + 4096;
 }
@@ -781,9 +788,11 @@ static int bin_observations(dd4dvar_t h, Layout& L, int n_times, const int* leve
     L.obs_start = ar.take<long long>(L.otot + 1);
     L.obs_idx = ar.take<int>(nb + 1); L.obs_lj = ar.take<int>(nb + 1);
     L.obs_y = ar.take<double>(nb + 1); L.obs_c = ar.take<double>(nb + 1); L.obs_r = ar.take<double>(nb + 1);
+    L.obs_rt = ar.take<double>(nb + 1);
     if (ar.off > ar.cap) return fail(h, -1, "set_observations: observation workspace too small");
     CU(cudaMemcpyAsync(L.obs_lj, ol.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemsetAsync(L.obs_r, 0, sizeof(double) * (nb + 1), h->stream));
+    CU(cudaMemsetAsync(L.obs_rt, 0, sizeof(double) * (nb + 1), h->stream));
     CU(cudaMemcpyAsync(L.obs_start, start.data(), sizeof(long long) * (L.otot + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(L.obs_idx, oi.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(L.obs_y, oy.data(), sizeof(double) * (nb + 1), cudaMemcpyHostToDevice, h->stream));
@@ -1004,6 +1013,112 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         h_history[3 * l + 2] = dl;
         if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
         if (!isfinite(h_history[3 * l]) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run: non-finite cost");
+    }
+    LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
+    return sync_check(h);
+}
+
+// ---- Gauss-Newton local minimiser (gn_kernels.cuh): wavefront layouts only ------------------
+namespace {
+// Hp (w-space) = H_GN pw about the trajectory the last forward sweep stored
+int gn_apply(dd4dvar_t h, Layout& L, const double* pw, double* Hp)
+{
+    const dim3 pgrid((L.maxnpad + 255) / 256, L.nsub);
+    LAUNCH(tk_init, pgrid, 256, L.dsubs, h->cp, pw, L.Zp, L.Za);
+    double* din = L.Zp; double* dout = L.Za;
+    const size_t smem = sizeof(double) * TK_SMEM_DOUBLES;
+    for (int n = 0; n < L.Wmax; ++n) {
+        tk_step<<<dim3(L.ntiles, L.nsub), SK_NT, smem, h->stream>>>(L.dsubs, n, h->mp, L.traj, L.ghost, din, dout, L.tiles_x);
+        ++h->launches;
+        if (L.have_obs)
+            LAUNCH(tk_obs, dim3(2, L.nsub), 128, L.dsubs, n + 1, L.obs_start, L.obs_lj, L.obs_c, dout, L.obs_rt);
+        std::swap(din, dout);
+    }
+    LAUNCH(ck_gn, L.nsub, 256, L.dsubs, L.dnb, L.geo, h->cp, pw, L.Zp, L.Za, L.have_obs ? L.obs_start : nullptr,
+           L.obs_lj, L.obs_c, L.obs_rt, L.gn_gx, L.gn_lamW);
+    WkArgs a = wave_args(h, L, nullptr, nullptr, nullptr);
+    a.obs_r = L.obs_rt; a.lamW = L.gn_lamW; a.gx = L.gn_gx;
+    if (L.wp.K == 2) wk_adjoint<2><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
+    else wk_adjoint<3><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
+    ++h->launches;
+    LAUNCH(ck_scale_grad, dim3(std::min(32, (3 * L.maxncell + 255) / 256), L.nsub), 256, L.dsubs, (const int*)nullptr,
+           h->cp, L.gn_gx, Hp);
+    return 0;
+}
+}  // namespace
+
+int dd4dvar_gn_hessvec(dd4dvar_t h, const double* d_controls, const double* d_p, double* d_out)
+{
+    if (!h || !d_controls || !d_p || !d_out) return fail(h, -1, "gn_hessvec: null argument");
+    if (!h->have_bg) return fail(h, -3, "gn_hessvec before set_background");
+    Layout& L = h->L;
+    if (L.path != 5) return fail(h, -2, "gn_hessvec: the Gauss-Newton solver needs a wavefront layout (path 5)");
+    CU(cudaMemcpyAsync(L.x, d_controls, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
+    sweep(h, L, false, nullptr, L.Jev, nullptr);
+    int rc = gn_apply(h, L, d_p, L.gn_Hp);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(d_out, L.gn_Hp, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
+    return sync_check(h);
+}
+
+// Algorithm 1 l.443-472 with the local minimiser of Algorithms 5-7 (Gauss-Newton + CG in w-space)
+int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_analysis, double* h_history)
+{
+    if (!h || outer_iters < 0 || n_gn < 0 || n_cg < 0 || !d_analysis || !h_history) return fail(h, -1, "run_gn: bad argument");
+    if (!h->have_bg) return fail(h, -3, "run_gn before set_background");
+    Layout& L = h->L; Layout& G = h->G;
+    if (L.path != 5) return fail(h, -2, "run_gn: the Gauss-Newton solver needs a wavefront layout (path 5)");
+    const int n1 = h->grid.nlon * h->grid.nlat;
+    const int nsub = L.nsub;
+    h->h_tmp.resize(std::max(nsub, 8));
+    int rc;
+    auto sumJ = [&](const double* dJ, double* out) -> int {
+        CU(cudaMemcpyAsync(h->h_tmp.data(), dJ, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
+        int r = sync_check(h); if (r) return r;
+        long double sacc = 0; for (int k = 0; k < nsub; ++k) sacc += h->h_tmp[k];
+        *out = (double)sacc; return 0;
+    };
+    auto gather_and_cost = [&](double* out) -> int {
+        LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, G.x);
+        return global_cost(h, out);
+    };
+    const dim3 vgrid(std::min(64, (3 * L.maxncell + 255) / 256), nsub);
+    auto controls_from_w = [&]() {
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+               (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+    };
+    if ((rc = gather_and_cost(&h_history[0]))) return rc;
+    h_history[1] = 0.0; h_history[2] = 0.0;
+    if (outer_iters == 0) {
+        controls_from_w();
+        sweep(h, L, false, nullptr, L.st.J, nullptr);
+        if ((rc = sumJ(L.st.J, &h_history[1]))) return rc;
+    }
+    double* dw = L.d; double* rv = L.wt; double* pv = L.gn;
+    for (int l = 1; l <= outer_iters; ++l) {
+        for (int it = 0; it < n_gn; ++it) {
+            controls_from_w();
+            sweep(h, L, true, nullptr, L.st.J, L.g);                   // J_ji, g = sigma_b grad_x J_ji, trajectory
+            if (l == 1 && it == 0 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
+            LAUNCH(gn_cg_init, nsub, GN_NT, L.dsubs, L.g, dw, rv, pv, L.st.t, L.st.trial);
+            for (int c = 0; c < n_cg; ++c) {
+                if ((rc = gn_apply(h, L, pv, L.gn_Hp))) return rc;
+                LAUNCH(gn_cg_update, nsub, GN_NT, L.dsubs, L.gn_Hp, dw, rv, pv, L.st.t, L.st.trial);
+            }
+            LAUNCH(gn_add, vgrid, 256, L.dsubs, L.w, dw);
+        }
+        // forward sweep at the final iterate: its trajectory is what the neighbours see next
+        controls_from_w();
+        sweep(h, L, false, nullptr, L.st.J, nullptr);
+        if (l == 1 && n_gn == 0 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
+        if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
+        exchange(h, L);
+        CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
+        if ((rc = sync_check(h))) return rc;
+        double dl = 0; for (int k = 0; k < nsub; ++k) dl = std::max(dl, h->h_tmp[k]);
+        h_history[3 * l + 2] = dl;
+        if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
+        if (!isfinite(h_history[3 * l]) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run_gn: non-finite cost");
     }
     LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
     return sync_check(h);
