@@ -138,7 +138,7 @@ def measured_traffic(kernel, cfg):
 
 PATH_NAMES = {1: "generic (block-tiled step kernels)", 2: "row-marching fused kernels", 3: "per-stage generic kernels",
               4: "wavefront forward (wk_forward) + row-marching adjoint (fk_adjoint2)",
-              5: "wavefront forward (wk_forward) + wavefront adjoint (wk_adjoint)"}
+              5: "wavefront forward (wk_forward) + control-level terms (ck_cost) + wavefront adjoint (wk_adjoint)"}
 
 
 def max_over_ranks(values, device=None):
@@ -257,8 +257,19 @@ def run_driver(args):
     prob = synth.make_problem(w, g.forecast)
     g.set_background(prob.xb, prob.sigma_b); g.set_observations(prob.obs)
     outer = args.outer if args.outer is not None else w.outer_iters
+    extra = {}
+    if args.gn:
+        # the paper's own local minimiser (Alg 5-7): Gauss-Newton + CG; one CG iteration = TLM sweep + adjoint sweep
+        xs = g.get_controls(); pw = torch.ones_like(xs)
+        g.gn_hessvec(xs, pw); torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record(); g.sweep_async(0); ev[1].record(); g.gn_hessvec(xs, pw); ev[2].record(); torch.cuda.synchronize()
+        fwd_ms = ev[0].elapsed_time(ev[1]); hv_ms = ev[1].elapsed_time(ev[2]) - fwd_ms
+        extra = {"local_solver": f"Gauss-Newton n_gn={args.n_gn} n_cg={args.n_cg}", "forward_sweep_ms": fwd_ms,
+                 "hessvec_ms": hv_ms, "hessvec": "one product with H_GN on every subdomain = TLM sweep (tk_step, one launch "
+                 "per step) + ck_gn + adjoint sweep (wk_adjoint); gn_hessvec call minus its forward sweep"}
     torch.cuda.synchronize(); t0 = time.perf_counter()
-    an, hist = g.run(outer)
+    an, hist = g.run_gn(outer, args.n_gn, args.n_cg) if args.gn else g.run(outer)
     torch.cuda.synchronize(); dt = time.perf_counter() - t0
     an = an.cpu().numpy()
     rm = lambda a, b: float(np.sqrt(np.mean((a - b) ** 2)))
@@ -266,7 +277,7 @@ def run_driver(args):
                       "launches": int(g.launch_count), "J_global": [float(x) for x in hist[:, 0]],
                       "sumJ_local": [float(x) for x in hist[:, 1]], "delta": [float(x) for x in hist[:, 2]],
                       "rmse_background_h_u_v": [rm(prob.xb[f], prob.truth0[f]) for f in range(3)],
-                      "rmse_analysis_h_u_v": [rm(an[f], prob.truth0[f]) for f in range(3)]}))
+                      "rmse_analysis_h_u_v": [rm(an[f], prob.truth0[f]) for f in range(3)], **extra}))
     g.close()
 
 
@@ -322,6 +333,9 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 row-marching, 3 per-stage, 4 wavefront fwd + row-marching adj, 5 wavefront")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
+    ap.add_argument("--gn", action="store_true", help="with --run: Gauss-Newton + CG local minimiser (dd4dvar_run_gn)")
+    ap.add_argument("--n-gn", type=int, default=2)
+    ap.add_argument("--n-cg", type=int, default=5)
     ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     ap.add_argument("--peaks", action="store_true", help="run the library's fp64 / shared-memory / shuffle microbenchmarks")
@@ -476,7 +490,7 @@ def main():
                          "forward_kernel": {"name": fname, "algorithmic_bytes_per_launch": fwd_b,
                                             "achieved": fwd_b / (t_f * 1e-3) / 1e9, "frac": fwd_b / (t_f * 1e-3) / 1e9 / peak,
                                             "traffic": measured_traffic(fname, args.config) if fused else None,
-                                            "note": "forward sweep + trajectory store + cost terms"},
+                                            "note": "forward sweep + trajectory store + cost terms (wk_forward and ck_cost, timed together)"},
                          "bytes_per_processed_point_step": (fwd_b + adj_b) / pts},
         }
         if not args.no_cpu_baseline and world == 1:

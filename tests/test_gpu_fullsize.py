@@ -212,3 +212,26 @@ def test_config4_every_layout_at_full_size(lay):
         Jo, go, _ = o.eval_global(x)
         Jg, gg = g.eval_global(x)
         assert abs(Jg - Jo) <= TOL_EVAL * abs(Jo) and rel(gg.cpu().numpy(), go) <= TOL_EVAL
+
+
+def test_config3_gauss_newton_operator_on_sampled_subdomains():
+    """SURVEY.md 8(f1) at the headline size: H_GN p (TLM sweep + adjoint sweep + control-level terms) of
+    sampled subdomains of config 3 against the oracle, first / middle / last window, pole and interior tiles."""
+    w = synth.CONFIGS[3]
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    assert g.active_path == 5
+    p12 = w.p_lon * w.p_lat
+    sample = [0, 5 * 16 + 7, 3 * p12 + 15 * 16 + 15, 4 * p12 + 8 * 16 + 3, 7 * p12 + 2, 7 * p12 + 15 * 16]
+    xs = g.get_controls()
+    flat_p = g.torch.zeros_like(xs)
+    ps = {}
+    for k in sample:
+        ps[k] = synth.random_fields(o.sub_shape(k), 500 + k)
+        flat_p[g.offsets[k]:g.offsets[k + 1]] = g.torch.from_numpy(ps[k].reshape(-1)).to(flat_p.device)
+    Hp = g.gn_hessvec(xs, flat_p)
+    for k in sample:
+        ref = o.gn_hessvec(k, o.get_control(k), ps[k])
+        got = Hp[g.offsets[k]:g.offsets[k + 1]].cpu().numpy().reshape(ref.shape)
+        assert rel(got, ref) <= 1e-10, (k, rel(got, ref))
+        assert np.abs(got - ref).max() <= 1e-9 * np.abs(ref).max(), k
