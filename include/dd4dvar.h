@@ -198,6 +198,11 @@ int dd4dvar_active_path(dd4dvar_t h);
  * returns 0 or -1 (negative weight). */
 int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later);
 
+/* Column 0 of the history of dd4dvar_run / dd4dvar_run_gn, J of eq (6) l.111 at the gathered analysis, costs one
+ * undecomposed forecast over the whole assimilation window per outer iteration (it is a diagnostic, not part of
+ * Algorithm 1).  on = 0: skip it, column 0 is NaN; default on. */
+int dd4dvar_set_history_global(dd4dvar_t h, int on);
+
 /* Measurement aid ("which roofline binds"): microbenchmarks of the device's
  * fp64 FMA rate, fp64 ADD rate, shared-memory load bandwidth and 64-bit warp-shuffle rate, the
  * secondary bounds of the stencil sweep next to HBM (SURVEY.md section 8(d) asks for the fp64 peak to

@@ -111,6 +111,7 @@ struct dd4dvar_s {
     double sig_o[3] = { 1, 1, 1 };
     Layout G, L;
     bool have_ws = false, have_bg = false;
+    bool history_global = true;         // evaluate J of eq (6) at the gathered analysis after every outer iteration
     void* ws = nullptr;
     size_t ws_bytes = 0;
     int* h_pin = nullptr;               // pinned scratch for small read-backs
@@ -962,6 +963,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         *out = (double)sacc; return 0;
     };
     auto gather_and_cost = [&](double* out) -> int {
+        if (!h->history_global) { *out = nan(""); return 0; }
         LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, G.x);
         return global_cost(h, out);
     };
@@ -1012,7 +1014,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         double dl = 0; for (int k = 0; k < nsub; ++k) dl = std::max(dl, h->h_tmp[k]);
         h_history[3 * l + 2] = dl;
         if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
-        if (!isfinite(h_history[3 * l]) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run: non-finite cost");
+        if ((h->history_global && !isfinite(h_history[3 * l])) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run: non-finite cost");
     }
     LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
     return sync_check(h);
@@ -1079,6 +1081,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
         *out = (double)sacc; return 0;
     };
     auto gather_and_cost = [&](double* out) -> int {
+        if (!h->history_global) { *out = nan(""); return 0; }
         LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, G.x);
         return global_cost(h, out);
     };
@@ -1118,7 +1121,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
         double dl = 0; for (int k = 0; k < nsub; ++k) dl = std::max(dl, h->h_tmp[k]);
         h_history[3 * l + 2] = dl;
         if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
-        if (!isfinite(h_history[3 * l]) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run_gn: non-finite cost");
+        if ((h->history_global && !isfinite(h_history[3 * l])) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run_gn: non-finite cost");
     }
     LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
     return sync_check(h);
@@ -1128,6 +1131,13 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
 {
     if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
     h->cp.bgw = w_later;
+    return 0;
+}
+
+int dd4dvar_set_history_global(dd4dvar_t h, int on)
+{
+    if (!h) return -1;
+    h->history_global = on != 0;
     return 0;
 }
 

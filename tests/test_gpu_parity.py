@@ -276,3 +276,14 @@ def test_two_live_handles_on_two_streams_with_different_grids():
         check_eval_local(oa, ga, xa)
         ga.close(); gb.close()
         del pka, pkb
+
+
+def test_history_global_switch_changes_only_the_diagnostic_column():
+    w, o, prob, g = make_pair("cfg0", 0)
+    an1, h1 = g.run(2)
+    g2 = gpu_problem(w, prob)
+    g2.set_history_global(False)
+    an2, h2 = g2.run(2)
+    assert np.all(np.isnan(h2[:, 0])) and np.all(np.isfinite(h1[:, 0]))
+    assert np.array_equal(h1[:, 1:], h2[:, 1:])
+    assert np.array_equal(an1.cpu().numpy(), an2.cpu().numpy())
