@@ -82,8 +82,7 @@ __device__ __forceinline__ void wa_issue_row(const WaCtx<K>& C, int r, bool with
     if ((unsigned)lj < (unsigned)g.ey) { src = C.tz + lj * g.ex; bytes = g.ex * 8u; fstride = g.ncell; dst += 32u; }
     else { src = C.gz + (lj < 0 ? r : g.gys + lj - g.ey) * g.px; bytes = g.px * 8u; fstride = g.nring; }
     wk_mbar_expect32(bar, 3u * bytes + (with_edges ? (uint32_t)(g.gys + g.gyn) * 16u : 0u));
-#pragma unroll 1
-    for (int f = 0; f < 3; ++f) { wk_g2s32(dst, src, bytes, bar); dst += C.ZP8; src += fstride; }
+    wk_g2s32(dst, src, bytes, bar); wk_g2s32(dst + C.ZP8, src + fstride, bytes, bar); wk_g2s32(dst + 2u * C.ZP8, src + 2 * fstride, bytes, bar);
     if (with_edges && g.gys) wk_g2s32(C.sm32 + 8u * C.I_EDS, C.ge, g.gys * 16u, bar);
     if (with_edges && g.gyn) wk_g2s32(C.sm32 + 8u * (C.I_EDS + 8), C.ge + g.gys * 2, g.gyn * 16u, bar);
 }

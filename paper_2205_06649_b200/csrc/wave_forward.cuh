@@ -391,10 +391,9 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
     if (wk_elect()) {
         wk_wait_read<2>();
         wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
-        uint32_t src = urow - 3u * P8;
+        const uint32_t src = urow - 3u * P8;
         double* dst = C.tout + l3 * g.ex;
-#pragma unroll 1
-        for (int f = 0; f < 3; ++f) { wk_s2g32(dst, src, g.ex * 8u); dst += g.ncell; src += FS8; }
+        wk_s2g32(dst, src, g.ex * 8u); wk_s2g32(dst + g.ncell, src + FS8, g.ex * 8u); wk_s2g32(dst + 2 * g.ncell, src + 2u * FS8, g.ex * 8u);
         wk_commit();
         if ((l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
         if (C.first && lj + WK_XD < g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
