@@ -157,9 +157,16 @@ def whole_job_value(units_per_rank, world, seconds):
     return world * units_per_rank / seconds
 
 
+LAYOUT = None          # --layout p_lon,p_lat,q_time,overlap: another decomposition of the chosen config's problem (config 4)
+
+
 def workload(cfg):
     if cfg in synth.CONFIGS:
-        return synth.CONFIGS[cfg]
+        w = synth.CONFIGS[cfg]
+        if LAYOUT:
+            import dataclasses
+            w = dataclasses.replace(w.with_layout(*LAYOUT), name=w.name.rsplit(" ", 2)[0] + " %dx%dx%d o%d" % tuple(LAYOUT))
+        return w
     raise SystemExit(f"unknown config {cfg}")
 
 
@@ -340,7 +347,11 @@ def main():
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     ap.add_argument("--peaks", action="store_true", help="run the library's fp64 / shared-memory / shuffle microbenchmarks")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the CUDA sources (for profiles/traffic.json)")
+    ap.add_argument("--layout", default=None, help="p_lon,p_lat,q_time,overlap: decomposition override (config 4 layouts on --config 2)")
     args = ap.parse_args()
+    if args.layout:
+        global LAYOUT
+        LAYOUT = [int(x) for x in args.layout.split(",")]
     if args.csrc_hash:
         print(csrc_hash())
         return

@@ -566,6 +566,9 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 wa_issue_lamrow<K>(C, -g.gys);
                 wa_issue_lamrow<K>(C, 1 - g.gys);
             }
+#if WK_STAGGER
+            if (C.has_leader && !C.first) { const int nd = WK_STAGGER < C.TLd + 1 ? WK_STAGGER : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+#endif
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
 #ifdef WK_PROF

@@ -31,6 +31,9 @@
 #define WK_NW 8                 // warps per CTA = time steps in flight per CTA
 #endif
 #define WK_NT (WK_NW * 32)
+#ifndef WK_STAGGER
+#define WK_STAGGER 0            // ticks a step starts behind its leader (0: as soon as the data allows, 4 ticks)
+#endif
 #define WK_EWC 4                // tile rows per staged chunk of east/west ghost cells (forward kernel)
 #define WK_EWCA 2               // the same in the adjoint kernel (its shared memory is full)
 #define WK_HDR 128              // doubles reserved at the start of shared memory (barriers, flags)

@@ -531,6 +531,11 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
 #ifdef WK_PROF
             C.pt = clock64();
 #endif
+#if WK_STAGGER
+            // start WK_STAGGER ticks (not just the 4 the data needs) behind the leader: the spare ticks absorb the
+            // jitter of the steps ahead; 8 steps x 7 ticks still fit into the ticks of one step
+            if (C.has_leader && !C.first) { const int nd = WK_STAGGER < C.TLd + 1 ? WK_STAGGER : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+#endif
             if (C.first || g.gys == 0) {
                 // what tick -1 would do: the control rows that ticks 0 and 1 read, the ghost cells of tile row 0
                 if (C.has_leader) { const int nd = C.dlead - 1 < C.TLd + 1 ? C.dlead - 1 : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
