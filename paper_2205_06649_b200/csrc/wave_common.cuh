@@ -140,10 +140,16 @@ __device__ __forceinline__ void wk_mbar_init32(uint32_t bar, int count)
 }
 __device__ __forceinline__ void wk_mbar_expect32(uint32_t bar, uint32_t bytes)
 {
+#ifdef WK_NODMA
+    return;
+#endif
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void wk_mbar_wait32(uint32_t bar, uint32_t parity)
 {
+#ifdef WK_NODMA
+    return;
+#endif
     uint32_t ok;
     do {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
@@ -152,11 +158,17 @@ __device__ __forceinline__ void wk_mbar_wait32(uint32_t bar, uint32_t parity)
 }
 __device__ __forceinline__ void wk_g2s32(uint32_t dst, const double* src, uint32_t bytes, uint32_t bar)
 {
+#ifdef WK_NODMA
+    return;
+#endif
     asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void wk_s2g32(double* dst, uint32_t src, uint32_t bytes)
 {
+#ifdef WK_NODMA
+    return;
+#endif
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void wk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
