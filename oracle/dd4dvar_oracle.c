@@ -342,6 +342,8 @@ typedef struct {
     int nsteps;
     int p1, p2, q, o;
     double mu, lambda;
+    int ovl_levels;   /* (25c) case 1 on every level of the window (eq (21) l.300 read literally: O_ik maps onto Delta_j x
+                       * (Omega_i n Omega_k)), not on the control level only (reading R12, the default 0) */
     double bgw;   /* weight of (25a) in windows j > 0 (0 = only at t_0, reading R7, the default; 1 = in every window as (25a) is printed) */
     int lbfgs_m, n_inner, max_bt; double c1;
     int nsub; Sub* sub;
@@ -553,6 +555,26 @@ static void local_eval(const DD* d, int k, const double* x, CostParts* cp, doubl
                 }
             }
     }
+    if (d->ovl_levels)                                    /* (25c) case 1 on the levels n = 1 .. W as well */
+        for (int n = 1; n <= W; ++n)
+            for (int fl = 0; fl < NF; ++fl) {
+                double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
+                for (int lj = 0; lj < s->ey; ++lj)
+                    for (int li = 0; li < s->ex; ++li) {
+                        int gi = imod(s->ei0 + li, nlon), gj = s->ej0 + lj;
+                        long c = (long)lj * s->ex + li;
+                        double zv = traj[((size_t)n * NF + fl) * nc + c];
+                        for (int cb = 0; cb < d->nrowcov[gj]; ++cb)
+                            for (int ca = 0; ca < d->ncolcov[gi]; ++ca) {
+                                int a2 = d->colcov[4 * gi + ca], b2 = d->rowcov[4 * gj + cb];
+                                if (a2 == s->a && b2 == s->b) continue;
+                                int k2 = sub_index(d, s->jw, b2, a2);
+                                long c2 = local_cell(d, &d->sub[k2], gi, gj);
+                                double dv = zv - frozen_traj(d, k2, s->s + n, fl, c2, gi, gj);
+                                Jsp += (long double)(dv * dv * ib);
+                            }
+                    }
+            }
     if (d->have_obs)
         for (long q = 0; q < d->nlocobs[k]; ++q) {        /* (25b) */
             const LocObs* ob = &d->locobs[k][q];
@@ -603,6 +625,24 @@ static void local_eval(const DD* d, int k, const double* x, CostParts* cp, doubl
                     double rr = traj[((size_t)n * NF + ob->fld) * nc + ob->cell] - ob->y;
                     lam[(size_t)ob->fld * nc + ob->cell] +=
                         2.0 * d->lambda * wt * rr / (d->sig_o[ob->fld] * d->sig_o[ob->fld]);
+                }
+            if (d->ovl_levels && n > 0)                    /* forcing of the all-level overlap term */
+                for (int fl = 0; fl < NF; ++fl) {
+                    double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
+                    for (int lj = 0; lj < s->ey; ++lj)
+                        for (int li = 0; li < s->ex; ++li) {
+                            int gi = imod(s->ei0 + li, nlon), gj = s->ej0 + lj;
+                            long c = (long)lj * s->ex + li;
+                            double zv = traj[((size_t)n * NF + fl) * nc + c];
+                            for (int cb = 0; cb < d->nrowcov[gj]; ++cb)
+                                for (int ca = 0; ca < d->ncolcov[gi]; ++ca) {
+                                    int a2 = d->colcov[4 * gi + ca], b2 = d->rowcov[4 * gj + cb];
+                                    if (a2 == s->a && b2 == s->b) continue;
+                                    int k2 = sub_index(d, s->jw, b2, a2);
+                                    long c2 = local_cell(d, &d->sub[k2], gi, gj);
+                                    lam[(size_t)fl * nc + c] += 2.0 * d->mu * (zv - frozen_traj(d, k2, level, fl, c2, gi, gj)) * ib;
+                                }
+                        }
                 }
             if (n > 0) {
                 fill_padded(d, k, level - 1, traj + (size_t)(n - 1) * NF * nc, Zp, &r);
@@ -828,7 +868,7 @@ void* orc_create(int nlon, int nlat, double radius, double omega, double gravity
     d->m.nlon = nlon; d->m.nlat = nlat; d->m.a = radius; d->m.Omega = omega; d->m.g = gravity;
     d->m.cos_clamp = cos_clamp; d->m.kappa = diffusion; d->m.dt = dt;
     d->nsteps = nsteps; d->p1 = p_lon; d->p2 = p_lat; d->q = q_time; d->o = overlap;
-    d->mu = mu; d->lambda = lambda; d->bgw = 0.0;
+    d->mu = mu; d->lambda = lambda; d->bgw = 0.0; d->ovl_levels = 0;
     d->lbfgs_m = lbfgs_m; d->n_inner = n_inner; d->max_bt = max_bt; d->c1 = c1;
     if (nlon < 3 || nlat < 2 || nsteps < 1) { *status = -1; free(d); return NULL; }
     model_tables(&d->m);
@@ -843,6 +883,7 @@ void* orc_create(int nlon, int nlat, double radius, double omega, double gravity
 }
 /* weight of the background term (25a) in the windows j > 0 (R7: default 0; 1 = as printed) */
 void orc_set_bg_weight(void* h, double w) { ((DD*)h)->bgw = w; }
+void orc_set_overlap_levels(void* h, int on) { ((DD*)h)->ovl_levels = on != 0; }
 static void free_local(DD* d)
 {
     for (int k = 0; k < d->nsub; ++k) {
@@ -1175,6 +1216,17 @@ static void local_gn_hessvec(const DD* d, int k, const double* traj, const doubl
                 double dz = dtr[((size_t)n * NF + ob->fld) * nc + ob->cell];
                 lam[(size_t)ob->fld * nc + ob->cell] +=
                     2.0 * d->lambda * wt * dz / (d->sig_o[ob->fld] * d->sig_o[ob->fld]);
+            }
+        if (d->ovl_levels && n > 0)
+            for (int fl = 0; fl < NF; ++fl) {
+                double ib = 1.0 / (d->sig_b[fl] * d->sig_b[fl]);
+                for (int lj = 0; lj < s->ey; ++lj)
+                    for (int li = 0; li < s->ex; ++li) {
+                        int gi = imod(s->ei0 + li, nlon), gj = s->ej0 + lj;
+                        long c = (long)lj * s->ex + li;
+                        int m = d->nrowcov[gj] * d->ncolcov[gi] - 1;       /* other extended tiles holding the cell */
+                        lam[(size_t)fl * nc + c] += 2.0 * d->mu * m * dtr[((size_t)n * NF + fl) * nc + c] * ib;
+                    }
             }
         if (n > 0) {
             fill_padded(d, k, level - 1, traj + (size_t)(n - 1) * NF * nc, Zp, &r);

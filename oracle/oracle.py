@@ -116,6 +116,12 @@ class Oracle:
         self.lib.orc_set_bg_weight(self._h, float(w))
 
     # ---- geometry
+    def set_overlap_levels(self, on):
+        """(25c) case 1 on every level of the window (eq (21), read literally) instead of the control level only."""
+        self.lib.orc_set_overlap_levels.argtypes = [C.c_void_p, C.c_int]
+        self.lib.orc_set_overlap_levels.restype = None
+        self.lib.orc_set_overlap_levels(self._h, int(bool(on)))
+
     def sub_info(self, k):
         out = (C.c_int * 16)()
         self.lib.orc_sub_info(self._h, k, out)
