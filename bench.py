@@ -347,6 +347,7 @@ def main():
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     ap.add_argument("--peaks", action="store_true", help="run the library's fp64 / shared-memory / shuffle microbenchmarks")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the CUDA sources (for profiles/traffic.json)")
+    ap.add_argument("--overlap-levels", action="store_true", help="spatial overlap penalty on every level of the window (needs --path 1)")
     ap.add_argument("--layout", default=None, help="p_lon,p_lat,q_time,overlap: decomposition override (config 4 layouts on --config 2)")
     args = ap.parse_args()
     if args.layout:
@@ -387,6 +388,8 @@ def main():
 
     # ---- build the replica of the workload on this rank (seeded synthetic inputs)
     g = DD4DVar.from_workload(w, path=args.path, device=f"cuda:{local_rank}")
+    if args.overlap_levels:
+        g.set_overlap_levels(True)                    # (25c) on every level of the window (generic kernels: --path 1)
     prob = synth.make_problem(w, g.forecast)          # truth trajectory from the library's own model
     g.set_background(prob.xb, prob.sigma_b)
     g.set_observations(prob.obs)
@@ -488,7 +491,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "counted": "useful = nlon*nlat*nsteps per sweep",
                        "processed_point_steps_per_sweep": pts, "processed_value": world * pts / (ms_step * 1e-3),
-                       "subdomains": g.nsub, "path": PATH_NAMES.get(ap, str(ap)),
+                       "subdomains": g.nsub, "path": PATH_NAMES.get(ap, str(ap)), "overlap_levels": bool(args.overlap_levels),
                        "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "outer_iteration_ms": 1e3 * outer_s, "outer_iteration_ms_without_global_history": 1e3 * outer_ng_s,

@@ -203,6 +203,13 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later);
  * Algorithm 1).  on = 0: skip it, column 0 is NaN; default on. */
 int dd4dvar_set_history_global(dd4dvar_t h, int on);
 
+/* The spatial overlap penalty (25c) case 1 l.310-314 acts on the control level of the window (R12, the
+ * default).  on = 1: on every level of the window, eq (21) l.300 read literally (O_ik maps onto Delta_j x (Omega_i n
+ * Omega_k)); the neighbours' frozen trajectories on the overlap rectangles are then kept in a second store,
+ * refreshed at every exchange.  Served by the generic kernels only: create with opts.path = 1, else -2; call
+ * before dd4dvar_set_background, else -3.  Not available with dd4dvar_run_gn. */
+int dd4dvar_set_overlap_levels(dd4dvar_t h, int on);
+
 /* Measurement aid ("which roofline binds"): microbenchmarks of the device's
  * fp64 FMA rate, fp64 ADD rate, shared-memory load bandwidth and 64-bit warp-shuffle rate, the
  * secondary bounds of the stencil sweep next to HBM (SURVEY.md section 8(d) asks for the fp64 peak to

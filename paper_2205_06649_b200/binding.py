@@ -51,7 +51,7 @@ EXPORTS = [
     "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
-    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global",
+    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global", "dd4dvar_set_overlap_levels",
     "dd4dvar_last_error", "dd4dvar_destroy",
 ]
 
@@ -96,6 +96,7 @@ def load_library():
     lib.dd4dvar_measure_peaks.argtypes = [vp, hd]
     lib.dd4dvar_set_bg_weight.argtypes = [vp, C.c_double]
     lib.dd4dvar_set_history_global.argtypes = [vp, C.c_int]
+    lib.dd4dvar_set_overlap_levels.argtypes = [vp, C.c_int]
     lib.dd4dvar_last_error.restype = C.c_char_p
     lib.dd4dvar_last_error.argtypes = [vp]
     lib.dd4dvar_destroy.restype = None
@@ -312,6 +313,10 @@ class DD4DVar:
         self._check("dd4dvar_gn_hessvec", self.lib.dd4dvar_gn_hessvec(self._h, controls.data_ptr(), p.data_ptr(),
                                                                       out.data_ptr()))
         return out
+
+    def set_overlap_levels(self, on):
+        """(25c) case 1 on every level of the window (generic kernels only; before set_background)."""
+        self._check("dd4dvar_set_overlap_levels", self.lib.dd4dvar_set_overlap_levels(self._h, int(bool(on))))
 
     def set_history_global(self, on):
         self._check("dd4dvar_set_history_global", self.lib.dd4dvar_set_history_global(self._h, int(bool(on))))

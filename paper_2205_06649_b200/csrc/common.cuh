@@ -23,6 +23,8 @@ struct Sub {
     long long ooff;          // index into obs_start: entries ooff .. ooff+W+1
     long long eoff;          // offset in the edge store [W][py][2] (frozen u^a of ghost columns 1, px-2)
     int nb0, nnb;            // this subdomain's overlap rectangles: entries nb0 .. nb0+nnb-1 of the NbRect table
+    int novl;                // cells of all those rectangles together
+    long long voff;          // offset in the overlap store [W][3][novl] (levels 1 .. W; option overlap_levels)
 };
 
 // One rectangle Omega_i ∩ Omega_k of the spatial overlap (eq (20)-(22) l.294-306, case 1 l.310-314):
@@ -30,7 +32,9 @@ struct Sub {
 // neighbour tile in the same window, whose control starts at coff2 (shape [3][ncell2], row length ex2).
 struct NbRect {
     long long coff2;
+    long long toff2;         // the neighbour's offset in the trajectory store
     int ex2, ncell2, i0, j0, w, h, ni0, nj0;
+    int ooff;                // first cell of this rectangle in the subdomain's overlap list (row-major inside the rectangle)
 };
 
 // Model constants with dt folded in (row tables live in device memory, length nlat).

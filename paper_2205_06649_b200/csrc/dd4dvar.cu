@@ -65,7 +65,9 @@ struct Layout {
     std::vector<NbRect> hnb;
     NbRect* dnb = nullptr;
     std::vector<int> colown, rowown, ncolcov, colcov, nrowcov, rowcov, tc_ei0, tc_ex, tr_ej0, tr_ey, wb;
-    long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0, etot = 0;
+    long long ctot = 0, ttot = 0, gtot = 0, ptot1 = 0, otot = 0, etot = 0, vtot = 0;
+    int maxnovl = 0;
+    double* ovl = nullptr;              // overlap store (option overlap_levels, generic path)
     int maxnpad = 0, maxncell = 0, maxnring = 0, Wmax = 0, CB = 1, maxcov = 1;
     // device
     Sub* dsubs = nullptr;
@@ -111,6 +113,7 @@ struct dd4dvar_s {
     double sig_o[3] = { 1, 1, 1 };
     Layout G, L;
     bool have_ws = false, have_bg = false;
+    bool overlap_levels = false;        // (25c) case 1 on every level of the window (generic path only)
     bool history_global = true;         // evaluate J of eq (6) at the gathered analysis after every outer iteration
     void* ws = nullptr;
     size_t ws_bytes = 0;
@@ -189,7 +192,7 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
     for (int v : L.nrowcov) mr = std::max(mr, v);
     L.maxcov = mc * mr;
     L.hs.resize(L.nsub);
-    L.ctot = L.ttot = L.gtot = L.ptot1 = L.otot = L.etot = 0;
+    L.ctot = L.ttot = L.gtot = L.ptot1 = L.otot = L.etot = L.vtot = 0; L.maxnovl = 0;
     L.maxnpad = L.maxncell = L.maxnring = L.Wmax = 0;
     for (int jw = 0; jw < q; ++jw)
         for (int b = 0; b < p2; ++b)
@@ -218,7 +221,7 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
     L.hnb.clear();
     for (int k = 0; k < L.nsub; ++k) {
         Sub& s = L.hs[k];
-        s.nb0 = (int)L.hnb.size();
+        s.nb0 = (int)L.hnb.size(); s.novl = 0;
         for (int b2 = 0; b2 < p2; ++b2)
             for (int a2 = 0; a2 < p1; ++a2) {
                 if (a2 == s.a && b2 == s.b) continue;
@@ -230,13 +233,16 @@ int build_layout(Layout& L, int nlon, int nlat, int N, int p1, int p2, int q, in
                     const int i0 = std::max(s.ei0, t0), i1 = std::min(s.ei0 + s.ex, t0 + t.ex);
                     if (i1 <= i0) continue;
                     NbRect r;
-                    r.coff2 = t.coff; r.ex2 = t.ex; r.ncell2 = t.ncell;
+                    r.coff2 = t.coff; r.toff2 = t.toff; r.ex2 = t.ex; r.ncell2 = t.ncell;
+                    r.ooff = s.novl; s.novl += (i1 - i0) * (j1 - j0);
                     r.i0 = i0 - s.ei0; r.j0 = j0 - s.ej0; r.w = i1 - i0; r.h = j1 - j0;
                     r.ni0 = i0 - t0; r.nj0 = j0 - t.ej0;
                     L.hnb.push_back(r);
                 }
             }
         s.nnb = (int)L.hnb.size() - s.nb0;
+        s.voff = L.vtot; L.vtot += (long long)s.W * 3 * s.novl;
+        L.maxnovl = std::max(L.maxnovl, s.novl);
     }
     {
         int mex = 0, mey = 0;
@@ -280,6 +286,7 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
         L.st.gam = ar.take<double>((size_t)L.nsub * std::max(m, 1));
         L.st.nactive = ar.take<int>(4);
     }
+    if ((L.path == 1 || L.path == 3) && L.vtot > 0) L.ovl = ar.take<double>(L.vtot);
     fused_plan_arrays(L.fp, ar_take_bytes, &ar);
     if (L.wp.enabled) {
         L.gedge = ar.take<double>(std::max<long long>(L.etot, 2));
@@ -376,6 +383,8 @@ void cost_generic(dd4dvar_t h, Layout& L, const int* mask, double* Jout)
            L.xfrozen, L.pred_end, L.traj, L.have_obs ? L.obs_start : nullptr, L.obs_idx, L.obs_y, L.obs_c,
            L.partial);
     LAUNCH(gk_cost_final, (L.nsub + 127) / 128, 128, L.nsub, mask, L.CB, L.partial, L.parts, Jout);
+    if (h->overlap_levels && L.ovl)
+        LAUNCH(gk_ovl_cost<NT_RED>, L.nsub, NT_RED, L.dsubs, L.dnb, mask, h->cp, L.traj, L.ovl, L.parts, Jout);
 }
 void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
 {
@@ -388,6 +397,8 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
         if (L.have_obs)
             LAUNCH(gk_obs_force, dim3(4, L.nsub), NT_GK, L.dsubs, mask, n, L.obs_start, L.obs_idx, L.obs_y,
                    L.obs_c, L.traj, cur);
+        if (n > 0 && h->overlap_levels && L.ovl)
+            LAUNCH(gk_ovl_force, cell_grid(L), NT_GK, L.dsubs, L.dnb, mask, n, h->cp, L.traj, L.ovl, cur);
         if (n > 0 && L.path != 3) {
             sk_adjoint_step<<<dim3(L.ntiles, L.nsub), SK_NT, sizeof(double) * SK_ADJ_SMEM_DOUBLES, h->stream>>>(
                 L.dsubs, mask, n - 1, h->mp, L.traj, L.ghost, cur, nxt, L.tiles_x);
@@ -524,6 +535,8 @@ void exchange(dd4dvar_t h, Layout& L)
     if (L.maxnring > 0)
         LAUNCH(xk_ghost_fill, dim3((L.maxnring + 127) / 128, L.nsub, std::min(L.Wmax, 8)), 128, L.dsubs, L.geo,
                L.traj, L.ghost);
+    if (h->overlap_levels && L.ovl && L.maxnovl > 0)
+        LAUNCH(xk_ovl_fill, dim3((L.maxnovl + 127) / 128, L.nsub, std::min(L.Wmax, 8)), 128, L.dsubs, L.dnb, L.traj, L.ovl);
     if (L.wp.enabled)
         LAUNCH(xk_edge_ua, dim3((2 * L.wp.maxpy + 63) / 64, L.nsub, std::min(L.Wmax, 8)), 64, L.dsubs, h->mp,
                L.ghost, L.gedge);
@@ -1131,6 +1144,16 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
 {
     if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
     h->cp.bgw = w_later;
+    return 0;
+}
+
+int dd4dvar_set_overlap_levels(dd4dvar_t h, int on)
+{
+    if (!h) return -1;
+    if (h->have_bg) return fail(h, -3, "set_overlap_levels after set_background");
+    if (on && h->L.path != 1 && h->L.path != 3)
+        return fail(h, -2, "set_overlap_levels: served by the generic kernels only (create with opts.path = 1)");
+    h->overlap_levels = on != 0;
     return 0;
 }
 

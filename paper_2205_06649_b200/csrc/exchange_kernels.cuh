@@ -160,3 +160,24 @@ __global__ void xk_edge_ua(const Sub* __restrict__ subs, ModelP m, const double*
         gedge[s.eoff + (long long)n * 2 * s.py + slot * 2 + side] = ua;
     }
 }
+
+// Option overlap_levels: the neighbours' trajectories of this iteration on the overlap rectangles, levels 1 .. W
+// (same window, same local level), into the compact overlap store [W][3][novl] of every subdomain.
+__global__ void xk_ovl_fill(const Sub* __restrict__ subs, const NbRect* __restrict__ nbr,
+                            const double* __restrict__ traj, double* __restrict__ ovl)
+{
+    const int k = blockIdx.y;
+    const Sub s = subs[k];
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= s.novl) return;
+    int r = 0;
+    while (r + 1 < s.nnb && nbr[s.nb0 + r + 1].ooff <= e) ++r;
+    const NbRect nb = nbr[s.nb0 + r];
+    const int q = e - nb.ooff, dj = q / nb.w, di = q - dj * nb.w;
+    const long long c2 = (long long)(nb.nj0 + dj) * nb.ex2 + nb.ni0 + di;
+    for (int n = 1 + blockIdx.z; n <= s.W; n += gridDim.z)
+#pragma unroll
+        for (int f = 0; f < DD_NF; ++f)
+            ovl[s.voff + ((long long)(n - 1) * DD_NF + f) * s.novl + e] =
+                traj[nb.toff2 + ((long long)n * DD_NF + f) * nb.ncell2 + c2];
+}

@@ -303,6 +303,69 @@ __global__ void gk_obs_force(const Sub* __restrict__ subs, const int* __restrict
 }
 
 // ------------------------------------------------------------------------------------------
+// Option overlap_levels: the spatial overlap penalty (25c) case 1 on EVERY level of the window
+// (eq (21) l.300 read literally), generic path only.  ovl: the neighbours' frozen trajectories on the overlap
+// rectangles, [W][3][novl] per subdomain (levels 1 .. W), refreshed by xk_ovl_fill at every exchange.
+// Adjoint forcing at local level n >= 1: gather form (every cell looks up the rectangles that hold it).
+__global__ void gk_ovl_force(const Sub* __restrict__ subs, const NbRect* __restrict__ nbr, const int* __restrict__ mask,
+                             int n, CostP cp, const double* __restrict__ traj, const double* __restrict__ ovl,
+                             double* __restrict__ lam)
+{
+    const int k = blockIdx.y;
+    if (mask && !mask[k]) return;
+    const Sub s = subs[k];
+    if (n < 1 || n > s.W || s.novl == 0) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= s.ncell) return;
+    const int lj = c / s.ex, li = c - lj * s.ex;
+    const double* t = traj + s.toff + (long long)n * DD_NF * s.ncell;
+    const double* o = ovl + s.voff + (long long)(n - 1) * DD_NF * s.novl;
+    double acc[3] = { 0.0, 0.0, 0.0 };
+    for (int r = 0; r < s.nnb; ++r) {
+        const NbRect nb = nbr[s.nb0 + r];
+        const int di = li - nb.i0, dj = lj - nb.j0;
+        if ((unsigned)di < (unsigned)nb.w && (unsigned)dj < (unsigned)nb.h) {
+            const int e = nb.ooff + dj * nb.w + di;
+#pragma unroll
+            for (int f = 0; f < 3; ++f) acc[f] += 2.0 * cp.mu * (t[(long long)f * s.ncell + c] - o[(long long)f * s.novl + e]) * cp.ib[f];
+        }
+    }
+    double* l = lam + s.poff;
+#pragma unroll
+    for (int f = 0; f < 3; ++f) l[(long long)f * s.npad + (lj + s.gys) * s.px + li + s.gx] += acc[f];
+}
+// its cost, added to the spatial-overlap part and to J_ji (one CTA per subdomain, fixed-order sums)
+template <int NT>
+__global__ void gk_ovl_cost(const Sub* __restrict__ subs, const NbRect* __restrict__ nbr, const int* __restrict__ mask,
+                            CostP cp, const double* __restrict__ traj, const double* __restrict__ ovl,
+                            double* __restrict__ parts, double* __restrict__ J)
+{
+    __shared__ double red[32];
+    const int k = blockIdx.x;
+    if (mask && !mask[k]) return;
+    const Sub s = subs[k];
+    double acc = 0.0;
+    for (int r = 0; r < s.nnb; ++r) {
+        const NbRect nb = nbr[s.nb0 + r];
+        const int ncr = nb.w * nb.h;
+        for (int q = threadIdx.x; q < ncr * s.W; q += NT) {
+            const int n = q / ncr + 1, e = q - (n - 1) * ncr;
+            const int dj = e / nb.w, di = e - dj * nb.w;
+            const int c = (nb.j0 + dj) * s.ex + nb.i0 + di;
+            const double* t = traj + s.toff + (long long)n * DD_NF * s.ncell;
+            const double* o = ovl + s.voff + (long long)(n - 1) * DD_NF * s.novl + nb.ooff + e;
+#pragma unroll
+            for (int f = 0; f < 3; ++f) {
+                const double dv = t[(long long)f * s.ncell + c] - o[(long long)f * s.novl];
+                acc += dv * dv * cp.ib[f];
+            }
+        }
+    }
+    acc = block_sum<NT>(acc, red);
+    if (threadIdx.x == 0) { parts[k * 5 + 2] += cp.mu * acc; J[k] += cp.mu * acc; }
+}
+
+// ------------------------------------------------------------------------------------------
 // cost terms of J_ji, eq (25) l.338-344: partial sums per (block, subdomain), fixed order.
 // parts: [nsub][CB][5] = bg (25a), obs (25b), spatial overlap, predecessor, successor (25c).
 template <int NT>

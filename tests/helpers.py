@@ -15,9 +15,11 @@ def oracle_problem(w, **kw):
     return o, prob
 
 
-def gpu_problem(w, prob, **kw):
+def gpu_problem(w, prob, overlap_levels=False, **kw):
     from paper_2205_06649_b200.binding import DD4DVar
     g = DD4DVar.from_workload(w, **kw)
+    if overlap_levels:
+        g.set_overlap_levels(True)
     g.set_background(prob.xb, prob.sigma_b)
     if prob.obs is not None:
         g.set_observations(prob.obs)

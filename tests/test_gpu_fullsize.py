@@ -235,3 +235,13 @@ def test_config3_gauss_newton_operator_on_sampled_subdomains():
         got = Hp[g.offsets[k]:g.offsets[k + 1]].cpu().numpy().reshape(ref.shape)
         assert rel(got, ref) <= 1e-10, (k, rel(got, ref))
         assert np.abs(got - ref).max() <= 1e-9 * np.abs(ref).max(), k
+
+
+def test_config4_layout_with_the_overlap_penalty_on_every_level():
+    """SURVEY.md 8(f4) at full size: the 4x4x4 o2 layout of config 4 (720x360, 32-step windows) with the spatial
+    overlap penalty on every level of the window (generic kernels), sampled subdomains against the oracle."""
+    w = synth.CONFIGS[2].with_layout(4, 4, 4, 2)
+    o, prob = oracle_problem(w)
+    o.set_overlap_levels(True)
+    g = gpu_problem(w, prob, overlap_levels=True, path=1)
+    check_sample(o, g, prob, [0, 5, 21, 38, 47, 63], 71)
