@@ -156,13 +156,19 @@ int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, d
 
 /* The same evaluation end to end with HOST buffers: h_controls is copied to the device, the
  * gradient sweep runs, costs and (if h_grads != NULL) gradients are copied back.  Pinned host
- * memory makes the copies asynchronous with respect to the host but they are inside the call. */
+ * memory makes the copies asynchronous with respect to the host but they are inside the call.
+ * With 64 or more subdomains the evaluation runs in four chunks of consecutive subdomains (they are independent:
+ * all neighbour data is frozen) so that the copies of one chunk overlap the sweeps of the others; the library
+ * creates two non-blocking copy streams for this on first use and destroys them with the handle.  Results are
+ * identical to dd4dvar_eval_local. */
 int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_costs, double* h_grads);
 
 /* Same evaluation, queued on the stream without host synchronisation or host output, at the
  * library's own current controls: used for timing the gradient sweep (bench.py).
  * mode 0: forward sweep + trajectory store + cost terms (a1-a3); 1: the whole gradient sweep
  * (a1-a4); 2: adjoint sweep only (a4), on the trajectories the last forward sweep stored. */
+/* (mode 2, the adjoint sweep alone, belongs to the forward sweep before it: on wavefront layouts it ADDS lambda^0 to the
+ * control-level part of the gradient that the forward sweep's cost kernel left behind; one adjoint sweep per forward sweep.) */
 int dd4dvar_sweep_async(dd4dvar_t h, int mode);
 
 /* Copy the current local controls of all subdomains ("all subdomains" array, physical units). */

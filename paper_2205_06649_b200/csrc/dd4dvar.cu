@@ -29,6 +29,7 @@ namespace {
 constexpr int NT_GK = 256;     // generic kernels: threads per block
 constexpr int NT_RED = 256;    // cost reduction
 constexpr int NT_LB = 512;     // L-BFGS CTA
+constexpr int EH_CHUNKS = 4;   // eval_local_host: chunks of subdomains whose copies overlap the sweeps of the others
 
 struct Arena {
     char* base = nullptr;
@@ -81,6 +82,7 @@ struct Layout {
     double *w = nullptr, *wt = nullptr, *g = nullptr, *gn = nullptr, *d = nullptr, *S = nullptr, *Y = nullptr;
     LbfgsState st{};
     int* okmask = nullptr;
+    int* cmask = nullptr;               // [EH_CHUNKS][nsub] subdomain masks of the chunks of eval_local_host
     // observations binned per (subdomain, local level)
     bool have_obs = false;
     long long* obs_start = nullptr;
@@ -117,6 +119,9 @@ struct dd4dvar_s {
     bool history_global = true;         // evaluate J of eq (6) at the gathered analysis after every outer iteration
     void* ws = nullptr;
     size_t ws_bytes = 0;
+    // eval_local_host: copy streams and events (created on first use, destroyed with the handle)
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_in = nullptr, ev_h2d[EH_CHUNKS] = {}, ev_sw[EH_CHUNKS] = {}, ev_out = nullptr;
     int* h_pin = nullptr;               // pinned scratch for small read-backs
     std::vector<double> h_tmp;
 };
@@ -274,6 +279,7 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
     L.Jev = ar.take<double>(L.nsub);
     L.dmax = ar.take<double>(L.nsub);
     L.okmask = ar.take<int>(L.nsub);
+    L.cmask = ar.take<int>((size_t)EH_CHUNKS * L.nsub);
     if (L.lbfgs) {
         L.w = ar.take<double>(L.ctot); L.wt = ar.take<double>(L.ctot); L.g = ar.take<double>(L.ctot);
         L.gn = ar.take<double>(L.ctot); L.d = ar.take<double>(L.ctot);
@@ -334,6 +340,12 @@ int upload_layout(dd4dvar_t h, Layout& L)
     const size_t o_ei0 = put(L.tc_ei0), o_ex = put(L.tc_ex), o_ej0 = put(L.tr_ej0), o_ey = put(L.tr_ey);
     const size_t o_wb = put(L.wb);
     CU(cudaMemcpyAsync(L.itab, t.data(), sizeof(int) * t.size(), cudaMemcpyHostToDevice, h->stream));
+    {
+        std::vector<int> cm((size_t)EH_CHUNKS * L.nsub, 0);
+        for (int k = 0; k < L.nsub; ++k) cm[(size_t)((long long)k * EH_CHUNKS / L.nsub) * L.nsub + k] = 1;
+        CU(cudaMemcpyAsync(L.cmask, cm.data(), sizeof(int) * cm.size(), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
     CU(cudaStreamSynchronize(h->stream));
     GeoP& g = L.geo;
     g.nlon = nlon; g.nlat = nlat; g.p1 = L.p1; g.p2 = L.p2; g.q = L.q;
@@ -894,10 +906,51 @@ int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_cos
     if (!h || !h_controls || !h_costs) return fail(h, -1, "eval_local_host: null argument");
     if (!h->have_bg) return fail(h, -3, "eval_local_host before set_background");
     Layout& L = h->L;
-    CU(cudaMemcpyAsync(L.x, h_controls, sizeof(double) * L.ctot, cudaMemcpyHostToDevice, h->stream));
-    sweep(h, L, h_grads != nullptr, nullptr, L.Jev, nullptr);
-    CU(cudaMemcpyAsync(h_costs, L.Jev, sizeof(double) * L.nsub, cudaMemcpyDeviceToHost, h->stream));
-    if (h_grads) CU(cudaMemcpyAsync(h_grads, L.gx, sizeof(double) * L.ctot, cudaMemcpyDeviceToHost, h->stream));
+    if (L.nsub < 16 * EH_CHUNKS) {              // small problems: one copy in, one sweep, one copy out
+        CU(cudaMemcpyAsync(L.x, h_controls, sizeof(double) * L.ctot, cudaMemcpyHostToDevice, h->stream));
+        sweep(h, L, h_grads != nullptr, nullptr, L.Jev, nullptr);
+        CU(cudaMemcpyAsync(h_costs, L.Jev, sizeof(double) * L.nsub, cudaMemcpyDeviceToHost, h->stream));
+        if (h_grads) CU(cudaMemcpyAsync(h_grads, L.gx, sizeof(double) * L.ctot, cudaMemcpyDeviceToHost, h->stream));
+    } else {
+        // Subdomains are independent inside one evaluation (all neighbour data is frozen), so the evaluation runs in
+        // EH_CHUNKS chunks of consecutive subdomains: the host -> device copy of chunk c+1 and the device -> host copy
+        // of chunk c-1 overlap the sweep of chunk c (two copy streams, masked sweeps on the caller's stream).
+        if (!h->s_h2d) {
+            CU(cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking));
+            CU(cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking));
+            CU(cudaEventCreateWithFlags(&h->ev_in, cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&h->ev_out, cudaEventDisableTiming));
+            for (int c = 0; c < EH_CHUNKS; ++c) {
+                CU(cudaEventCreateWithFlags(&h->ev_h2d[c], cudaEventDisableTiming));
+                CU(cudaEventCreateWithFlags(&h->ev_sw[c], cudaEventDisableTiming));
+            }
+        }
+        CU(cudaEventRecord(h->ev_in, h->stream));                       // the copies start after the caller's earlier work
+        CU(cudaStreamWaitEvent(h->s_h2d, h->ev_in, 0));
+        CU(cudaStreamWaitEvent(h->s_d2h, h->ev_in, 0));
+        int kb[EH_CHUNKS + 1];
+        for (int c = 0; c <= EH_CHUNKS; ++c) {                          // chunk c = subdomains with k * EH_CHUNKS / nsub == c
+            int k = (int)(((long long)c * L.nsub + EH_CHUNKS - 1) / EH_CHUNKS);
+            kb[c] = k > L.nsub ? L.nsub : k;
+        }
+        auto off = [&](int k) { return k < L.nsub ? L.hs[k].coff : L.ctot; };
+        for (int c = 0; c < EH_CHUNKS; ++c) {
+            const long long o0 = off(kb[c]), o1 = off(kb[c + 1]);
+            CU(cudaMemcpyAsync(L.x + o0, h_controls + o0, sizeof(double) * (o1 - o0), cudaMemcpyHostToDevice, h->s_h2d));
+            CU(cudaEventRecord(h->ev_h2d[c], h->s_h2d));
+        }
+        for (int c = 0; c < EH_CHUNKS; ++c) {
+            const long long o0 = off(kb[c]), o1 = off(kb[c + 1]);
+            CU(cudaStreamWaitEvent(h->stream, h->ev_h2d[c], 0));
+            sweep(h, L, h_grads != nullptr, L.cmask + (size_t)c * L.nsub, L.Jev, nullptr);
+            CU(cudaEventRecord(h->ev_sw[c], h->stream));
+            CU(cudaStreamWaitEvent(h->s_d2h, h->ev_sw[c], 0));
+            CU(cudaMemcpyAsync(h_costs + kb[c], L.Jev + kb[c], sizeof(double) * (kb[c + 1] - kb[c]), cudaMemcpyDeviceToHost, h->s_d2h));
+            if (h_grads) CU(cudaMemcpyAsync(h_grads + o0, L.gx + o0, sizeof(double) * (o1 - o0), cudaMemcpyDeviceToHost, h->s_d2h));
+        }
+        CU(cudaEventRecord(h->ev_out, h->s_d2h));
+        CU(cudaStreamWaitEvent(h->stream, h->ev_out, 0));
+    }
     int rc = sync_check(h);
     if (rc) return rc;
     for (int k = 0; k < L.nsub; ++k)
@@ -1194,6 +1247,12 @@ void dd4dvar_destroy(dd4dvar_t h)
 {
     if (!h) return;
     fused_teardown(h->stream, h->L.fp);
+    if (h->s_h2d) {
+        cudaStreamSynchronize(h->s_h2d); cudaStreamSynchronize(h->s_d2h);
+        cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
+        cudaEventDestroy(h->ev_in); cudaEventDestroy(h->ev_out);
+        for (int c = 0; c < EH_CHUNKS; ++c) { cudaEventDestroy(h->ev_h2d[c]); cudaEventDestroy(h->ev_sw[c]); }
+    }
     delete h;
 }
 

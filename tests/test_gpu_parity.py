@@ -287,3 +287,24 @@ def test_history_global_switch_changes_only_the_diagnostic_column():
     assert np.all(np.isnan(h2[:, 0])) and np.all(np.isfinite(h1[:, 0]))
     assert np.array_equal(h1[:, 1:], h2[:, 1:])
     assert np.array_equal(an1.cpu().numpy(), an2.cpu().numpy())
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_eval_local_host_equals_eval_local(cfg):
+    """The host-buffer entry point (copies inside the call; chunked and overlapped with the sweeps from 64
+    subdomains on) returns exactly what the device-buffer entry point returns."""
+    import torch
+    w = synth.CONFIGS[cfg]
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    xs = perturbed_controls(o, prob, 5)
+    flat = g.pack(xs)
+    costs, parts, grads = g.eval_local(flat)
+    h_ctrl = flat.cpu().pin_memory()
+    h_grad = torch.empty_like(h_ctrl).pin_memory()
+    h_cost = np.zeros(g.nsub)
+    for _ in range(2):
+        h_grad.zero_(); h_cost[:] = 0
+        g.eval_local_host(h_ctrl, h_cost, h_grad)
+        assert np.array_equal(h_cost, costs)
+        assert np.array_equal(h_grad.numpy(), grads.cpu().numpy())
