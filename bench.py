@@ -288,6 +288,42 @@ def run_driver(args):
     g.close()
 
 
+def run_sharded(args):
+    """Algorithm 1 with the time windows sharded over the ranks (paper_2205_06649_b200/parallel.py): time per outer
+    iteration, total work fixed ("strong").  One process per GPU under torchrun; N = 1 runs the same driver."""
+    import torch
+    import torch.distributed as dist
+    from paper_2205_06649_b200.parallel import ShardedDD4DVar
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    w = workload(args.config)
+    sh = ShardedDD4DVar(w, device=f"cuda:{local_rank}", path=args.path)
+    prob = synth.make_problem(w, sh.g.forecast)
+    sh.set_background(prob.xb, prob.sigma_b); sh.set_observations(prob.obs)
+    outer = args.outer if args.outer is not None else 3
+    sh.run(1)                                           # warm-up iteration
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(dev); t0 = time.perf_counter()
+    an, hist = sh.run(outer)
+    torch.cuda.synchronize(dev); dt = time.perf_counter() - t0
+    (dt,) = max_over_ranks([dt], dev)
+    if rank == 0:
+        print(json.dumps({"metric": "outer iterations of Algorithm 1 per second, windows sharded over the GPUs", "value": outer / dt,
+                          "unit": "outer iterations/s", "n_gpus": world, "scaling": "strong", "ms_per_outer_iteration": 1e3 * dt / outer,
+                          "config": {"workload": w.name, "windows_per_rank": [b[1] - b[0] for b in
+                                     __import__("paper_2205_06649_b200.parallel", fromlist=["x"]).window_blocks(w.q_time, world)],
+                                     "exchange_bytes_per_iteration": int(2 * 8 * sh.g.ctot)},
+                          "sumJ_local": [float(x) for x in hist[:, 0]], "delta": [float(x) for x in hist[:, 1]]}))
+    sh.close()
+    if world > 1:
+        dist.barrier(); dist.destroy_process_group()
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: time-to-analysis and grid-point.steps/s per layout on the fixed
     0.5 deg / 128-step problem (one JSON line per layout; the paper's time-complexity analysis)."""
@@ -340,6 +376,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 row-marching, 3 per-stage, 4 wavefront fwd + row-marching adj, 5 wavefront")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
+    ap.add_argument("--shard", action="store_true", help="Algorithm 1 with the time windows sharded over the ranks (torchrun, one per GPU)")
     ap.add_argument("--gn", action="store_true", help="with --run: Gauss-Newton + CG local minimiser (dd4dvar_run_gn)")
     ap.add_argument("--n-gn", type=int, default=2)
     ap.add_argument("--n-cg", type=int, default=5)
@@ -363,6 +400,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
         run_sweep(args)
+        return
+    if args.shard:
+        run_sharded(args)
         return
     if args.run:
         run_driver(args)

@@ -209,6 +209,23 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later);
  * Algorithm 1).  on = 0: skip it, column 0 is NaN; default on. */
 int dd4dvar_set_history_global(dd4dvar_t h, int on);
 
+/* Sharded runs, one process per GPU: within an outer iteration the local problems are independent
+ * (eq (37) l.433) and there is one exchange step per outer iteration (Alg 1 l.465).  Every process holds the whole
+ * problem and OWNS the subdomains of the time windows [j0, j1): dd4dvar_run moves only those; its exchange freezes the
+ * controls of the owned subdomains and the end states of the owned windows.  After every dd4dvar_run(h, 1, ...) the
+ * caller completes the exchange between the processes on the two buffers of dd4dvar_exchange_buffer (device pointers
+ * into the workspace, "all subdomains" control layout): which = 0 frozen controls, owner = the subdomain's own window;
+ * which = 1 predecessor end states, owner = the window BEFORE the subdomain's.  Spatial neighbours share a window, so
+ * the ghost-ring store never crosses processes.  In a sharded run the history rows of dd4dvar_run are local (column 0
+ * needs dd4dvar_set_history_global(h, 0)); dd4dvar_get_local_stats returns J_ji and |u_ji^l - u_ji^(l-1)|_inf per
+ * subdomain (valid for the owned ones) for the caller's reductions, dd4dvar_gather_analysis the analysis (eq (12)-(13)
+ * l.194-201) from the frozen controls.  paper_2205_06649_b200/parallel.py drives this with torch.distributed.
+ * set_owned_windows: after set_workspace; (0, q_time) switches sharding off.  dd4dvar_run_gn is not sharded (-2). */
+int dd4dvar_set_owned_windows(dd4dvar_t h, int j0, int j1);
+int dd4dvar_exchange_buffer(dd4dvar_t h, int which, void** d_ptr, long long* count);
+int dd4dvar_get_local_stats(dd4dvar_t h, double* h_J, double* h_dmax);
+int dd4dvar_gather_analysis(dd4dvar_t h, double* d_analysis);
+
 /* The spatial overlap penalty (25c) case 1 l.310-314 acts on the control level of the window (R12, the
  * default).  on = 1: on every level of the window, eq (21) l.300 read literally (O_ik maps onto Delta_j x (Omega_i n
  * Omega_k)); the neighbours' frozen trajectories on the overlap rectangles are then kept in a second store,

@@ -51,7 +51,8 @@ EXPORTS = [
     "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
-    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global", "dd4dvar_set_overlap_levels",
+    "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global", "dd4dvar_set_overlap_levels", "dd4dvar_set_owned_windows", "dd4dvar_exchange_buffer",
+    "dd4dvar_get_local_stats", "dd4dvar_gather_analysis",
     "dd4dvar_last_error", "dd4dvar_destroy",
 ]
 
@@ -97,6 +98,10 @@ def load_library():
     lib.dd4dvar_set_bg_weight.argtypes = [vp, C.c_double]
     lib.dd4dvar_set_history_global.argtypes = [vp, C.c_int]
     lib.dd4dvar_set_overlap_levels.argtypes = [vp, C.c_int]
+    lib.dd4dvar_set_owned_windows.argtypes = [vp, C.c_int, C.c_int]
+    lib.dd4dvar_exchange_buffer.argtypes = [vp, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_longlong)]
+    lib.dd4dvar_get_local_stats.argtypes = [vp, hd, hd]
+    lib.dd4dvar_gather_analysis.argtypes = [vp, dp]
     lib.dd4dvar_last_error.restype = C.c_char_p
     lib.dd4dvar_last_error.argtypes = [vp]
     lib.dd4dvar_destroy.restype = None
@@ -313,6 +318,28 @@ class DD4DVar:
         self._check("dd4dvar_gn_hessvec", self.lib.dd4dvar_gn_hessvec(self._h, controls.data_ptr(), p.data_ptr(),
                                                                       out.data_ptr()))
         return out
+
+    # ---- sharded runs (one process per GPU owns a block of time windows; see parallel.py)
+    def set_owned_windows(self, j0, j1):
+        self._check("dd4dvar_set_owned_windows", self.lib.dd4dvar_set_owned_windows(self._h, int(j0), int(j1)))
+
+    def exchange_view(self, which):
+        """fp64 view (no copy) of an exchange buffer inside the workspace: 0 frozen controls, 1 predecessor end states."""
+        ptr = C.c_void_p(); cnt = C.c_longlong()
+        self._check("dd4dvar_exchange_buffer", self.lib.dd4dvar_exchange_buffer(self._h, int(which), C.byref(ptr), C.byref(cnt)))
+        off = ptr.value - self._ws.data_ptr()
+        assert off >= 0 and off % 8 == 0 and off + 8 * cnt.value <= self._ws.numel()
+        return self._ws[off:off + 8 * cnt.value].view(self.torch.float64)
+
+    def local_stats(self):
+        J = np.zeros(self.nsub); dm = np.zeros(self.nsub)
+        self._check("dd4dvar_get_local_stats", self.lib.dd4dvar_get_local_stats(self._h, _hd(J), _hd(dm)))
+        return J, dm
+
+    def gather_analysis(self):
+        an = self.torch.empty(self.shape, dtype=self.torch.float64, device=self.device)
+        self._check("dd4dvar_gather_analysis", self.lib.dd4dvar_gather_analysis(self._h, an.data_ptr()))
+        return an
 
     def set_overlap_levels(self, on):
         """(25c) case 1 on every level of the window (generic kernels only; before set_background)."""

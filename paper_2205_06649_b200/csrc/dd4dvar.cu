@@ -82,7 +82,10 @@ struct Layout {
     double *w = nullptr, *wt = nullptr, *g = nullptr, *gn = nullptr, *d = nullptr, *S = nullptr, *Y = nullptr;
     LbfgsState st{};
     int* okmask = nullptr;
-    int* cmask = nullptr;               // [EH_CHUNKS][nsub] subdomain masks of the chunks of eval_local_host
+    int* cmask = nullptr;
+    int *own = nullptr, *notown = nullptr;  // sharded runs: 1 for the subdomains this process owns / does not own
+    bool sharded = false;
+    int own_j0 = 0, own_j1 = 0;               // [EH_CHUNKS][nsub] subdomain masks of the chunks of eval_local_host
     // observations binned per (subdomain, local level)
     bool have_obs = false;
     long long* obs_start = nullptr;
@@ -280,6 +283,7 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
     L.dmax = ar.take<double>(L.nsub);
     L.okmask = ar.take<int>(L.nsub);
     L.cmask = ar.take<int>((size_t)EH_CHUNKS * L.nsub);
+    L.own = ar.take<int>(L.nsub); L.notown = ar.take<int>(L.nsub);
     if (L.lbfgs) {
         L.w = ar.take<double>(L.ctot); L.wt = ar.take<double>(L.ctot); L.g = ar.take<double>(L.ctot);
         L.gn = ar.take<double>(L.ctot); L.d = ar.take<double>(L.ctot);
@@ -543,7 +547,8 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
 // Alg 1 l.465: this iteration's results become the next one's frozen data
 void exchange(dd4dvar_t h, Layout& L)
 {
-    LAUNCH(xk_freeze<NT_RED>, L.nsub, NT_RED, L.dsubs, L.geo, L.traj, L.x, L.xfrozen, L.pred_end, L.dmax);
+    LAUNCH(xk_freeze<NT_RED>, L.nsub, NT_RED, L.dsubs, L.geo, L.traj, L.x, L.xfrozen, L.pred_end, L.dmax,
+           L.sharded ? (const int*)L.own : (const int*)nullptr);
     if (L.maxnring > 0)
         LAUNCH(xk_ghost_fill, dim3((L.maxnring + 127) / 128, L.nsub, std::min(L.Wmax, 8)), 128, L.dsubs, L.geo,
                L.traj, L.ghost);
@@ -1019,6 +1024,7 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
     Layout& L = h->L; Layout& G = h->G;
     const int n1 = h->grid.nlon * h->grid.nlat;
     const int nsub = L.nsub;
+    const int* own = L.sharded ? L.own : nullptr;       // sharded runs: only the subdomains of the owned windows move
     LbfgsP lp; lp.m = h->opt.lbfgs_m; lp.max_bt = h->opt.max_backtrack; lp.c1 = h->opt.armijo_c1; lp.ctot = L.ctot;
     h->h_tmp.resize(std::max(nsub, 8));
     int rc;
@@ -1038,19 +1044,20 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
     h_history[1] = 0.0; h_history[2] = 0.0;
     const dim3 vgrid(std::min(64, (3 * L.maxncell + 255) / 256), nsub);
     if (outer_iters == 0) {
-        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
-        sweep(h, L, false, nullptr, L.st.J, nullptr);
+        sweep(h, L, false, own, L.st.J, nullptr);
         if ((rc = sumJ(L.st.J, &h_history[1]))) return rc;
     }
     for (int l = 1; l <= outer_iters; ++l) {
         // local functional changed: clear the history (R10), evaluate J_ji and its gradient at w
         CU(cudaMemsetAsync(L.st.nh, 0, sizeof(int) * nsub, h->stream));
         CU(cudaMemsetAsync(L.st.head, 0, sizeof(int) * nsub, h->stream));
-        CU(cudaMemsetAsync(L.st.done, 0, sizeof(int) * nsub, h->stream));
-        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+        if (own) CU(cudaMemcpyAsync(L.st.done, L.notown, sizeof(int) * nsub, cudaMemcpyDeviceToDevice, h->stream));
+        else CU(cudaMemsetAsync(L.st.done, 0, sizeof(int) * nsub, h->stream));
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
-        sweep(h, L, true, nullptr, L.st.J, L.g);
+        sweep(h, L, true, own, L.st.J, L.g);
         if (l == 1 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
         for (int it = 0; it < h->opt.n_inner; ++it) {
             LAUNCH(lk_direction<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.g, L.S, L.Y, L.d);
@@ -1070,9 +1077,9 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
             LAUNCH(lk_update<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.w, L.wt, L.g, L.gn, L.S, L.Y);
         }
         // one more forward sweep so that the stored trajectory belongs to the accepted iterate
-        LAUNCH(lk_trial, vgrid, 256, L.dsubs, (const int*)nullptr, h->cp, (const double*)nullptr, L.w,
+        LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
-        sweep(h, L, false, nullptr, L.Jev, nullptr);
+        sweep(h, L, false, own, L.Jev, nullptr);
         if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
         exchange(h, L);
         CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
@@ -1136,6 +1143,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
     if (!h->have_bg) return fail(h, -3, "run_gn before set_background");
     Layout& L = h->L; Layout& G = h->G;
     if (L.path != 5) return fail(h, -2, "run_gn: the Gauss-Newton solver needs a wavefront layout (path 5)");
+    if (L.sharded) return fail(h, -2, "run_gn: not available in sharded runs (dd4dvar_set_owned_windows)");
     const int n1 = h->grid.nlon * h->grid.nlat;
     const int nsub = L.nsub;
     h->h_tmp.resize(std::max(nsub, 8));
@@ -1198,6 +1206,52 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
     if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
     h->cp.bgw = w_later;
     return 0;
+}
+
+// ---- sharded runs: one process per GPU owns a block of time windows -------------
+int dd4dvar_set_owned_windows(dd4dvar_t h, int j0, int j1)
+{
+    if (!h) return -1;
+    if (!h->have_ws) return fail(h, -3, "set_owned_windows before set_workspace");
+    Layout& L = h->L;
+    if (j0 < 0 || j1 > L.q || j0 >= j1) return fail(h, -1, "set_owned_windows: need 0 <= j0 < j1 <= q_time");
+    std::vector<int> own(L.nsub), notown(L.nsub);
+    for (int k = 0; k < L.nsub; ++k) { own[k] = L.hs[k].jw >= j0 && L.hs[k].jw < j1; notown[k] = !own[k]; }
+    CU(cudaMemcpyAsync(L.own, own.data(), sizeof(int) * L.nsub, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(L.notown, notown.data(), sizeof(int) * L.nsub, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    L.sharded = !(j0 == 0 && j1 == L.q); L.own_j0 = j0; L.own_j1 = j1;
+    return 0;
+}
+
+int dd4dvar_exchange_buffer(dd4dvar_t h, int which, void** d_ptr, long long* count)
+{
+    if (!h || !d_ptr || !count) return -1;
+    if (!h->have_ws) return fail(h, -3, "exchange_buffer before set_workspace");
+    Layout& L = h->L;
+    switch (which) {
+    case 0: *d_ptr = L.xfrozen; *count = L.ctot; return 0;
+    case 1: *d_ptr = L.pred_end; *count = L.ctot; return 0;
+    default: return fail(h, -1, "exchange_buffer: which = 0 (frozen controls) or 1 (predecessor end states)");
+    }
+}
+
+int dd4dvar_get_local_stats(dd4dvar_t h, double* h_J, double* h_dmax)
+{
+    if (!h || !h_J || !h_dmax) return fail(h, -1, "get_local_stats: null argument");
+    if (!h->have_bg) return fail(h, -3, "get_local_stats before set_background");
+    CU(cudaMemcpyAsync(h_J, h->L.st.J, sizeof(double) * h->L.nsub, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaMemcpyAsync(h_dmax, h->L.dmax, sizeof(double) * h->L.nsub, cudaMemcpyDeviceToHost, h->stream));
+    return sync_check(h);
+}
+
+int dd4dvar_gather_analysis(dd4dvar_t h, double* d_analysis)
+{
+    if (!h || !d_analysis) return fail(h, -1, "gather_analysis: null argument");
+    if (!h->have_bg) return fail(h, -3, "gather_analysis before set_background");
+    const int n1 = h->grid.nlon * h->grid.nlat;
+    LAUNCH(xk_gather, (n1 + 255) / 256, 256, h->L.dsubs, h->L.geo, 1, 0, h->L.xfrozen, d_analysis);
+    return sync_check(h);
 }
 
 int dd4dvar_set_overlap_levels(dd4dvar_t h, int on)

@@ -43,26 +43,31 @@ __global__ void xk_ghost_fill(const Sub* __restrict__ subs, GeoP geo, const doub
 template <int NT>
 __global__ void xk_freeze(const Sub* __restrict__ subs, GeoP geo, const double* __restrict__ traj,
                           const double* __restrict__ x, double* __restrict__ xfrozen,
-                          double* __restrict__ pred_end, double* __restrict__ dmax)
+                          double* __restrict__ pred_end, double* __restrict__ dmax, const int* __restrict__ own)
 {
+    // own (sharded runs, dd4dvar_set_owned_windows): this process freezes the controls of the subdomains it owns and
+    // the end states of the windows it owns (= pred_end of their successors); the rest is imported from the owners
     __shared__ double sh[32];
     const int k = blockIdx.x;
     const Sub s = subs[k];
     const int n3 = DD_NF * s.ncell;
+    const bool mine = !own || own[k];
     double mx = 0.0;
     const double* tp = nullptr;
-    if (s.jw > 0) {
+    if (s.jw > 0 && (!own || own[k - geo.p1 * geo.p2])) {
         const Sub& sp = subs[k - geo.p1 * geo.p2];
         tp = traj + sp.toff + (long long)sp.W * DD_NF * sp.ncell;
     }
     for (int q = threadIdx.x; q < n3; q += NT) {
-        const double xn = x[s.coff + q];
-        mx = fmax(mx, fabs(xn - xfrozen[s.coff + q]));
-        xfrozen[s.coff + q] = xn;
+        if (mine) {
+            const double xn = x[s.coff + q];
+            mx = fmax(mx, fabs(xn - xfrozen[s.coff + q]));
+            xfrozen[s.coff + q] = xn;
+        }
         if (tp) pred_end[s.coff + q] = tp[q];
     }
     mx = block_max<NT>(mx, sh);
-    if (threadIdx.x == 0) dmax[k] = mx;
+    if (threadIdx.x == 0 && mine) dmax[k] = mx;
 }
 
 // traj[k][n] <- restriction of global level s_k + n (source = the undecomposed layout's store)
