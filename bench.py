@@ -324,6 +324,46 @@ def run_sharded(args):
         dist.barrier(); dist.destroy_process_group()
 
 
+def run_table3(args):
+    """The shape of the paper's weak-scaling experiment (Table 3; eq (57)): local problems of
+    fixed size n_loc = 32 (owned 32x32 cells, overlap 2, 16-step windows), QP = 2 ... 4096 subdomains, here all on ONE
+    GPU: time of one gradient sweep of all QP local problems and the software scale-up QP * T(one local problem) / T(QP),
+    with T(one local problem) taken from the QP = 2 run (its two subdomains run side by side on two SMs)."""
+    import dataclasses
+    import torch
+    from paper_2205_06649_b200.binding import DD4DVar
+    dev = torch.device("cuda", 0)
+    layouts = [(2, 1, 1), (2, 2, 1), (2, 2, 2), (4, 2, 2), (4, 4, 2), (4, 4, 4), (8, 4, 4), (8, 8, 4), (8, 8, 8), (16, 8, 8),
+               (16, 16, 8), (32, 16, 8)]
+    t1 = None
+    for (p1, p2, q) in layouts:
+        nlon, nlat, nsteps = 32 * p1, 32 * p2, 16 * q
+        deg = 360.0 / nlon
+        w = synth.Workload(90, nlon, nlat, min(600.0, 300.0 * deg), nsteps, 5, 0.05, 4, p1, p2, q, 2, 1,
+                           name=f"table3 n_loc=32 {p1}x{p2}x{q}")
+        g = DD4DVar.from_workload(w, device="cuda:0", path=args.path)
+        prob = synth.make_problem(w, g.forecast)
+        g.set_background(prob.xb, prob.sigma_b); g.set_observations(prob.obs)
+        for _ in range(3):
+            g.sweep_async(1)
+        torch.cuda.synchronize(dev)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        n = 10
+        ev[0].record()
+        for _ in range(n):
+            g.sweep_async(1)
+        ev[1].record(); torch.cuda.synchronize(dev)
+        ms = ev[0].elapsed_time(ev[1]) / n
+        if t1 is None:
+            t1 = ms
+        qp = p1 * p2 * q
+        print(json.dumps({"table": 3, "QP": qp, "layout": f"{p1}x{p2}x{q}", "grid": f"{nlon}x{nlat}", "steps": nsteps,
+                          "problem_size": 3 * 32 * 32 * qp, "path": PATH_NAMES.get(g.active_path, str(g.active_path)).split("(")[0].strip(),
+                          "sweep_ms": ms, "scale_up": qp * t1 / ms,
+                          "useful_point_steps_per_s": nlon * nlat * nsteps / (ms * 1e-3)}), flush=True)
+        g.close()
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: time-to-analysis and grid-point.steps/s per layout on the fixed
     0.5 deg / 128-step problem (one JSON line per layout; the paper's time-complexity analysis)."""
@@ -376,6 +416,7 @@ def main():
     ap.add_argument("--path", type=int, default=0, help="0 auto, 1 generic, 2 row-marching, 3 per-stage, 4 wavefront fwd + row-marching adj, 5 wavefront")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--run", action="store_true", help="time the whole driver: run(outer_iters) on --config")
+    ap.add_argument("--table3", action="store_true", help="the paper's weak-scaling shape (Table 3): n_loc = 32, QP = 2 ... 4096 local problems on one GPU")
     ap.add_argument("--shard", action="store_true", help="Algorithm 1 with the time windows sharded over the ranks (torchrun, one per GPU)")
     ap.add_argument("--gn", action="store_true", help="with --run: Gauss-Newton + CG local minimiser (dd4dvar_run_gn)")
     ap.add_argument("--n-gn", type=int, default=2)
@@ -400,6 +441,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.sweep:
         run_sweep(args)
+        return
+    if args.table3:
+        run_table3(args)
         return
     if args.shard:
         run_sharded(args)
@@ -500,6 +544,7 @@ def main():
     e2e_s = (time.perf_counter() - t0) / e2e_steps
 
     # one outer iteration of Algorithm 1 (a5 L-BFGS + a6 exchange + the sweeps it needs), reported
+    g.run(1)                                         # (untimed: first use of the driver's kernels)
     torch.cuda.synchronize(dev)
     t0 = time.perf_counter()
     g.run(1)
@@ -535,7 +580,7 @@ def main():
                        "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "outer_iteration_ms": 1e3 * outer_s, "outer_iteration_ms_without_global_history": 1e3 * outer_ng_s,
-                       "outer_iteration": "run(1): 5 L-BFGS iterations (a5) + exchange (a6) + J_global, not in the timed region"},
+                       "outer_iteration": "run(1) after one untimed run(1): 5 L-BFGS iterations (a5) + exchange (a6) + J_global, not in the timed region"},
             "clocks": clocks,
             "e2e": {"value": world * useful / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.ctot * 8),
                     "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
