@@ -118,6 +118,7 @@ struct dd4dvar_s {
     double sig_o[3] = { 1, 1, 1 };
     Layout G, L;
     bool have_ws = false, have_bg = false;
+    int coop_grid = 0;                  // resident CTAs of sk_forward_multi (0: cooperative launch not available)
     bool overlap_levels = false;        // (25c) case 1 on every level of the window (generic path only)
     bool history_global = true;         // evaluate J of eq (6) at the gathered analysis after every outer iteration
     void* ws = nullptr;
@@ -382,6 +383,18 @@ void forward_generic(dd4dvar_t h, Layout& L, const int* mask)
     // level 0 of the store = the control
     LAUNCH(gk_store_control, cell_grid(L), NT_GK, L.dsubs, mask, L.x, L.traj);
     if (L.path != 3) {
+        if (h->coop_grid > 0 && L.Wmax > 1) {
+            // all steps in one cooperative launch (grid-wide barrier between the steps)
+            const Sub* subs = L.dsubs; int n0 = 0, n1 = L.Wmax, tiles_x = L.tiles_x, ntiles = L.ntiles, nsub = L.nsub;
+            double* traj = L.traj; const double* ghost = L.ghost; ModelP mp = h->mp;
+            void* args[] = { &subs, &mask, &n0, &n1, &mp, &traj, &ghost, &tiles_x, &ntiles, &nsub };
+            const int grid = std::min(h->coop_grid, L.ntiles * L.nsub);
+            if (cudaLaunchCooperativeKernel((const void*)sk_forward_multi, dim3(grid), dim3(SK_NT), args, 0, h->stream) == cudaSuccess) {
+                ++h->launches;
+                return;
+            }
+            cudaGetLastError();                 // fall back to one launch per step
+        }
         for (int n = 0; n < L.Wmax; ++n)
             LAUNCH(sk_forward_step, dim3(L.ntiles, L.nsub), SK_NT, L.dsubs, mask, n, h->mp, L.traj, L.ghost, L.tiles_x);
         return;
@@ -670,6 +683,14 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
     if (cudaFuncSetAttribute(sk_adjoint_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(sizeof(double) * SK_ADJ_SMEM_DOUBLES)) != cudaSuccess)
         return fail(h, -4, "shared-memory opt-in of sk_adjoint_step failed");
+    {
+        int dev = 0, nsm = 0, coop = 0, per_sm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sk_forward_multi, SK_NT, 0) == cudaSuccess)
+            h->coop_grid = per_sm * nsm;
+    }
     if (cudaFuncSetAttribute(tk_step, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(sizeof(double) * TK_SMEM_DOUBLES)) != cudaSuccess)
         return fail(h, -4, "shared-memory opt-in of tk_step failed");

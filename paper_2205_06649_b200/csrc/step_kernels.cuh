@@ -5,6 +5,7 @@
 // kernels of generic_kernels.cuh need four to six, and are checked against them and the oracle.
 // Same ranges, same gather-form adjoint (model_math.cuh), same padded-array conventions.
 #pragma once
+#include <cooperative_groups.h>
 #include "common.cuh"
 #include "generic_kernels.cuh"
 #include "model_math.cuh"
@@ -49,27 +50,23 @@ __device__ __forceinline__ bool sk_range(const Reg& r, int k, int i, int j)
 }
 
 // ------------------------------------------------------------------------------------------
-// forward step n: Z^{n+1} = Phi(Z^n) on one 32x16 output tile
-__global__ void __launch_bounds__(SK_NT) sk_forward_step(const Sub* __restrict__ subs, const int* __restrict__ mask,
-                                                         int n, ModelP m, double* traj, const double* __restrict__ ghost,
-                                                         int tiles_x)
+// forward step n: Z^{n+1} = Phi(Z^n) on one 32x16 output tile (tx, ty) of subdomain s; shared memory: z0 [3][H0*W0],
+// za [3][H1*W1], h1 [H2*W2] (a caller that loops over tiles needs no barrier between two calls: the first
+// phase of a call writes z0 only, which the last phase of the previous call does not read)
+#define SK_FWD_SMEM_DOUBLES (3 * (SK_TY + 6) * (SK_TX + 6) + 3 * (SK_TY + 4) * (SK_TX + 4) + (SK_TY + 2) * (SK_TX + 2))
+__device__ __forceinline__ void sk_forward_tile(const Sub& s, int tx, int ty, int n, const ModelP& m, double* traj,
+                                                const double* __restrict__ ghost, double* __restrict__ z0,
+                                                double* __restrict__ za, double* __restrict__ h1)
 {
     constexpr int W0 = SK_TX + 6, H0 = SK_TY + 6, W1 = SK_TX + 4, H1 = SK_TY + 4, W2 = SK_TX + 2, H2 = SK_TY + 2;
-    __shared__ double z0[3][H0 * W0];
-    __shared__ double za[3][H1 * W1];
-    __shared__ double h1[H2 * W2];
-    const int k = blockIdx.y;
-    if (mask && !mask[k]) return;
-    const Sub s = subs[k];
-    if (n >= s.W) return;
+    constexpr int N0 = H0 * W0, N1 = H1 * W1;
     const Reg r = make_reg(s);
-    const int tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
     const int oi = s.gx + tx * SK_TX, oj = s.gys + ty * SK_TY;      // first output cell (padded coords)
     if (oi >= s.gx + s.ex || oj >= s.gys + s.ey) return;
     const double* t = traj + s.toff + (long long)n * DD_NF * s.ncell;
     const double* g = ghost + s.goff + (long long)n * DD_NF * s.nring;
     // ---- Z0 on the tile + 3
-    for (int c = threadIdx.x; c < H0 * W0; c += SK_NT) {
+    for (int c = threadIdx.x; c < N0; c += SK_NT) {
         const int lj = c / W0, li = c - lj * W0;
         const int i = oi - 3 + li, j = oj - 3 + lj;
         double v0 = 0.0, v1 = 0.0, v2 = 0.0;
@@ -77,23 +74,24 @@ __global__ void __launch_bounds__(SK_NT) sk_forward_step(const Sub* __restrict__
             const int iw = sk_wrap(r, i);
             v0 = sk_z0(s, r, t, g, 0, iw, j); v1 = sk_z0(s, r, t, g, 1, iw, j); v2 = sk_z0(s, r, t, g, 2, iw, j);
         }
-        z0[0][c] = v0; z0[1][c] = v1; z0[2][c] = v2;
+        z0[c] = v0; z0[N0 + c] = v1; z0[2 * N0 + c] = v2;
     }
     __syncthreads();
     // ---- stage A on the tile + 2 (range 1)
-    for (int c = threadIdx.x; c < H1 * W1; c += SK_NT) {
+    for (int c = threadIdx.x; c < N1; c += SK_NT) {
         const int lj = c / W1, li = c - lj * W1;
         const int i = oi - 2 + li, j = oj - 2 + lj;
         double a0 = 0.0, a1 = 0.0, a2 = 0.0;
         if (sk_range(r, 1, i, j)) {
             int jN, jS; double sN, sS; sk_ns(r, j, jN, jS, sN, sS);
             const int cc = (lj + 1) * W0 + li + 1, cN = (jN - oj + 3) * W0 + li + 1, cS = (jS - oj + 3) * W0 + li + 1;
-            const double cu = m.dtcz[r.joff + j] * z0[1][cc], cv = m.dtcm * z0[2][cc];
-            a0 = mm_stageA(z0[0][cc], z0[0][cc + 1], z0[0][cc - 1], z0[0][cN], z0[0][cS], cu, cv, m.kap);
-            a1 = mm_stageA(z0[1][cc], z0[1][cc + 1], z0[1][cc - 1], z0[1][cN], z0[1][cS], cu, cv, m.kap);
-            a2 = mm_stageA(z0[2][cc], z0[2][cc + 1], z0[2][cc - 1], sN * z0[2][cN], sS * z0[2][cS], cu, cv, m.kap);
+            const double* zh = z0; const double* zu = z0 + N0; const double* zv = z0 + 2 * N0;
+            const double cu = m.dtcz[r.joff + j] * zu[cc], cv = m.dtcm * zv[cc];
+            a0 = mm_stageA(zh[cc], zh[cc + 1], zh[cc - 1], zh[cN], zh[cS], cu, cv, m.kap);
+            a1 = mm_stageA(zu[cc], zu[cc + 1], zu[cc - 1], zu[cN], zu[cS], cu, cv, m.kap);
+            a2 = mm_stageA(zv[cc], zv[cc + 1], zv[cc - 1], sN * zv[cN], sS * zv[cS], cu, cv, m.kap);
         }
-        za[0][c] = a0; za[1][c] = a1; za[2][c] = a2;
+        za[c] = a0; za[N1 + c] = a1; za[2 * N1 + c] = a2;
     }
     __syncthreads();
     // ---- h1 on the tile + 1 (range 2)
@@ -105,9 +103,10 @@ __global__ void __launch_bounds__(SK_NT) sk_forward_step(const Sub* __restrict__
             int jN, jS; double sN, sS; sk_ns(r, j, jN, jS, sN, sS);
             const int cc = (lj + 1) * W1 + li + 1, cN = (jN - oj + 2) * W1 + li + 1, cS = (jS - oj + 2) * W1 + li + 1;
             const int gj = r.joff + j;
-            const double D = mm_div(za[1][cc + 1], za[1][cc - 1], sN * za[2][cN], sS * za[2][cS], m.dtcz[gj], m.dtcm,
+            const double* ua = za + N1; const double* va = za + 2 * N1;
+            const double D = mm_div(ua[cc + 1], ua[cc - 1], sN * va[cN], sS * va[cS], m.dtcz[gj], m.dtcm,
                                     m.rp[gj], m.rm[gj]);
-            v = mm_h1(za[0][cc], D);
+            v = mm_h1(za[cc], D);
         }
         h1[c] = v;
     }
@@ -123,10 +122,43 @@ __global__ void __launch_bounds__(SK_NT) sk_forward_step(const Sub* __restrict__
         const int ch = (lj + 1) * W2 + li + 1, chN = (jN - oj + 1) * W2 + li + 1, chS = (jS - oj + 1) * W2 + li + 1;
         const int gj = r.joff + j;
         const double dtf = m.dtf[gj], dtt = m.dtt[gj];
-        const double u1 = mm_u1(za[1][ca], za[2][ca], h1[ch + 1], h1[ch - 1], m.gdtcz[gj], dtf, dtt);
-        const double v1 = mm_v1(za[2][ca], u1, h1[chN], h1[chS], m.gdtcm, dtf, dtt);
+        const double u1 = mm_u1(za[N1 + ca], za[2 * N1 + ca], h1[ch + 1], h1[ch - 1], m.gdtcz[gj], dtf, dtt);
+        const double v1 = mm_v1(za[2 * N1 + ca], u1, h1[chN], h1[chS], m.gdtcm, dtf, dtt);
         const int lc = (j - s.gys) * s.ex + (i - s.gx);
         tn[lc] = h1[ch]; tn[s.ncell + lc] = u1; tn[2LL * s.ncell + lc] = v1;
+    }
+}
+__global__ void __launch_bounds__(SK_NT) sk_forward_step(const Sub* __restrict__ subs, const int* __restrict__ mask,
+                                                         int n, ModelP m, double* traj, const double* __restrict__ ghost,
+                                                         int tiles_x)
+{
+    __shared__ double smf[SK_FWD_SMEM_DOUBLES];
+    const int k = blockIdx.y;
+    if (mask && !mask[k]) return;
+    const Sub s = subs[k];
+    if (n >= s.W) return;
+    sk_forward_tile(s, blockIdx.x % tiles_x, blockIdx.x / tiles_x, n, m, traj, ghost, smf,
+                    smf + 3 * (SK_TY + 6) * (SK_TX + 6), smf + 3 * (SK_TY + 6) * (SK_TX + 6) + 3 * (SK_TY + 4) * (SK_TX + 4));
+}
+// The steps n0 .. n1-1 of every subdomain in ONE cooperative launch: persistent CTAs loop over the (subdomain, tile)
+// pairs of a step, a grid-wide barrier separates the steps (the undecomposed forecast of 256 steps is otherwise 256
+// launches of a 10-microsecond kernel).  Launched with cudaLaunchCooperativeKernel, grid <= resident CTAs.
+__global__ void __launch_bounds__(SK_NT) sk_forward_multi(const Sub* __restrict__ subs, const int* __restrict__ mask,
+                                                          int n0, int n1, ModelP m, double* traj,
+                                                          const double* __restrict__ ghost, int tiles_x, int ntiles, int nsub)
+{
+    __shared__ double smf[SK_FWD_SMEM_DOUBLES];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    for (int n = n0; n < n1; ++n) {
+        for (int q = blockIdx.x; q < ntiles * nsub; q += gridDim.x) {
+            const int k = q / ntiles, tile = q - k * ntiles;
+            if (mask && !mask[k]) continue;
+            const Sub s = subs[k];
+            if (n >= s.W) continue;
+            sk_forward_tile(s, tile % tiles_x, tile / tiles_x, n, m, traj, ghost, smf,
+                            smf + 3 * (SK_TY + 6) * (SK_TX + 6), smf + 3 * (SK_TY + 6) * (SK_TX + 6) + 3 * (SK_TY + 4) * (SK_TX + 4));
+        }
+        grid.sync();
     }
 }
 
