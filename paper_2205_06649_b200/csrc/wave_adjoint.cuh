@@ -36,6 +36,10 @@
 #pragma once
 #include "wave_common.cuh"
 
+#ifndef WK_APAIR
+#define WK_APAIR 1        // 1: the ticks without a pole-wall event run in pairs (no register moves); 0: one tick body + rotation (smaller code)
+#endif
+
 template <int K> struct WaState {     // every history has depth one: slot [t & 1] is written at tick t and read at tick t + 1
     double zc[2][3][K];             // [slot][field][column]: Z^{n-1} row t-1 (own columns), kept for one tick as row t-2
     double hz[2][3][2];             // E/W halo of rows t-1, t-2
@@ -589,6 +593,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                     else wa_tick<K, 0, false>(t, S, C, sm, tab);
                     wa_rotate<K>(S);
                 }
+#if WK_APAIR
                 if (ph == 0) {
 #pragma unroll 1
                     for (; t < tp1; t += 2) {
@@ -596,6 +601,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                         wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
                     }
                 }
+#endif
             }
             if (C.first) wk_cpa_wait<0>();
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);

@@ -25,6 +25,9 @@
 #pragma once
 #include "wave_common.cuh"
 
+#ifndef WK_FUNROLL
+#define WK_FUNROLL 1      // steady ticks per loop iteration: 1 (register moves, but the loop body stays inside the instruction cache: 3.28 ms), 3 (3.63 ms), 6 (6.67 ms); 0: no steady tick (3.87 ms)
+#endif
 #define WK_XD 3         // a first step fetches its control rows this many ticks ahead (4 mbarrier slots: WK_XD <= 3)
 
 
@@ -553,7 +556,31 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             const int ts1 = g.gys + g.ey - 1;
 #pragma unroll 1
             for (int t = 0; t < C.T;) {
-                if (t >= ts0 && t + 3 <= ts1) {
+#if WK_FUNROLL == 6
+                if (t >= ts0 && t + 6 <= ts1) {
+                    wf_tick_steady<K>(t, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 1, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 2, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 3, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 4, R, C, sm, tab);
+                    wf_tick_steady<K>(t + 5, R, C, sm, tab);
+                    t += 6;
+                    const int rowb = C.st + (t - 1 - g.gys) * C.P;
+                    R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
+                } else
+#endif
+#if WK_FUNROLL == 0
+                if (false) {
+                } else
+#elif WK_FUNROLL == 1
+                if (t >= ts0 && t + 1 <= ts1) {
+                    wf_tick_steady<K>(t, R, C, sm, tab);
+                    t += 1;
+                    const int rowb = C.st + (t - 1 - g.gys) * C.P;
+                    R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
+                } else
+#endif
+                if (WK_FUNROLL == 3 && t >= ts0 && t + 3 <= ts1) {
                     wf_tick_steady<K>(t, R, C, sm, tab);
                     wf_tick_steady<K>(t + 1, R, C, sm, tab);
                     wf_tick_steady<K>(t + 2, R, C, sm, tab);
