@@ -1,11 +1,10 @@
 // cost_kernels.cuh -- the control-level terms of the local functional J_ji (eq (25) l.338-344) for the
 // wavefront sweep kernels (wave_forward.cuh / wave_adjoint.cuh), one CTA per subdomain.
 //
-// wk_forward leaves the trajectory store, the misfits 2 c (H Z^n - y) of the levels n >= 1 (obs_r) and the
-// H (25b) cost of those levels per warp (obpart).  Everything of J_ji that needs only data in global
-// memory is evaluated here, in one bandwidth-bound pass over the control:
+// wk_forward leaves the trajectory store.  Every term of J_ji is evaluated here from data in global memory, in
+// one bandwidth-bound pass over the control plus the sparse samples of the trajectory at the observations:
 //   (25a) background term, weight 1/multiplicity (R6, R7)
-//   (25b) at level 0 (the control itself) and the sum of the warps' partial sums
+//   (25b) misfits, cost and the forcing 2 c (H Z^n - y) of the adjoint sweep (obs_r) at every level of the window
 //   (25c) spatial overlap with the frozen controls of the neighbour tiles (gather form: every cell
 //         looks up the rectangles that contain it), predecessor window, successor window (Z^W)
 // and, for the adjoint sweep that follows,
@@ -94,13 +93,26 @@ __global__ void __launch_bounds__(CK_NT, 5) ck_cost(const WkArgs A)
             gx[o] += r2;
         }
     }
+    // H (25b) at the levels 1 .. W: sampled from the trajectory store the forward sweep has just written
+    if (A.obs_start) {
+        for (int n = 1; n <= s.W; ++n) {
+            const long long a0 = A.obs_start[s.ooff + n], a1 = A.obs_start[s.ooff + n + 1];
+            const double* tn = A.traj + s.toff + (long long)n * 3 * nc;
+            for (long long q = a0 + tid; q < a1; q += CK_NT) {
+                const int pk = A.obs_lj[q];
+                const double rr = tn[(long long)((pk >> 8) & 3) * nc + (pk >> 12) * s.ex + (pk & 255)] - A.obs_y[q];
+                const double cq = A.obs_c[q];
+                ob += cq * rr * rr;
+                A.obs_r[q] = 2.0 * cq * rr;
+            }
+        }
+    }
     bg = block_sum<CK_NT>(bg, red);
     sp = block_sum<CK_NT>(sp, red);
     pr = block_sum<CK_NT>(pr, red);
     su = block_sum<CK_NT>(su, red);
     ob = block_sum<CK_NT>(ob, red);
     if (tid == 0) {
-        for (int q = 0; q < WK_NW; ++q) ob += A.obpart[(long long)k * WK_NW + q];
         const double v[5] = { bg, ob, A.cp.mu * sp, A.cp.mu * pr, A.cp.mu * su };
         double tot = 0.0;
         for (int q = 0; q < 5; ++q) { A.parts[k * 5 + q] = v[q]; tot += v[q]; }

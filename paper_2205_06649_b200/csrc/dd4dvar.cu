@@ -54,7 +54,6 @@ struct WavePlan {
     double* wtab = nullptr;             // [p2][maxpy + 2][8] row tables per tile row (wave_common.cuh)
     int wtab_stride = 0;
     double* lamW = nullptr;             // [ctot] adjoint variable at the window end (ck_cost -> wk_adjoint)
-    double* obpart = nullptr;           // [nsub][WK_NW] H (25b) cost per warp (wk_forward -> ck_cost)
 };
 
 struct Layout {
@@ -305,7 +304,6 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
         L.wp.wtab_stride = (L.wp.maxpy + 2) * 8;
         L.wp.wtab = ar.take<double>((size_t)L.p2 * L.wp.wtab_stride);
         L.wp.lamW = ar.take<double>(L.ctot);
-        L.wp.obpart = ar.take<double>((size_t)L.nsub * WK_NW);
         if (L.lbfgs) { L.gn_lamW = ar.take<double>(L.ctot); L.gn_gx = ar.take<double>(L.ctot); L.gn_Hp = ar.take<double>(L.ctot); }
     }
 }
@@ -456,7 +454,7 @@ WkArgs wave_args(dd4dvar_t h, Layout& L, const int* mask, double* Jout, double* 
     a.obs_y = L.obs_y; a.obs_c = L.obs_c; a.obs_r = L.obs_r;
     a.parts = L.parts; a.J = Jout; a.gx = L.gx; a.gw = gw;
     a.maxex = L.wp.maxex; a.maxey = L.wp.maxey; a.maxpx = L.wp.maxpx; a.maxpy = L.wp.maxpy;
-    a.wtab = L.wp.wtab; a.wtab_stride = L.wp.wtab_stride; a.lamW = L.wp.lamW; a.obpart = L.wp.obpart;
+    a.wtab = L.wp.wtab; a.wtab_stride = L.wp.wtab_stride; a.lamW = L.wp.lamW;
     a.Lf = wk_layout(false, a.maxex, a.maxey, a.maxpx, a.maxpy);
     a.La = wk_layout(true, a.maxex, a.maxey, a.maxpx, a.maxpy);
     return a;

@@ -95,7 +95,6 @@ struct WkArgs {
     int maxex, maxey, maxpx, maxpy;
     const double* wtab; int wtab_stride;    // row tables per tile row b: [p2][maxpy + 2][8] (entry r+1 <-> padded row r = -1 .. py)
     double* lamW;               // [ctot] adjoint variable at the window end, written by ck_cost: 2 mu (Z^W - x_succ) / sigma_b^2
-    double* obpart;             // [nsub][WK_NW] H (25b) cost of the steps each warp ran (levels 1 .. W)
     WkLayout Lf, La;            // shared-memory layouts (forward, adjoint), computed on the host: constant-bank operands
 };
 

@@ -18,8 +18,10 @@
 // and the leader's bulk store of every row this warp is about to overwrite has left shared memory).
 // The first step of a subdomain (n = 0) follows the LAST step of the previous subdomain of this CTA: its
 // input rows, the control, arrive from global memory two ticks ahead (TMA into the resident rows the
-// previous subdomain has finished with); J_ji's control-level terms, the level-0 copy of the trajectory
-// store and the successor-window term run in ck_cost (cost_kernels.cuh) after this kernel.
+// previous subdomain has finished with); all cost terms of J_ji (the misfits H Z^n - y included, sampled from the
+// trajectory store: 2 % of the points), the level-0 copy of the trajectory store and the successor-window term
+// run in ck_cost (cost_kernels.cuh) after this kernel: with observations every 8th level and 8 steps in flight
+// one of the steps of the pipeline always carried observations and set the pace of all (7 % of the kernel).
 // There is ONE tick body (uniform branches only, the hot loop must stay inside the instruction
 // cache); the tick loop is unrolled by three so that the row histories rotate by renaming.
 #pragma once
@@ -43,7 +45,7 @@ template <int K> struct WfCtx {
     int st, P, FS, I_SN, I_EW, I_EDS, I_EDE, T;
     uint32_t sm32, a_lead, a_mine, b_sn, b_ew;      // shared-window addresses: progress words, barriers
     unsigned gs10, need0;                            // (global step << 10), ((global step - 1) << 10)
-    bool has_leader, have_obs, injL, injR;           // injL / injR per lane
+    bool has_leader, injL, injR;                     // injL / injR per lane
     bool first;                                      // step 0 of a subdomain: its input rows (the control) arrive from global memory
     int dlead, TLd;                                  // tick t starts when the leader has published min(t + dlead, TLd + 1)
     uint32_t b_x;                                    // mbarriers of the control rows in flight (4 slots)
@@ -54,9 +56,6 @@ template <int K> struct WfCtx {
     double kap, dtcm, gdtcm;
     const double *gz, *ge; double* tout;
     const WkArgs* A;
-    long long qcur, qend;
-    int p_pk; double p_y, p_c;                       // prefetched observation of this lane (packed row|field|column)
-    double obw;
     unsigned par;
 #ifdef WK_PROF
     long long pf[8], pt;
@@ -267,26 +266,7 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
         if (prep && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
     }
     WKP(4)
-    // ---- H (25b) at level n+1 on this row: misfit, its cost, and the adjoint forcing r
-    if (out && C.have_obs) {
-        const WkArgs& A = *C.A;
-        for (;;) {
-            const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == l3);
-            const int cnt = __popc(mm);
-            if (cnt == 0) break;
-            if (C.lane < cnt) {
-                const double rr = sm[C.st + ((C.p_pk >> 8) & 3) * C.FS + l3 * C.P + (C.p_pk & 255)] - C.p_y;
-                C.obw += C.p_c * rr * rr;
-                A.obs_r[C.qcur + C.lane] = 2.0 * C.p_c * rr;
-            }
-            C.qcur += cnt;
-            C.p_pk = 0x7fffffff;
-            if (C.qcur + C.lane < C.qend) {
-                C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_y = A.obs_y[C.qcur + C.lane]; C.p_c = A.obs_c[C.qcur + C.lane];
-            }
-            if (cnt < 32) break;
-        }
-    }
+
     WKP(5)
     // ---- (6) rotate the row histories
 #pragma unroll
@@ -402,26 +382,7 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
         if (C.first && lj + WK_XD < g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
     }
     WKP(4)
-    // ---- H (25b) at level n+1 on row t-3
-    if (C.have_obs) {
-        const WkArgs& A = *C.A;
-        for (;;) {
-            const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == l3);
-            const int cnt = __popc(mm);
-            if (cnt == 0) break;
-            if (C.lane < cnt) {
-                const double rr = sm[C.st + ((C.p_pk >> 8) & 3) * C.FS + l3 * C.P + (C.p_pk & 255)] - C.p_y;
-                C.obw += C.p_c * rr * rr;
-                A.obs_r[C.qcur + C.lane] = 2.0 * C.p_c * rr;
-            }
-            C.qcur += cnt;
-            C.p_pk = 0x7fffffff;
-            if (C.qcur + C.lane < C.qend) {
-                C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_y = A.obs_y[C.qcur + C.lane]; C.p_c = A.obs_c[C.qcur + C.lane];
-            }
-            if (cnt < 32) break;
-        }
-    }
+
     WKP(5)
     // ---- rotate the row histories
 #pragma unroll
@@ -476,7 +437,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
         const WkGeo g = wk_geo(s);
         const int T = g.py + 3 - g.gyn;         // the last tile row (padded row py - 1 - gyn) leaves the pipeline three ticks after it enters
         const int n0 = (int)((unsigned)(w + 1) - gnext) & (WK_NW - 1);      // my first step in this subdomain
-        C.obw = 0.0;                            // this lane's share of H (25b) over this warp's steps
         if (n0 < g.W) {
             C.g = g; C.T = T;
             // ---------------- per-lane column map of this tile
@@ -510,13 +470,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             C.gz = A.ghost + s.goff + (long long)n * 3 * g.nring;
             C.ge = A.gedge + s.eoff + (long long)n * 2 * g.py;
             C.tout = A.traj + s.toff + (long long)(n + 1) * 3 * g.ncell;
-            C.qcur = 0; C.qend = 0;
-            if (A.obs_start) { C.qcur = A.obs_start[s.ooff + n + 1]; C.qend = A.obs_start[s.ooff + n + 2]; }
-            C.have_obs = C.qend > C.qcur;
-            C.p_pk = 0x7fffffff; C.p_y = 0.0; C.p_c = 0.0;
-            if (C.have_obs && C.qcur + lane < C.qend) {
-                C.p_pk = A.obs_lj[C.qcur + lane]; C.p_y = A.obs_y[C.qcur + lane]; C.p_c = A.obs_c[C.qcur + lane];
-            }
             if (wk_elect()) {
                 if (g.gys) wf_issue_ns(C, false); else if (g.gyn) wf_issue_ns(C, true);
                 wf_issue_chunk(C, 0);
@@ -597,10 +550,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             __syncwarp();
         }
         }
-        // ---------------- H (25b) over the steps this warp ran (fixed order: lanes, then warps in ck_cost)
-        double obw = C.obw;
-        for (int o = 16; o > 0; o >>= 1) obw += __shfl_down_sync(0xffffffffu, obw, o);
-        if (lane == 0) A.obpart[(long long)k * WK_NW + w] = obw;
         // (one step number is skipped when the window length is a multiple of the warp count, so that the
         //  levels that carry observations do not always fall on the same warp)
         glast = gnext + (unsigned)g.W - 1u;
