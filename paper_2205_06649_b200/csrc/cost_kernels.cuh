@@ -9,7 +9,8 @@
 //         looks up the rectangles that contain it), predecessor window, successor window (Z^W)
 // and, for the adjoint sweep that follows,
 //   gx   := gradient of the control-level terms (wk_adjoint adds lambda^0 with reductions)
-//   lamW := 2 mu (Z^W - x_succ) / sigma_b^2, the adjoint variable at the window end (zero in the last window)
+//   lamW := 2 mu (Z^W - x_succ) / sigma_b^2 (zero in the last window) + the observation forcing of level W: the adjoint
+//           variable at the window end
 //   level 0 of the trajectory store := the control.
 // Sums: per thread in cell order, then the fixed tree of block_sum: no atomics, run-to-run identical.
 #pragma once
@@ -103,7 +104,11 @@ __global__ void __launch_bounds__(CK_NT, 5) ck_cost(const WkArgs A)
                 const double rr = tn[(long long)((pk >> 8) & 3) * nc + (pk >> 12) * s.ex + (pk & 255)] - A.obs_y[q];
                 const double cq = A.obs_c[q];
                 ob += cq * rr * rr;
-                A.obs_r[q] = 2.0 * cq * rr;
+                const double r2 = 2.0 * cq * rr;
+                A.obs_r[q] = r2;
+                // the forcing of level W goes straight into lambda^W (unique cells inside a level; the __syncthreads above
+                // ordered the writes of lamW): the first adjoint step of the window then carries no observation work
+                if (n == s.W) lw[(long long)((pk >> 8) & 3) * nc + (pk >> 12) * s.ex + (pk & 255)] += r2;
             }
         }
     }

@@ -208,6 +208,12 @@ __global__ void __launch_bounds__(256) ck_gn(const Sub* __restrict__ subs, const
             rt[q] = r2;
             gxh[o] += r2;
         }
+        // level W: the forcing tk_obs left in rt goes into lambda^W (wk_adjoint carries no observation work at level W)
+        const long long b0 = obs_start[s.ooff + s.W], b1 = obs_start[s.ooff + s.W + 1];
+        for (long long q = b0 + tid; q < b1; q += 256) {
+            const int pk = obs_lj[q];
+            lamW[s.coff + (long long)((pk >> 8) & 3) * nc + (pk >> 12) * s.ex + (pk & 255)] += rt[q];
+        }
     }
 }
 

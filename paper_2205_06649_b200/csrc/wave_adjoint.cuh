@@ -541,7 +541,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
             C.ge = A.gedge + s.eoff + (long long)(n - 1) * 2 * g.py;
             C.tz = A.traj + s.toff + (long long)(n - 1) * n3;
             C.qcur = 0; C.qend = 0;
-            if (A.obs_start) { C.qcur = A.obs_start[s.ooff + n]; C.qend = A.obs_start[s.ooff + n + 1]; }
+            if (A.obs_start && m > 0) { C.qcur = A.obs_start[s.ooff + n]; C.qend = A.obs_start[s.ooff + n + 1]; }   // (level W: its forcing is part of lambda^W, ck_cost / ck_gn)
             C.have_obs = C.qend > C.qcur;
             C.p_pk = 0x7fffffff; C.p_r = 0.0;
             if (C.have_obs && C.qcur + lane < C.qend) { C.p_pk = A.obs_lj[C.qcur + lane]; C.p_r = A.obs_r[C.qcur + lane]; }
