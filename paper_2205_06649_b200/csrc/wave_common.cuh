@@ -31,6 +31,9 @@
 #define WK_NW 8                 // warps per CTA = time steps in flight per CTA
 #endif
 #define WK_NT (WK_NW * 32)
+#ifndef WK_SKIP
+#define WK_SKIP 0u         // step numbers skipped between two subdomains (1u rotates the warp <-> level assignment: no gain, 4 idle ticks)
+#endif
 #ifndef WK_STAGGER
 #define WK_STAGGER 0            // ticks a step starts behind its leader (0: as soon as the data allows, 4 ticks)
 #endif

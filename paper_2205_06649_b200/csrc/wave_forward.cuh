@@ -550,10 +550,8 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             __syncwarp();
         }
         }
-        // (one step number is skipped when the window length is a multiple of the warp count, so that the
-        //  levels that carry observations do not always fall on the same warp)
         glast = gnext + (unsigned)g.W - 1u;
-        gnext = glast + 1u + ((g.W & (WK_NW - 1)) == 0 ? 1u : 0u);
+        gnext = glast + 1u + WK_SKIP;
         TL = T; gysL = g.gys;
     }
 #ifdef WK_PROF
