@@ -133,8 +133,9 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
  * l.14-16) and solves the normal equations (42)-(43) l.620-626 in w = V^+ (u - u^b), V = diag(sigma_b)
  * (eq (44)-(46) l.630-649, "B-preconditioned") by exactly n_cg conjugate-gradient iterations from dw = 0, then
  * takes the full step (Alg 5 l.8).  One CG iteration = one tangent-linear sweep + one adjoint sweep (ADJ, Alg 6
- * l.17-19) on every subdomain.  Arguments and history as dd4dvar_run.  Needs a layout the wavefront kernels
- * serve (dd4dvar_active_path == 5), else -2. */
+ * l.17-19) on every subdomain.  Arguments and history as dd4dvar_run.  Served by the wavefront kernels
+ * (dd4dvar_active_path == 5) and by the generic kernels (paths 1, 3: any layout; they keep the tangent-linear
+ * trajectory in a second trajectory-sized store); -2 on the row-marching paths 2 and 4. */
 int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_analysis, double* h_history);
 
 /* Test hook: the Gauss-Newton operator H_GN = 2 grad F^T grad F of every J_ji (F = stacked residuals of eq (25)

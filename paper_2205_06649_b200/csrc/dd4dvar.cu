@@ -92,7 +92,8 @@ struct Layout {
     int* obs_lj = nullptr;
     double *obs_y = nullptr, *obs_c = nullptr, *obs_r = nullptr;
     double* obs_rt = nullptr;           // Gauss-Newton: forcing 2 c H dZ of the tangent-linear sweep
-    double *gn_lamW = nullptr, *gn_gx = nullptr, *gn_Hp = nullptr;     // Gauss-Newton: [ctot] each (wavefront layouts)
+    double *gn_lamW = nullptr, *gn_gx = nullptr, *gn_Hp = nullptr;     // Gauss-Newton: [ctot] each
+    double *gn_dtraj = nullptr, *gn_zero = nullptr;                    // Gauss-Newton on generic layouts: TLM trajectory [ttot], zeros
     FusedPlan fp{};
     WavePlan wp{};
 };
@@ -297,6 +298,11 @@ void plan_layout(Layout& L, Arena& ar, int nlon, int nlat, int m)
         L.st.nactive = ar.take<int>(4);
     }
     if ((L.path == 1 || L.path == 3) && L.vtot > 0) L.ovl = ar.take<double>(L.vtot);
+    if ((L.path == 1 || L.path == 3) && L.lbfgs) {
+        L.gn_gx = ar.take<double>(L.ctot); L.gn_Hp = ar.take<double>(L.ctot);
+        L.gn_dtraj = ar.take<double>(L.ttot);
+        L.gn_zero = ar.take<double>(std::max(L.ctot, L.vtot) + 2);
+    }
     fused_plan_arrays(L.fp, ar_take_bytes, &ar);
     if (L.wp.enabled) {
         L.gedge = ar.take<double>(std::max<long long>(L.etot, 2));
@@ -359,6 +365,7 @@ int upload_layout(dd4dvar_t h, Layout& L)
     // adjoint buffers: the ghost ring must be (and stays) zero
     CU(cudaMemsetAsync(L.lamA, 0, sizeof(double) * 3 * L.ptot1, h->stream));
     CU(cudaMemsetAsync(L.lamB, 0, sizeof(double) * 3 * L.ptot1, h->stream));
+    if (L.gn_zero) CU(cudaMemsetAsync(L.gn_zero, 0, sizeof(double) * (std::max(L.ctot, L.vtot) + 2), h->stream));
     CU(cudaMemsetAsync(L.xfrozen, 0, sizeof(double) * L.ctot, h->stream));
     CU(cudaMemsetAsync(L.pred_end, 0, sizeof(double) * L.ctot, h->stream));
     CU(cudaMemsetAsync(L.x, 0, sizeof(double) * L.ctot, h->stream));
@@ -413,19 +420,26 @@ void cost_generic(dd4dvar_t h, Layout& L, const int* mask, double* Jout)
     if (h->overlap_levels && L.ovl)
         LAUNCH(gk_ovl_cost<NT_RED>, L.nsub, NT_RED, L.dsubs, L.dnb, mask, h->cp, L.traj, L.ovl, L.parts, Jout);
 }
-void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
+// lin != nullptr: the same sweep as the adjoint of the TANGENT-LINEAR misfits (Gauss-Newton product, gn_kernels.cuh): the
+// forcing terms are taken from the tangent-linear trajectory `lin` against zeros (they are linear in it), the control-level
+// terms from the perturbation dx; the step adjoints still linearise about L.traj.
+void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw, const double* lin = nullptr,
+                     const double* dx = nullptr, const double* zero = nullptr, const double* zero_obs = nullptr,
+                     double* gx_out = nullptr)
 {
     double* buf[2] = { L.lamA, L.lamB };
-    LAUNCH(gk_adj_init, cell_grid(L), NT_GK, L.dsubs, mask, L.Wmax, L.q, L.p1 * L.p2, h->cp, L.traj,
-           L.xfrozen, L.lamA, L.lamB);
+    const double* ftraj = lin ? lin : L.traj;
+    const double* fxf = lin ? zero : L.xfrozen;
+    LAUNCH(gk_adj_init, cell_grid(L), NT_GK, L.dsubs, mask, L.Wmax, L.q, L.p1 * L.p2, h->cp, ftraj,
+           fxf, L.lamA, L.lamB);
     for (int n = L.Wmax; n >= 0; --n) {
         double* cur = buf[(L.Wmax - n) & 1];
         double* nxt = buf[(L.Wmax - n + 1) & 1];
         if (L.have_obs)
-            LAUNCH(gk_obs_force, dim3(4, L.nsub), NT_GK, L.dsubs, mask, n, L.obs_start, L.obs_idx, L.obs_y,
-                   L.obs_c, L.traj, cur);
+            LAUNCH(gk_obs_force, dim3(4, L.nsub), NT_GK, L.dsubs, mask, n, L.obs_start, L.obs_idx, lin ? zero_obs : L.obs_y,
+                   L.obs_c, ftraj, cur);
         if (n > 0 && h->overlap_levels && L.ovl)
-            LAUNCH(gk_ovl_force, cell_grid(L), NT_GK, L.dsubs, L.dnb, mask, n, h->cp, L.traj, L.ovl, cur);
+            LAUNCH(gk_ovl_force, cell_grid(L), NT_GK, L.dsubs, L.dnb, mask, n, h->cp, ftraj, lin ? zero : L.ovl, cur);
         if (n > 0 && L.path != 3) {
             sk_adjoint_step<<<dim3(L.ntiles, L.nsub), SK_NT, sizeof(double) * SK_ADJ_SMEM_DOUBLES, h->stream>>>(
                 L.dsubs, mask, n - 1, h->mp, L.traj, L.ghost, cur, nxt, L.tiles_x);
@@ -438,8 +452,12 @@ void adjoint_generic(dd4dvar_t h, Layout& L, const int* mask, double* gw)
             LAUNCH(gk_adjL0, pad_grid(L), NT_GK, L.dsubs, mask, n - 1, h->mp, L.Zp, L.A, nxt);
         }
     }
-    LAUNCH(gk_grad_final, cell_grid(L), NT_GK, L.dsubs, mask, L.geo, h->cp, L.x, L.xbs, L.xfrozen,
-           L.pred_end, buf[L.Wmax & 1], L.gx, gw);
+    if (lin)
+        LAUNCH(gk_grad_final, cell_grid(L), NT_GK, L.dsubs, mask, L.geo, h->cp, dx, zero, zero, zero, buf[L.Wmax & 1],
+               gx_out, gw);
+    else
+        LAUNCH(gk_grad_final, cell_grid(L), NT_GK, L.dsubs, mask, L.geo, h->cp, L.x, L.xbs, L.xfrozen,
+               L.pred_end, buf[L.Wmax & 1], L.gx, gw);
 }
 
 
@@ -1121,12 +1139,22 @@ int gn_apply(dd4dvar_t h, Layout& L, const double* pw, double* Hp)
     LAUNCH(tk_init, pgrid, 256, L.dsubs, h->cp, pw, L.Zp, L.Za);
     double* din = L.Zp; double* dout = L.Za;
     const size_t smem = sizeof(double) * TK_SMEM_DOUBLES;
+    const bool generic = L.path != 5;
+    if (generic) LAUNCH(tk_store, cell_grid(L), NT_GK, L.dsubs, 0, din, L.gn_dtraj);
     for (int n = 0; n < L.Wmax; ++n) {
         tk_step<<<dim3(L.ntiles, L.nsub), SK_NT, smem, h->stream>>>(L.dsubs, n, h->mp, L.traj, L.ghost, din, dout, L.tiles_x);
         ++h->launches;
-        if (L.have_obs)
+        if (generic) LAUNCH(tk_store, cell_grid(L), NT_GK, L.dsubs, n + 1, dout, L.gn_dtraj);
+        else if (L.have_obs)
             LAUNCH(tk_obs, dim3(2, L.nsub), 128, L.dsubs, n + 1, L.obs_start, L.obs_lj, L.obs_c, dout, L.obs_rt);
         std::swap(din, dout);
+    }
+    if (generic) {
+        // generic layouts: the adjoint sweep of the per-stage / block-tiled kernels with the tangent-linear trajectory as
+        // the source of every forcing term (obs_rt serves as the all-zero observation vector: it is never written here)
+        LAUNCH(gn_scale_x, dim3(std::min(32, (3 * L.maxncell + 255) / 256), L.nsub), 256, L.dsubs, h->cp, pw, L.gn_gx);
+        adjoint_generic(h, L, nullptr, Hp, L.gn_dtraj, L.gn_gx, L.gn_zero, L.obs_rt, nullptr);
+        return 0;
     }
     LAUNCH(ck_gn, L.nsub, 256, L.dsubs, L.dnb, L.geo, h->cp, pw, L.Zp, L.Za, L.have_obs ? L.obs_start : nullptr,
            L.obs_lj, L.obs_c, L.obs_rt, L.gn_gx, L.gn_lamW);
@@ -1146,7 +1174,7 @@ int dd4dvar_gn_hessvec(dd4dvar_t h, const double* d_controls, const double* d_p,
     if (!h || !d_controls || !d_p || !d_out) return fail(h, -1, "gn_hessvec: null argument");
     if (!h->have_bg) return fail(h, -3, "gn_hessvec before set_background");
     Layout& L = h->L;
-    if (L.path != 5) return fail(h, -2, "gn_hessvec: the Gauss-Newton solver needs a wavefront layout (path 5)");
+    if (L.path == 2 || L.path == 4 || !L.gn_Hp) return fail(h, -2, "gn_hessvec: the Gauss-Newton solver is served by the wavefront (path 5) and the generic kernels (path 1, 3)");
     CU(cudaMemcpyAsync(L.x, d_controls, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
     sweep(h, L, false, nullptr, L.Jev, nullptr);
     int rc = gn_apply(h, L, d_p, L.gn_Hp);
@@ -1161,7 +1189,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
     if (!h || outer_iters < 0 || n_gn < 0 || n_cg < 0 || !d_analysis || !h_history) return fail(h, -1, "run_gn: bad argument");
     if (!h->have_bg) return fail(h, -3, "run_gn before set_background");
     Layout& L = h->L; Layout& G = h->G;
-    if (L.path != 5) return fail(h, -2, "run_gn: the Gauss-Newton solver needs a wavefront layout (path 5)");
+    if (L.path == 2 || L.path == 4 || !L.gn_Hp) return fail(h, -2, "run_gn: the Gauss-Newton solver is served by the wavefront (path 5) and the generic kernels (path 1, 3)");
     if (L.sharded) return fail(h, -2, "run_gn: not available in sharded runs (dd4dvar_set_owned_windows)");
     const int n1 = h->grid.nlon * h->grid.nlat;
     const int nsub = L.nsub;

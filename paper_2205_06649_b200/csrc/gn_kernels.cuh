@@ -148,6 +148,21 @@ __global__ void __launch_bounds__(SK_NT) tk_step(const Sub* __restrict__ subs, i
     }
 }
 
+// generic layouts: level lev of the tangent-linear trajectory, padded array -> trajectory-store layout [(W+1)][3][ncell]
+__global__ void tk_store(const Sub* __restrict__ subs, int lev, const double* __restrict__ dz, double* __restrict__ dtraj)
+{
+    const int k = blockIdx.y;
+    const Sub s = subs[k];
+    if (lev > s.W) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= s.ncell) return;
+    const int lj = c / s.ex, li = c - lj * s.ex;
+    const int pc = (lj + s.gys) * s.px + li + s.gx;
+#pragma unroll
+    for (int f = 0; f < 3; ++f)
+        dtraj[s.toff + ((long long)lev * 3 + f) * s.ncell + c] = dz[s.poff + (long long)f * s.npad + pc];
+}
+
 // forcing of the adjoint sweep at local level lev: rt[q] = 2 c (H dZ^lev)[q]  (c = lambda w / sigma_o^2, eq (25b))
 __global__ void tk_obs(const Sub* __restrict__ subs, int lev, const long long* __restrict__ obs_start,
                        const int* __restrict__ obs_lj, const double* __restrict__ obs_c,
@@ -215,6 +230,14 @@ __global__ void __launch_bounds__(256) ck_gn(const Sub* __restrict__ subs, const
             lamW[s.coff + (long long)((pk >> 8) & 3) * nc + (pk >> 12) * s.ex + (pk & 255)] += rt[q];
         }
     }
+}
+
+// dx = sigma_b p (x-space perturbation of the control)
+__global__ void gn_scale_x(const Sub* __restrict__ subs, CostP cp, const double* __restrict__ pw, double* __restrict__ dx)
+{
+    const Sub s = subs[blockIdx.y];
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < 3 * s.ncell; c += gridDim.x * blockDim.x)
+        dx[s.coff + c] = cp.sb[c / s.ncell] * pw[s.coff + c];
 }
 
 // ---- conjugate gradients on H_GN dw = -g, one CTA per subdomain; vectors in control layout [3][ncell]
