@@ -158,8 +158,9 @@ int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, d
 /* The same evaluation end to end with HOST buffers: h_controls is copied to the device, the
  * gradient sweep runs, costs and (if h_grads != NULL) gradients are copied back.  Pinned host
  * memory makes the copies asynchronous with respect to the host but they are inside the call.
- * With 64 or more subdomains the evaluation runs in four chunks of consecutive subdomains (they are independent:
- * all neighbour data is frozen) so that the copies of one chunk overlap the sweeps of the others; the library
+ * With 64 or more subdomains the evaluation runs in six chunks of consecutive subdomains (they are independent:
+ * all neighbour data is frozen) so that the copies of one chunk overlap the sweeps of the others (on the wavefront
+ * path the chunks are whole rounds of the persistent grid, 1, 2, .. rounds from either end); the library
  * creates two non-blocking copy streams for this on first use and destroys them with the handle.  Results are
  * identical to dd4dvar_eval_local. */
 int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_costs, double* h_grads);

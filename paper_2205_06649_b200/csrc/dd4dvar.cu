@@ -29,7 +29,10 @@ namespace {
 constexpr int NT_GK = 256;     // generic kernels: threads per block
 constexpr int NT_RED = 256;    // cost reduction
 constexpr int NT_LB = 512;     // L-BFGS CTA
-constexpr int EH_CHUNKS = 4;   // eval_local_host: chunks of subdomains whose copies overlap the sweeps of the others
+#ifndef DD_EH_CHUNKS
+#define DD_EH_CHUNKS 6
+#endif
+constexpr int EH_CHUNKS = DD_EH_CHUNKS;     // eval_local_host: chunks of subdomains whose copies overlap the sweeps of the others
 
 struct Arena {
     char* base = nullptr;
@@ -336,6 +339,45 @@ void wave_plan_init(WavePlan& wp, const Sub* subs, int nsub)
     wp.enabled = 1;
 }
 
+// eval_local_host: bounds of its EH_CHUNKS chunks of consecutive subdomains.  A CTA of the wavefront kernels takes the
+// subdomains k = b, b + grid, ... in turn (wave_common.cuh), so there the bounds are multiples of the grid size: every
+// chunk is a whole number of rounds and the masked sweeps together take as many rounds as one full sweep.  A round is
+// copied in (or out) in about half the time it is swept, so the copy of a chunk hides behind the sweep of a neighbour of
+// half its size: chunks of 1, 2, .. rounds from either end (what is exposed is the first round's copy in and the last
+// round's copy out), the two in the middle share the rest (config 3: 14 rounds = 1 + 2 + 4 + 4 + 2 + 1).
+void eh_bounds(const Layout& L, int* kb)
+{
+    const int gran = L.wp.enabled && L.wp.grid > 0 ? L.wp.grid : 0;
+    const int R = gran ? (L.nsub + gran - 1) / gran : 0;
+    constexpr int NE = (EH_CHUNKS - 2) / 2;             // doubling chunks at either end
+    if (EH_CHUNKS >= 4 && EH_CHUNKS % 2 == 0 && R >= 4 * ((1 << NE) - 1) + 2) {
+        int r[EH_CHUNKS];
+        int used = 0;
+        for (int i = 0; i < NE; ++i) { r[i] = r[EH_CHUNKS - 1 - i] = 1 << i; used += 2 << i; }
+        r[NE] = (R - used + 1) / 2; r[NE + 1] = (R - used) / 2;
+        kb[0] = 0;
+        for (int c = 0; c < EH_CHUNKS; ++c) kb[c + 1] = std::min(L.nsub, kb[c] + gran * r[c]);
+        kb[EH_CHUNKS] = L.nsub;
+        return;
+    }
+    for (int c = 0; c <= EH_CHUNKS; ++c) {
+        const long long k = ((long long)c * L.nsub + EH_CHUNKS - 1) / EH_CHUNKS;
+        kb[c] = k > L.nsub ? L.nsub : (int)k;
+    }
+}
+
+int upload_chunk_masks(dd4dvar_t h, Layout& L)
+{
+    int kb[EH_CHUNKS + 1];
+    eh_bounds(L, kb);
+    std::vector<int> cm((size_t)EH_CHUNKS * L.nsub, 0);
+    for (int c = 0; c < EH_CHUNKS; ++c)
+        for (int k = kb[c]; k < kb[c + 1]; ++k) cm[(size_t)c * L.nsub + k] = 1;
+    CU(cudaMemcpyAsync(L.cmask, cm.data(), sizeof(int) * cm.size(), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return 0;
+}
+
 int upload_layout(dd4dvar_t h, Layout& L)
 {
     const int nlon = h->grid.nlon, nlat = h->grid.nlat;
@@ -349,12 +391,6 @@ int upload_layout(dd4dvar_t h, Layout& L)
     const size_t o_ei0 = put(L.tc_ei0), o_ex = put(L.tc_ex), o_ej0 = put(L.tr_ej0), o_ey = put(L.tr_ey);
     const size_t o_wb = put(L.wb);
     CU(cudaMemcpyAsync(L.itab, t.data(), sizeof(int) * t.size(), cudaMemcpyHostToDevice, h->stream));
-    {
-        std::vector<int> cm((size_t)EH_CHUNKS * L.nsub, 0);
-        for (int k = 0; k < L.nsub; ++k) cm[(size_t)((long long)k * EH_CHUNKS / L.nsub) * L.nsub + k] = 1;
-        CU(cudaMemcpyAsync(L.cmask, cm.data(), sizeof(int) * cm.size(), cudaMemcpyHostToDevice, h->stream));
-        CU(cudaStreamSynchronize(h->stream));
-    }
     CU(cudaStreamSynchronize(h->stream));
     GeoP& g = L.geo;
     g.nlon = nlon; g.nlat = nlat; g.p1 = L.p1; g.p2 = L.p2; g.q = L.q;
@@ -740,6 +776,8 @@ int dd4dvar_set_workspace(dd4dvar_t h, void* d_buf, size_t bytes)
         CU(cudaMemcpyAsync(h->L.wp.wtab, wt.data(), sizeof(double) * wt.size(), cudaMemcpyHostToDevice, h->stream));
         CU(cudaStreamSynchronize(h->stream));
     }
+    rc = upload_chunk_masks(h, h->L);
+    if (rc) return rc;
     if (h->L.fp.enabled) {
         h->h_ctab.assign(6 * (size_t)FK_CTAB, 0.0);
         if (fused_upload_tables(h->stream, h->h_tab.data(), nlat, h->h_ctab.data(), h->d_ctab))
@@ -948,7 +986,7 @@ int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_cos
     if (!h || !h_controls || !h_costs) return fail(h, -1, "eval_local_host: null argument");
     if (!h->have_bg) return fail(h, -3, "eval_local_host before set_background");
     Layout& L = h->L;
-    if (L.nsub < 16 * EH_CHUNKS) {              // small problems: one copy in, one sweep, one copy out
+    if (L.nsub < 64) {                          // small problems: one copy in, one sweep, one copy out
         CU(cudaMemcpyAsync(L.x, h_controls, sizeof(double) * L.ctot, cudaMemcpyHostToDevice, h->stream));
         sweep(h, L, h_grads != nullptr, nullptr, L.Jev, nullptr);
         CU(cudaMemcpyAsync(h_costs, L.Jev, sizeof(double) * L.nsub, cudaMemcpyDeviceToHost, h->stream));
@@ -971,10 +1009,7 @@ int dd4dvar_eval_local_host(dd4dvar_t h, const double* h_controls, double* h_cos
         CU(cudaStreamWaitEvent(h->s_h2d, h->ev_in, 0));
         CU(cudaStreamWaitEvent(h->s_d2h, h->ev_in, 0));
         int kb[EH_CHUNKS + 1];
-        for (int c = 0; c <= EH_CHUNKS; ++c) {                          // chunk c = subdomains with k * EH_CHUNKS / nsub == c
-            int k = (int)(((long long)c * L.nsub + EH_CHUNKS - 1) / EH_CHUNKS);
-            kb[c] = k > L.nsub ? L.nsub : k;
-        }
+        eh_bounds(L, kb);
         auto off = [&](int k) { return k < L.nsub ? L.hs[k].coff : L.ctot; };
         for (int c = 0; c < EH_CHUNKS; ++c) {
             const long long o0 = off(kb[c]), o1 = off(kb[c + 1]);

@@ -105,6 +105,15 @@ def test_config3_sampled_subdomains_and_invariants():
             assert abs(parts[k, q] - po[1 + q]) <= TOL_EVAL * abs(po[0]), (k, q)
         assert rel(gl[k].cpu().numpy(), go) <= TOL_EVAL, (k, rel(gl[k].cpu().numpy(), go))
         assert rel(g.get_local_trajectory(k).cpu().numpy(), tr) <= 1e-12, k
+    # the host-buffer entry point in the configuration bench.py times for `e2e` (six chunks of 1 + 2 + 4 + 4 + 2 + 1
+    # rounds of 148 subdomains, copies overlapped with the masked sweeps): bit for bit what the one-sweep call returned
+    import torch
+    h_ctrl = flat.cpu().pin_memory()
+    h_grad = torch.zeros_like(h_ctrl).pin_memory()
+    h_cost = np.zeros(g.nsub)
+    g.eval_local_host(h_ctrl, h_cost, h_grad)
+    assert np.array_equal(h_cost, costs)
+    assert np.array_equal(h_grad.numpy(), grads.cpu().numpy())
 
 
 def test_config4_large_tile_layout_follows_the_oracle_iteration():
