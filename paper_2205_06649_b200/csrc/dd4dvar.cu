@@ -333,6 +333,7 @@ void wave_plan_init(WavePlan& wp, const Sub* subs, int nsub)
     if (wp.maxpx - 4 <= 64) wp.K = 2;
     else if (wp.maxpx - 4 <= 96) wp.K = 3;
     else return;
+    if (wp.maxey > WK_AROWS(wp.K)) return;      // rows of the adjoint kernel's resident state (compile-time field stride)
     wp.smem_fwd = sizeof(double) * (size_t)wk_layout(false, wp.maxex, wp.maxey, wp.maxpx, wp.maxpy).total;
     wp.smem_adj = sizeof(double) * (size_t)wk_layout(true, wp.maxex, wp.maxey, wp.maxpx, wp.maxpy).total;
     if (wp.smem_fwd > WK_SMEM_MAX || wp.smem_adj > WK_SMEM_MAX) return;

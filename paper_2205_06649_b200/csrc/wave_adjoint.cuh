@@ -50,9 +50,11 @@ template <int K> struct WaState {     // every history has depth one: slot [t & 
 };
 template <int K> struct WaCtx {
     WkGeo g;
-    int lam, FS, u1, I_ZR, ZP, I_EW, I_EDS, I_EDE, T, maxey;
+    static constexpr int ZP = WK_AZP(K), FS = WK_AFS(K), maxey = WK_AROWS(K);   // ring row pitch, field stride, zero row
+    static constexpr uint32_t SL8 = 24u * ZP, ZP8 = 8u * ZP, FS8 = 8u * FS;      // strides in bytes
+    int lam, u1, I_ZR, I_EW, I_EDS, I_EDE, T;
     uint32_t sm32, a_lead, a_mine, b_z, b_ew;
-    uint32_t zl, zu, SL8, ZP8, FS8, la0;     // per-lane ring / lambda base addresses (shared window), strides in bytes
+    uint32_t zl, zu, la0;           // per-lane ring / lambda base addresses (shared window)
     unsigned gs10, need0;
     bool has_leader, have_obs, injL, injR, lane0, laneL;    // lane0 / laneL: first lane, lane 31
     bool first, last;               // adjoint step of level W (its input rows arrive from global memory) / of level 1 (its output is the gradient)
@@ -477,12 +479,12 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
     const int lw = (w + WK_NW - 1) % WK_NW;
 
     WaCtx<K> C;
-    C.lam = Ly.st; C.u1 = Ly.u1; C.ZP = Ly.ZP; C.FS = Ly.FS; C.maxey = A.maxey;
+    C.lam = Ly.st; C.u1 = Ly.u1;                // (Ly.ZP, Ly.FS: compile-time constants of K, wave_common.cuh)
     C.I_ZR = IW + Ly.zr; C.I_EW = IW + Ly.ew; C.I_EDS = IW + Ly.eds; C.I_EDE = IW + Ly.ede;
     C.sm32 = sm32; C.a_lead = sm32 + 8u * WK_PROG + 4u * lw; C.a_mine = sm32 + 8u * WK_PROG + 4u * w;
     C.b_z = sm32 + 8u * (w * WK_BAR_PER_WARP); C.b_ew = C.b_z + 24u;
     C.c0 = 2 + K * lane; C.lane = lane; C.lane0 = lane == 0; C.laneL = lane == 31;
-    C.zu = sm32 + 8u * C.I_ZR; C.zl = C.zu + 8u * C.c0; C.SL8 = 8u * 3 * Ly.ZP; C.ZP8 = 8u * Ly.ZP; C.FS8 = 8u * Ly.FS;
+    C.zu = sm32 + 8u * C.I_ZR; C.zl = C.zu + 8u * C.c0;
     C.la0 = sm32 + 8u * (Ly.st + K * lane);
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm; C.c0k = 1.0 - 4.0 * A.m.kap; C.mu2 = 2.0 * A.cp.mu;
     C.A = &A; C.par = 0u;

@@ -43,13 +43,19 @@
 #define WK_NTAB 3               // row-table slots: 8 steps in flight span at most 3 subdomains when every window has >= 4 steps
 #define WK_TABSZ(maxpy) (((maxpy) + 2) * 8)
 #define WK_SMEM_MAX 232448      // 227 KB: largest opt-in dynamic shared memory of one CTA on sm_100a
+// Adjoint kernel: the strides of its shared-memory arrays are COMPILE-TIME constants of K (immediate offsets in the
+// hot loop instead of address arithmetic): ring row pitch 32 K + 6 (the widest padded row + 2), lambda / u^n field
+// stride (WK_AROWS + 1) rows of 32 K cells, WK_AROWS = the tallest extended tile the 227 KB hold.
+#define WK_AZP(K) (32 * (K) + 6)
+#define WK_AROWS(K) ((K) == 3 ? 49 : 80)
+#define WK_AFS(K) ((WK_AROWS(K) + 1) * 32 * (K))
 
 // Shared-memory layout in doubles (same function on host and device).
 //   header | row tables [WK_NTAB][(maxpy+2)][8] | resident state | per-warp staging
 // forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
 //   [tile ex][E ghosts 3][pad 2][W ghosts of the NEXT row 3], so that padded column c of tile row
 //   lj is at  st + f*FS + lj*P + (c - 3)  for every c (W ghosts sit in the previous row's tail).
-// adjoint resident state: lambda [3][maxey+1][32 K] and u1 [maxey+1][32 K]: lambda is zero outside
+// adjoint resident state: lambda [3][WK_AROWS+1][32 K] and u1 [WK_AROWS+1][32 K]: lambda is zero outside
 //   the extended tile, so only the columns the lanes own are kept; the cells of ghost columns and
 //   the extra row stay zero and serve every read that falls outside the tile.
 struct WkLayout {
@@ -67,13 +73,15 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
     } else {
         // row pitch = 32 K cells (one cell per lane and owned column: cell q <-> padded column q + 2, so
         // q = 0 and q > ex are permanently zero), plus one all-zero row (index maxey) per field
-        L.P = maxpx - 4 <= 64 ? 64 : 96; L.FS = (maxey + 1) * L.P;
+        // (field stride and ring pitch do not depend on the layout: WK_AFS, WK_AZP; row WK_AROWS is the all-zero row)
+        const int K = maxpx - 4 <= 64 ? 2 : 3;
+        L.P = 32 * K; L.FS = WK_AFS(K);
         L.st = o; o += 3 * L.FS;
         L.u1 = o; o += L.FS;
     }
     L.wbase = o;
     int p = 0;
-    L.ZP = maxpx + 2;
+    L.ZP = adj ? WK_AZP(maxpx - 4 <= 64 ? 2 : 3) : maxpx + 2;
     if (!adj) { L.sn = p; p += 9 * maxpx; L.zr = 0; }
     else { L.zr = p; p += 9 * L.ZP; L.sn = 0; }
     const int ewc = adj ? WK_EWCA : WK_EWC;
