@@ -52,7 +52,7 @@
 
 // Shared-memory layout in doubles (same function on host and device).
 //   header | row tables [WK_NTAB][(maxpy+2)][8] | resident state | per-warp staging
-// forward resident state: [3][maxey][P] with pitch P = maxex + 8; a tile row holds
+// forward resident state: [3][WK_AROWS][P] with pitch P = WK_AZP = 32 K + 6 >= maxex + 8; a tile row holds
 //   [tile ex][E ghosts 3][pad 2][W ghosts of the NEXT row 3], so that padded column c of tile row
 //   lj is at  st + f*FS + lj*P + (c - 3)  for every c (W ghosts sit in the previous row's tail).
 // adjoint resident state: lambda [3][WK_AROWS+1][32 K] and u1 [WK_AROWS+1][32 K]: lambda is zero outside
@@ -67,7 +67,7 @@ __host__ __device__ inline WkLayout wk_layout(bool adj, int maxex, int maxey, in
     int o = WK_HDR;
     L.tab = o; o += WK_NTAB * WK_TABSZ(maxpy);      // row tables of the subdomains in flight
     if (!adj) {
-        L.P = maxex + 8; L.FS = maxey * L.P;
+        L.P = WK_AZP(maxpx - 4 <= 64 ? 2 : 3); L.FS = WK_AROWS(maxpx - 4 <= 64 ? 2 : 3) * L.P;    // (compile-time in the kernel)
         L.st = o + 8; o += 8 + 3 * L.FS + 64;       // 64 doubles of slack: lanes beyond px read past a row
         L.u1 = 0;
     } else {

@@ -42,7 +42,8 @@ template <int K> struct WfRegs {
 // everything a tick needs besides the histories (uniform unless noted)
 template <int K> struct WfCtx {
     WkGeo g;
-    int st, P, FS, I_SN, I_EW, I_EDS, I_EDE, T;
+    static constexpr int P = WK_AZP(K), FS = WK_AROWS(K) * WK_AZP(K);     // row pitch, field stride (compile-time, wave_common.cuh)
+    int st, I_SN, I_EW, I_EDS, I_EDE, T;
     uint32_t sm32, a_lead, a_mine, b_sn, b_ew;      // shared-window addresses: progress words, barriers
     unsigned gs10, need0;                            // (global step << 10), ((global step - 1) << 10)
     bool has_leader, injL, injR;                     // injL / injR per lane
@@ -288,7 +289,7 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
 {
     const WkGeo& g = C.g;
     const int lj = t - g.gys;
-    const uint32_t P8 = 8u * C.P, FS8 = 8u * C.FS;
+    constexpr uint32_t P8 = 8u * WfCtx<K>::P, FS8 = 8u * WfCtx<K>::FS;
     WKP(7)
     if (C.has_leader) { const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
     if (C.first) wf_wait_xrow<K>(C, lj);
@@ -413,14 +414,14 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
     const int lw = (w + WK_NW - 1) % WK_NW;     // the warp that runs the previous step
 
     WfCtx<K> C;
-    C.st = Ly.st; C.P = Ly.P; C.FS = Ly.FS;
+    C.st = Ly.st;                               // (Ly.P, Ly.FS: compile-time constants of K)
     C.I_SN = IW + Ly.sn; C.I_EW = IW + Ly.ew; C.I_EDS = IW + Ly.eds; C.I_EDE = IW + Ly.ede;
     C.sm32 = sm32; C.a_lead = sm32 + 8u * WK_PROG + 4u * lw; C.a_mine = sm32 + 8u * WK_PROG + 4u * w;
     C.b_sn = sm32 + 8u * (w * WK_BAR_PER_WARP); C.b_ew = C.b_sn + 8u; C.b_x = C.b_sn + 32u;
     C.c0 = 2 + K * lane; C.lane = lane;
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm;
     C.A = &A; C.par = 0u;
-    const int FS = Ly.FS;
+    constexpr int FS = WfCtx<K>::FS;
 #ifdef WK_PROF
     for (int q = 0; q < 8; ++q) C.pf[q] = 0;
 #endif
