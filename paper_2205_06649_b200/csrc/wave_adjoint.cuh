@@ -92,19 +92,6 @@ __device__ __forceinline__ void wa_issue_row(const WaCtx<K>& C, int r, bool with
     if (with_edges && g.gys) wk_g2s32(C.sm32 + 8u * C.I_EDS, C.ge, g.gys * 16u, bar);
     if (with_edges && g.gyn) wk_g2s32(C.sm32 + 8u * (C.I_EDS + 8), C.ge + g.gys * 2, g.gyn * 16u, bar);
 }
-// the same for a tile row (tile row l2) into the compile-time slot SLOT
-template <int K>
-__device__ __forceinline__ void wa_issue_tile_row(const WaCtx<K>& C, int l2, const int SLOT)
-{
-    const uint32_t bar = C.b_z + 8u * SLOT;
-    const uint32_t bytes = C.g.ex * 8u;
-    const uint32_t dst = C.zu + SLOT * C.SL8 + 32u;
-    const double* src = C.tz + l2 * C.g.ex;
-    wk_mbar_expect32(bar, 3u * bytes);
-    wk_g2s32(dst, src, bytes, bar);
-    wk_g2s32(dst + C.ZP8, src + C.g.ncell, bytes, bar);
-    wk_g2s32(dst + 2u * C.ZP8, src + 2 * C.g.ncell, bytes, bar);
-}
 template <int K>
 __device__ __forceinline__ void wa_issue_chunk(const WaCtx<K>& C, int c)
 {
@@ -132,18 +119,6 @@ __device__ __forceinline__ void wa_prep_row(WaCtx<K>& C, double* __restrict__ sm
         const int cs = (l / WK_EWCA) & 1, lr = l % WK_EWCA;
         if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * cs, (C.par >> (3 + cs)) & 1u); C.par ^= 8u << cs; }
         if (C.lane < 20) sm[C.I_ZR + slot * 3 * C.ZP + C.gcp_dst] = sm[C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs];
-    }
-}
-// the same for a tile row (tile row l) in the compile-time slot SLOT
-template <int K>
-__device__ __forceinline__ void wa_prep_tile_row(WaCtx<K>& C, int l, const int SLOT)
-{
-    wk_mbar_wait32(C.b_z + 8u * SLOT, (C.par >> SLOT) & 1u); C.par ^= 1u << SLOT;
-    const int cs = (l / WK_EWCA) & 1, lr = l % WK_EWCA;
-    if (lr == 0) { wk_mbar_wait32(C.b_ew + 8u * cs, (C.par >> (3 + cs)) & 1u); C.par ^= 8u << cs; }
-    if (C.lane < 20) {
-        const double gv = wk_lds<0>(C.sm32 + 8u * (C.gcp_base + cs * C.gcp_ss + lr * C.gcp_rs));
-        wk_sts<0>(C.zu + SLOT * C.SL8 + 8u * C.gcp_dst, gv);
     }
 }
 
