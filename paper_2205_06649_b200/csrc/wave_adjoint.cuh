@@ -166,6 +166,35 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     double (&zS)[3][K] = S.zc[po];
     WKP(7)
 
+    // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row.  First in the tick:
+    // the read-modify-write of the forcing and the first step's row copies complete behind stages (1) and (2a), which
+    // work on the warp's private ring (4.43 -> 4.33 ms against the poll after stage (2a); one poll per pair of ticks: 4.29 ms)
+    if (C.has_leader && (WALL || P2 == 0)) {        // (a pair of ticks: one poll, for what the second tick needs)
+        const int nd = t + 1 + C.dlead < C.TLd + 1 ? t + 1 + C.dlead : C.TLd + 1;
+        wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
+    }
+    if (C.first) {                                  // row t of lambda^W / u^W has landed; fetch row t + 2
+        wk_cpa_wait<1>();
+        wa_issue_lamrow<K>(C, lj + 2);
+        __syncwarp();
+    }
+    WKP(0)
+    if (tile && C.have_obs) {
+        const WkArgs& A = *C.A;
+        for (;;) {
+            const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == lj);
+            const int cnt = __popc(mm);
+            if (cnt == 0) break;
+            if (C.lane < cnt) sm[C.lam + ((C.p_pk >> 8) & 3) * C.FS + lj * (32 * K) + 1 + (C.p_pk & 255)] += C.p_r;
+            C.qcur += cnt;
+            C.p_pk = 0x7fffffff;
+            if (C.qcur + C.lane < C.qend) { C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_r = A.obs_r[C.qcur + C.lane]; }
+            if (cnt < 32) break;
+        }
+        __syncwarp();
+    }
+    WKP(5)
+
     // ---- (1) Z^{n-1}: own columns of row t, E/W halo and edge u^a of row t-1
     double eL, eR;
     {
@@ -239,33 +268,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         uaW = 0.0; uaE = 0.0;
     }
     WKP(2)
-
-    // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row
-    if (C.has_leader) {
-        const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1;
-        wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
-    }
-    if (C.first) {                                  // row t of lambda^W / u^W has landed; fetch row t + 2
-        wk_cpa_wait<1>();
-        wa_issue_lamrow<K>(C, lj + 2);
-        __syncwarp();
-    }
-    WKP(0)
-    if (tile && C.have_obs) {
-        const WkArgs& A = *C.A;
-        for (;;) {
-            const unsigned mm = __ballot_sync(0xffffffffu, (C.p_pk >> 12) == lj);
-            const int cnt = __popc(mm);
-            if (cnt == 0) break;
-            if (C.lane < cnt) sm[C.lam + ((C.p_pk >> 8) & 3) * C.FS + lj * (32 * K) + 1 + (C.p_pk & 255)] += C.p_r;
-            C.qcur += cnt;
-            C.p_pk = 0x7fffffff;
-            if (C.qcur + C.lane < C.qend) { C.p_pk = A.obs_lj[C.qcur + C.lane]; C.p_r = A.obs_r[C.qcur + C.lane]; }
-            if (cnt < 32) break;
-        }
-        __syncwarp();
-    }
-    WKP(5)
 
     // ---- (2b) lambda^n: v rows t, t-1, t-2; h, u and u^n row t-1.  UB, HB, P and the row-local parts of A on row t-1
     const uint32_t lrow = C.la0 + (uint32_t)lj * PL8;      // own cell 0 of lambda_h, tile row lj (may lie outside the tile)
