@@ -134,7 +134,9 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
     const bool tile = (unsigned)lj < (unsigned)g.ey;
     // ---- (0) row t becomes readable
     WKP(7)
-    if (C.has_leader) { const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+    if (C.has_leader && !(t & 1)) {             // (one poll for two ticks: every even tick waits for what the next one needs)
+        const int nd = t + 1 + C.dlead < C.TLd + 1 ? t + 1 + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
+    }
     WKP(0)
     int ra = 0, rfs = 0, re = 0;                    // own column 0 of row t, field stride, edge-u^a index
     if (tile) {                                      // (its E/W ghost cells were put in place one tick earlier)
@@ -291,7 +293,9 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
     const int lj = t - g.gys;
     constexpr uint32_t P8 = 8u * WfCtx<K>::P, FS8 = 8u * WfCtx<K>::FS;
     WKP(7)
-    if (C.has_leader) { const int nd = t + C.dlead < C.TLd + 1 ? t + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
+    if (C.has_leader && !(t & 1)) {             // (one poll for two ticks: every even tick waits for what the next one needs)
+        const int nd = t + 1 + C.dlead < C.TLd + 1 ? t + 1 + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
+    }
     if (C.first) wf_wait_xrow<K>(C, lj);
     WKP(0)
     // ---- loads: own columns of row t, E/W halo and edge u^a of row t-1
