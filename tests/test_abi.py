@@ -129,3 +129,30 @@ def test_geometry_follows_the_definitions_written_out_in_python(lib):
                     covered[jw][np.ix_(own_j, own_i)] += 1
         assert np.all(covered == 1)             # the owned tiles partition the grid in every window
         lib.dd4dvar_destroy(h)
+
+
+def test_wavefront_kernels_take_layouts_up_to_their_row_limit_and_no_further(lib):
+    """Eligibility of the wavefront kernels: the resident state has a compile-time number of rows
+    (80 for tiles of up to 68 padded columns, 49 up to 100).  One row more: the default falls back to another kernel
+    family and an explicit request for the wavefront path is refused (-2), without a GPU."""
+    from paper_2205_06649_b200.binding import Grid, Decomp, Window, Opts
+    lib.dd4dvar_create.argtypes = [ctypes.c_void_p] * 6
+    lib.dd4dvar_active_path.argtypes = [ctypes.c_void_p]
+    lib.dd4dvar_destroy.argtypes = [ctypes.c_void_p]
+
+    def create(nlon, nlat, path):
+        h = ctypes.c_void_p()
+        g = Grid(nlon, nlat, 6.371e6, 7.292e-5, 9.806, 0.64, 0.02)
+        d = Decomp(2, 2, 2, 2, 1.0, 1.0); w = Window(60.0, 8); op = Opts(5, 5, 20, 1e-4, path)
+        rc = lib.dd4dvar_create(ctypes.byref(g), ctypes.byref(d), ctypes.byref(w), ctypes.byref(op), None, ctypes.byref(h))
+        p = lib.dd4dvar_active_path(h) if rc == 0 else None
+        if rc == 0:
+            lib.dd4dvar_destroy(h)
+        return rc, p
+
+    assert create(116, 156, 0) == (0, 5)            # extended tiles 62 x 80 (K = 2)
+    assert create(116, 158, 0)[1] in (1, 2)         # 62 x 81
+    assert create(116, 158, 5)[0] == -2
+    assert create(180, 94, 0) == (0, 5)             # 94 x 49 (K = 3)
+    assert create(180, 96, 0)[1] in (1, 2)          # 94 x 50
+    assert create(180, 96, 5)[0] == -2

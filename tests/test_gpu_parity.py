@@ -32,6 +32,8 @@ LAYOUTS = {
                       obs_frac=0.3, obs_every=1),
     # K = 2 (px = 38), many short windows
     "wave_k2": dict(nlon=56, nlat=20, nsteps=17, p_lon=2, p_lat=2, q_time=4, overlap=2),
+    # K = 2 at the row limit of the wavefront kernels' resident state (extended tiles of 79 rows, WK_AROWS(2) = 80), px = 68
+    "wave_k2_tall": dict(nlon=116, nlat=154, dt=60.0, nsteps=8, p_lon=2, p_lat=2, q_time=2, overlap=2),
 }
 PATHS = [1, 2, 3, 4, 5]
 
