@@ -82,7 +82,9 @@ typedef struct {
  *       4 = wavefront forward kernel (shared-memory resident tile, TMA-staged rows, cost terms fused)
  *       + row-marching adjoint kernel, 5 = wavefront forward + wavefront adjoint kernels
  *       (4 and 5: create fails with -2 unless every tile has a ghost ring in longitude, an even
- *       number of columns and at most 100 padded columns). */
+ *       number of columns, at most 100 padded columns, an extended tile of at most 49 rows (80 rows
+ *       up to 68 padded columns), and every window at least 4 steps; "cost terms fused" is the round-1
+ *       wording: the cost terms run in the kernel ck_cost between the two sweeps). */
 typedef struct {
     int lbfgs_m, n_inner, max_backtrack;
     double armijo_c1;
