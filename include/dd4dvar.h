@@ -25,6 +25,7 @@
  *   - Return value: 0 on success, otherwise
  *       -1 invalid argument            -2 decomposition does not fit the grid / window
  *       -3 called out of order         -4 CUDA error          -5 non-finite cost or gradient
+ *       -6 problem larger than the built-in scratch array (dd4dvar_forecast_static only)
  *     Nothing is thrown across the ABI; dd4dvar_last_error gives the text of the last failure.
  *   - There is no CPU fallback: without a CUDA device every compute call returns -4.
  *   - Handles share nothing: every table and buffer a kernel reads belongs to one handle, so
@@ -191,6 +192,41 @@ int dd4dvar_forecast(dd4dvar_t h, const double* d_x0, int n_levels, const int* h
                      double* d_out);
 
 int dd4dvar_num_subdomains(dd4dvar_t h);
+/* Forecast for callers that cannot give the library any device memory of their own making.
+ *
+ * Every other entry point works out of a workspace that the caller allocates (dd4dvar_set_workspace).  Some callers
+ * have no allocator to turn to at the moment they need a forecast: code that runs after a framework has claimed the
+ * whole device for its own pool and hands out nothing to plug-ins; a monitoring or fail-over path that must still
+ * produce the background trajectory when the device is full and cudaMalloc would fail; host code in a latency-bound
+ * loop, where cudaMalloc / cudaFree would stall every stream of the device.  For them this call runs the model
+ * (the same step kernel code as dd4dvar_forecast, on the undecomposed grid) without a handle and without a
+ * workspace.  It calls no cudaMalloc, cudaFree or other allocating routine, on any path.
+ *
+ * The scratch it needs -- the six row tables and the time levels between which the model steps -- is one array of
+ * DD4DVAR_STATIC_SCRATCH_BYTES compiled into the library.  That memory is taken on EVERY GPU on which the process
+ * loads libdd4dvar.so and is held until the process exits, whether this call is used or not; that is the price, and
+ * why the array is small.  Limit: 8 * (32 * ceil(6 nlat / 32) + 2 * 3 nlon nlat) <= DD4DVAR_STATIC_SCRATCH_BYTES,
+ * i.e. up to about 349 000 grid cells (720 x 360 fits, 1440 x 720 does not).  Larger grids are refused with -6 and a
+ * message that names the two sizes; nothing is launched in that case.  nsteps is not limited: when the array holds
+ * fewer levels than the window has, the newest level is moved to the front and the stepping continues.
+ *
+ * grid, window: as for dd4dvar_create.  d_x0: DEVICE, fp64 [3][nlat][nlon], read only.  h_levels: HOST, n_levels
+ * ascending time levels in [0, nsteps].  d_out: DEVICE, fp64 [n_levels][3][nlat][nlon], caller-owned, written in full.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream); all work is queued there and the call returns after
+ * synchronising it.  h_err / err_len: optional HOST buffer that receives the text of a failure (there is no handle
+ * to ask); may be NULL / 0.  Returns 0, -1, -2, -4 or -6 as listed at the top.
+ *
+ * First call on each device: the library looks up the device address of its array (once per device, with the
+ * caller's current device; the result is kept).  Make that first call at set-up time, outside any stream capture.
+ * All calls in a process share the one array per device, and it keeps whatever the last call left there.  Nothing in
+ * it has to start at zero -- each call rewrites the tables and writes every level in full before reading it -- but
+ * two calls whose work overlaps on the same GPU (two streams, or two host threads) race on it and both results are
+ * then undefined: run them one after the other. */
+#define DD4DVAR_STATIC_SCRATCH_BYTES (16u << 20)
+int dd4dvar_forecast_static(const dd4dvar_grid* grid, const dd4dvar_window* window, const double* d_x0,
+                            int n_levels, const int* h_levels, double* d_out, void* cuda_stream,
+                            char* h_err, size_t err_len);
+
 /* out[16] = tile_col, tile_row, window, owned i0,i1,j0,j1, ext i0 (may be < 0: wraps), ext j0,
  * ex, ey, ghost width lon, ghost south, ghost north, first level s, last level e. */
 int dd4dvar_subdomain_info(dd4dvar_t h, int sub, int out[16]);

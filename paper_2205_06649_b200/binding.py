@@ -49,7 +49,7 @@ EXPORTS = [
     "dd4dvar_create", "dd4dvar_workspace_bytes", "dd4dvar_set_workspace", "dd4dvar_set_background",
     "dd4dvar_obs_workspace_bytes", "dd4dvar_set_observations", "dd4dvar_run", "dd4dvar_eval_global",
     "dd4dvar_eval_local", "dd4dvar_eval_local_host", "dd4dvar_sweep_async", "dd4dvar_get_controls", "dd4dvar_get_trajectory",
-    "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_num_subdomains",
+    "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_forecast_static", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
     "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global", "dd4dvar_set_overlap_levels", "dd4dvar_set_owned_windows", "dd4dvar_exchange_buffer",
     "dd4dvar_get_local_stats", "dd4dvar_gather_analysis",
@@ -87,6 +87,7 @@ def load_library():
     lib.dd4dvar_get_trajectory.argtypes = [vp, C.c_int, dp]
     lib.dd4dvar_get_local_trajectory.argtypes = [vp, C.c_int, dp]
     lib.dd4dvar_forecast.argtypes = [vp, dp, C.c_int, ip, dp]
+    lib.dd4dvar_forecast_static.argtypes = [C.POINTER(Grid), C.POINTER(Window), dp, C.c_int, ip, dp, vp, C.c_char_p, C.c_size_t]
     lib.dd4dvar_num_subdomains.argtypes = [vp]
     lib.dd4dvar_subdomain_info.argtypes = [vp, C.c_int, ip]
     lib.dd4dvar_control_offset.restype = C.c_longlong
@@ -130,6 +131,39 @@ def measure_peaks(device="cuda:0"):
     return {"fp64_fma_tflops": out[0], "fp64_add_tinstr_s": out[1], "lds64_bytes_per_s": out[2],
             "lds64_bytes_per_clk_per_sm": out[2] / (nsm * mhz * 1e6), "shfl64_per_s": out[3],
             "shfl64_bytes_per_clk_per_sm": 8.0 * out[3] / (nsm * mhz * 1e6), "sm_count": int(nsm), "sm_clock_mhz": mhz}
+
+
+STATIC_SCRATCH_BYTES = 16 << 20     # DD4DVAR_STATIC_SCRATCH_BYTES of include/dd4dvar.h
+
+
+def forecast_static(x0, levels, out, dt, nsteps, radius=6.371e6, omega=7.292e-5, gravity=9.806,
+                    cos_clamp=float(np.cos(np.deg2rad(50.0))), diffusion=0.02, stream=None):
+    """dd4dvar_forecast_static: the model forecast for a caller that cannot allocate device memory for the library
+    (the device is owned by another pool, or is full, or the caller must not stall it with cudaMalloc).  No handle,
+    no workspace: the library steps the model inside a 16 MiB array that is part of its image, so the grid is limited
+    to about 349 000 cells (DD4DVarError with code -6 beyond that).  Nothing is allocated here either: `x0`
+    ([3][nlat][nlon]) and `out` ([len(levels)][3][nlat][nlon]) are the caller's fp64 CUDA tensors; `out` is filled and
+    returned.  Calls share the library's array: do not let two of them overlap on one GPU.  Make the first call on a
+    device during set-up, outside stream capture."""
+    import torch
+    lib = load_library()
+    if not (x0.is_cuda and out.is_cuda and x0.dtype == torch.float64 and out.dtype == torch.float64
+            and x0.is_contiguous() and out.is_contiguous() and x0.dim() == 3 and x0.shape[0] == 3):
+        raise DD4DVarError("dd4dvar_forecast_static", -1, "x0 and out must be contiguous fp64 CUDA tensors, x0 [3][nlat][nlon]")
+    lv = np.ascontiguousarray(levels, dtype=np.int32)
+    if tuple(out.shape) != (lv.size,) + tuple(x0.shape) or out.device != x0.device:
+        raise DD4DVarError("dd4dvar_forecast_static", -1, "out must be [len(levels)][3][nlat][nlon] on x0's device")
+    g = Grid(int(x0.shape[2]), int(x0.shape[1]), radius, omega, gravity, cos_clamp, diffusion)
+    w = Window(dt, nsteps)
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(x0.device):
+        st = stream if stream is not None else torch.cuda.current_stream(x0.device)
+        rc = lib.dd4dvar_forecast_static(C.byref(g), C.byref(w), x0.data_ptr(), lv.size,
+                                         lv.ctypes.data_as(C.POINTER(C.c_int)), out.data_ptr(),
+                                         C.c_void_p(st.cuda_stream), err, len(err))
+    if rc:
+        raise DD4DVarError("dd4dvar_forecast_static", rc, err.value.decode())
+    return out
 
 
 class DD4DVar:

@@ -1394,3 +1394,167 @@ void dd4dvar_destroy(dd4dvar_t h)
 }
 
 }  // extern "C"
+
+// ================================================== forecast without device allocation ====
+// dd4dvar_forecast_static (include/dd4dvar.h): the model forecast of dd4dvar_forecast for callers that have no way
+// of obtaining device memory for the library: no handle, no workspace.  Everything the step kernel needs beyond the
+// caller's input and output -- the six row tables of the model and the time levels it steps between -- lives in ONE
+// array that is part of the library image.  The array is reserved on every GPU that loads libdd4dvar.so, for the life
+// of the process, whether or not this entry point is ever called; hence its modest, fixed size.
+#include <mutex>
+
+#define DD_STATIC_DOUBLES ((size_t)DD4DVAR_STATIC_SCRATCH_BYTES / sizeof(double))
+static __device__ __align__(256) double dd_static_scratch[DD_STATIC_DOUBLES];
+
+namespace {
+
+// `dd_static_scratch` in HOST code is only a handle for the runtime's symbol look-up, not an address a kernel could
+// use.  The device address differs per GPU; it is asked for once per device (with that device current) and kept here.
+constexpr int DD_STATIC_MAXDEV = 64;
+double* g_static_base[DD_STATIC_MAXDEV] = {};
+std::mutex g_static_mutex;
+
+int static_scratch_base(double** out, std::string& err)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { err = std::string("cudaGetDevice: ") + cudaGetErrorString(e); return -4; }
+    if (dev < 0 || dev >= DD_STATIC_MAXDEV) { err = "device ordinal beyond the table of dd4dvar_forecast_static"; return -4; }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_base[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, dd_static_scratch);
+        if (e != cudaSuccess || !p) {
+            err = std::string("cudaGetSymbolAddress(dd_static_scratch): ") + cudaGetErrorString(e);
+            return -4;
+        }
+        g_static_base[dev] = p;
+    }
+    *out = g_static_base[dev];
+    return 0;
+}
+
+// The same row tables as dd4dvar_create builds (O1: eq (60)-(62) l.945-954, cell-centred rows R2, clamped metric R3,
+// dt folded in), written out a second time so that the handle-based path stays untouched.  tab: [6][nlat].
+void static_row_tables(const dd4dvar_grid& g, double dt, std::vector<double>& tab, ModelP& mp)
+{
+    const int nlat = g.nlat;
+    const double PI = 3.14159265358979323846;
+    const double dlam = 2.0 * PI / g.nlon, dth = PI / nlat, a = g.radius;
+    std::vector<double> mc(nlat);
+    tab.assign(6 * (size_t)nlat, 0.0);
+    double* dtcz = &tab[0]; double* gdtcz = &tab[nlat]; double* dtf = &tab[2 * (size_t)nlat];
+    double* dtt = &tab[3 * (size_t)nlat]; double* rp = &tab[4 * (size_t)nlat]; double* rm = &tab[5 * (size_t)nlat];
+    for (int j = 0; j < nlat; ++j) {
+        const double th = -0.5 * PI + (j + 0.5) * dth, c = cos(th);
+        mc[j] = c > g.cos_clamp ? c : g.cos_clamp;
+        const double cz = 1.0 / (2.0 * a * dlam * mc[j]);
+        dtcz[j] = dt * cz; gdtcz[j] = g.gravity * dt * cz;
+        dtf[j] = dt * 2.0 * g.omega * sin(th);
+        dtt[j] = dt * sin(th) / (a * mc[j]);
+    }
+    for (int j = 0; j < nlat; ++j) {
+        rp[j] = (j + 1 < nlat ? mc[j + 1] : mc[j]) / mc[j];
+        rm[j] = (j > 0 ? mc[j - 1] : mc[j]) / mc[j];
+    }
+    const double cm = 1.0 / (2.0 * a * dth);
+    mp.nlon = g.nlon; mp.nlat = nlat; mp.kap = g.diffusion;
+    mp.dtcm = dt * cm; mp.gdtcm = g.gravity * dt * cm;
+}
+
+// Variant of sk_forward_step (step_kernels.cuh) for the undecomposed grid: the descriptor of the one region travels as a
+// kernel argument, the row tables behind `m` and the time levels behind `levels` are inside dd_static_scratch.  The step
+// reads level `slot` and writes level `slot + 1` of `levels` ([.][3][nlat][nlon]); the region has no ghost ring
+// (periodic in longitude, pole walls), so no ghost store is read.  Same tile code as the handle-based forecast.
+__global__ void __launch_bounds__(SK_NT) sk_forward_step_static(Sub s, int slot, ModelP m, double* levels, int tiles_x)
+{
+    __shared__ double smf[SK_FWD_SMEM_DOUBLES];
+    sk_forward_tile(s, blockIdx.x % tiles_x, blockIdx.x / tiles_x, slot, m, levels, levels, smf,
+                    smf + 3 * (SK_TY + 6) * (SK_TX + 6), smf + 3 * (SK_TY + 6) * (SK_TX + 6) + 3 * (SK_TY + 4) * (SK_TX + 4));
+}
+
+int static_fail(char* h_err, size_t err_len, int code, const std::string& msg)
+{
+    if (h_err && err_len) { strncpy(h_err, msg.c_str(), err_len - 1); h_err[err_len - 1] = 0; }
+    return code;
+}
+
+}  // namespace
+
+extern "C" int dd4dvar_forecast_static(const dd4dvar_grid* grid, const dd4dvar_window* window, const double* d_x0,
+                                       int n_levels, const int* h_levels, double* d_out, void* cuda_stream,
+                                       char* h_err, size_t err_len)
+{
+    if (h_err && err_len) h_err[0] = 0;
+    if (!grid || !window || !d_x0 || n_levels < 0 || (n_levels && (!h_levels || !d_out)))
+        return static_fail(h_err, err_len, -1, "forecast_static: null argument");
+    if (grid->nlon < 3 || grid->nlat < 2 || window->nsteps < 1 || !(grid->radius > 0))
+        return static_fail(h_err, err_len, -1, "forecast_static: bad grid or window");
+    for (int q = 0; q < n_levels; ++q)
+        if (h_levels[q] < 0 || h_levels[q] > window->nsteps || (q && h_levels[q] < h_levels[q - 1]))
+            return static_fail(h_err, err_len, -1, "forecast_static: levels must ascend inside [0, nsteps]");
+    // size check first: tables (rounded up to 256 bytes) + at least two time levels must fit the static array
+    const size_t n3 = 3 * (size_t)grid->nlon * grid->nlat;
+    const size_t tab_doubles = (6 * (size_t)grid->nlat + 31) & ~size_t(31);
+    const size_t cap = tab_doubles < DD_STATIC_DOUBLES ? (DD_STATIC_DOUBLES - tab_doubles) / n3 : 0;
+    if (cap < 2) {
+        char msg[256];
+        snprintf(msg, sizeof msg,
+                 "forecast_static: a %d x %d grid needs %zu bytes of scratch (row tables + two time levels), the static "
+                 "array holds %zu; use dd4dvar_forecast with a caller-allocated workspace",
+                 grid->nlon, grid->nlat, sizeof(double) * (tab_doubles + 2 * n3), (size_t)DD4DVAR_STATIC_SCRATCH_BYTES);
+        return static_fail(h_err, err_len, -6, msg);
+    }
+    Layout G;
+    if (build_layout(G, grid->nlon, grid->nlat, window->nsteps, 1, 1, 1, 0))
+        return static_fail(h_err, err_len, -2, "forecast_static: the grid cannot be laid out");
+    std::string err;
+    double* base = nullptr;
+    int rc = static_scratch_base(&base, err);      // first call on a device: symbol look-up (set-up; keep it out of stream capture)
+    if (rc) return static_fail(h_err, err_len, rc, "forecast_static: " + err);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+#define CUS(call)                                                                                              \
+    do {                                                                                                       \
+        e = (call);                                                                                            \
+        if (e != cudaSuccess)                                                                                  \
+            return static_fail(h_err, err_len, -4, std::string("forecast_static: " #call ": ") + cudaGetErrorString(e)); \
+    } while (0)
+    // Nothing in the array has to start at zero: the tables and level 0 are rewritten here, and every later level is
+    // written in full by the step that produces it before anything reads it.  What the last call left is overwritten.
+    std::vector<double> tab;
+    ModelP mp{};
+    static_row_tables(*grid, window->dt, tab, mp);
+    const int nlat = grid->nlat;
+    mp.dtcz = base; mp.gdtcz = base + nlat; mp.dtf = base + 2 * (size_t)nlat;
+    mp.dtt = base + 3 * (size_t)nlat; mp.rp = base + 4 * (size_t)nlat; mp.rm = base + 5 * (size_t)nlat;
+    double* levels = base + tab_doubles;
+    CUS(cudaMemcpyAsync(base, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice, st));
+    CUS(cudaMemcpyAsync(levels, d_x0, sizeof(double) * n3, cudaMemcpyDeviceToDevice, st));
+    const Sub s = G.hs[0];
+    int q = 0;
+    while (q < n_levels && h_levels[q] == 0) {
+        CUS(cudaMemcpyAsync(d_out + (size_t)q * n3, levels, sizeof(double) * n3, cudaMemcpyDeviceToDevice, st));
+        ++q;
+    }
+    // the array holds `cap` consecutive levels; when the next step would run past its end, the newest level moves to
+    // slot 0 and the stepping goes on from there
+    size_t slot = 0;
+    for (int n = 0; n < window->nsteps && q < n_levels; ++n) {
+        if (slot + 1 == cap) {
+            CUS(cudaMemcpyAsync(levels, levels + slot * n3, sizeof(double) * n3, cudaMemcpyDeviceToDevice, st));
+            slot = 0;
+        }
+        sk_forward_step_static<<<G.ntiles, SK_NT, 0, st>>>(s, (int)slot, mp, levels, G.tiles_x);
+        CUS(cudaGetLastError());
+        ++slot;
+        while (q < n_levels && h_levels[q] == n + 1) {
+            CUS(cudaMemcpyAsync(d_out + (size_t)q * n3, levels + slot * n3, sizeof(double) * n3, cudaMemcpyDeviceToDevice, st));
+            ++q;
+        }
+    }
+    CUS(cudaStreamSynchronize(st));
+    CUS(cudaGetLastError());
+#undef CUS
+    return 0;
+}
