@@ -77,15 +77,14 @@ typedef struct {
 
 /* Local minimiser (L-BFGS, R10): history length, iterations per outer iteration,
  * maximum number of step halvings, Armijo constant.
- * path: 0 = choose automatically, 1 = force the generic kernels (one block-tiled launch per step,
- *       any tile size), 2 = force the fused persistent kernels (create fails with -2 if a tile
- *       does not fit), 3 = force the per-stage generic kernels (cross-check),
- *       4 = wavefront forward kernel (shared-memory resident tile, TMA-staged rows, cost terms fused)
- *       + row-marching adjoint kernel, 5 = wavefront forward + wavefront adjoint kernels
- *       (4 and 5: create fails with -2 unless every tile has a ghost ring in longitude, an even
- *       number of columns, at most 100 padded columns, an extended tile of at most 49 rows (80 rows
- *       up to 68 padded columns), and every window at least 4 steps; "cost terms fused" is the round-1
- *       wording: the cost terms run in the kernel ck_cost between the two sweeps). */
+ * path: 0 = choose automatically (5 where eligible, else 2, else 1), 1 = force the generic kernels (one block-tiled
+ *       launch per step, any tile size), 2 = force the fused row-marching kernels (create fails with -2 if a tile does
+ *       not fit), 3 = force the per-stage generic kernels (cross-check), 4 = wavefront forward kernel (tile resident in
+ *       shared memory, one time step per warp, TMA-staged rows) + row-marching adjoint kernel, 5 = wavefront forward +
+ *       wavefront adjoint kernels.  On 4 and 5 the cost terms (25a)-(25c) run in the kernel ck_cost between the two
+ *       sweeps.  4 and 5: create fails with -2 unless every tile has a ghost ring in longitude, an even number of
+ *       columns, at most 100 padded columns, an extended tile of at most 49 rows (80 rows up to 68 padded columns),
+ *       and every window at least 4 steps. */
 typedef struct {
     int lbfgs_m, n_inner, max_backtrack;
     double armijo_c1;
@@ -159,8 +158,10 @@ int dd4dvar_eval_local(dd4dvar_t h, const double* d_controls, double* h_costs, d
                        double* d_grads);
 
 /* The same evaluation end to end with HOST buffers: h_controls is copied to the device, the
- * gradient sweep runs, costs and (if h_grads != NULL) gradients are copied back.  Pinned host
- * memory makes the copies asynchronous with respect to the host but they are inside the call.
+ * gradient sweep runs, costs and (if h_grads != NULL) gradients are copied back; the copies are inside the call.
+ * The overlap of copies and sweeps described next needs PINNED (page-locked) host buffers: with pageable memory every
+ * copy blocks the host until it is done, the next chunk's sweep is queued late, and the call is correct but no faster
+ * than copy + sweep + copy in sequence.
  * With 64 or more subdomains the evaluation runs in six chunks of consecutive subdomains (they are independent:
  * all neighbour data is frozen) so that the copies of one chunk overlap the sweeps of the others (on the wavefront
  * path the chunks are whole rounds of the persistent grid, 1, 2, .. rounds from either end); the library
@@ -191,7 +192,6 @@ int dd4dvar_get_local_trajectory(dd4dvar_t h, int sub, double* d_out);
 int dd4dvar_forecast(dd4dvar_t h, const double* d_x0, int n_levels, const int* h_levels,
                      double* d_out);
 
-int dd4dvar_num_subdomains(dd4dvar_t h);
 /* Forecast for callers that cannot give the library any device memory of their own making.
  *
  * Every other entry point works out of a workspace that the caller allocates (dd4dvar_set_workspace).  Some callers
@@ -227,13 +227,14 @@ int dd4dvar_forecast_static(const dd4dvar_grid* grid, const dd4dvar_window* wind
                             int n_levels, const int* h_levels, double* d_out, void* cuda_stream,
                             char* h_err, size_t err_len);
 
+int dd4dvar_num_subdomains(dd4dvar_t h);
 /* out[16] = tile_col, tile_row, window, owned i0,i1,j0,j1, ext i0 (may be < 0: wraps), ext j0,
  * ex, ey, ghost width lon, ghost south, ghost north, first level s, last level e. */
 int dd4dvar_subdomain_info(dd4dvar_t h, int sub, int out[16]);
 /* offset (in doubles) of subdomain `sub` inside an "all subdomains" array; sub = nsub gives the
  * total length. */
 long long dd4dvar_control_offset(dd4dvar_t h, int sub);
-/* which kernels serve the local sweeps: 1 generic, 2 fused persistent */
+/* which kernels serve the local sweeps: the value of dd4dvar_opts.path in effect, 1 .. 5 (see there) */
 int dd4dvar_active_path(dd4dvar_t h);
 
 /* Weight of the background term (25a) l.338 in the time windows j > 0 (R7).  The paper is
@@ -270,7 +271,7 @@ int dd4dvar_gather_analysis(dd4dvar_t h, double* d_analysis);
  * default).  on = 1: on every level of the window, eq (21) l.300 read literally (O_ik maps onto Delta_j x (Omega_i n
  * Omega_k)); the neighbours' frozen trajectories on the overlap rectangles are then kept in a second store,
  * refreshed at every exchange.  Served by the generic kernels only: create with opts.path = 1, else -2; call
- * before dd4dvar_set_background, else -3.  Not available with dd4dvar_run_gn. */
+ * before dd4dvar_set_background, else -3.  dd4dvar_run_gn and dd4dvar_gn_hessvec return -2 while it is on. */
 int dd4dvar_set_overlap_levels(dd4dvar_t h, int on);
 
 /* Measurement aid ("which roofline binds"): microbenchmarks of the device's

@@ -521,29 +521,9 @@ void adjoint_only(dd4dvar_t h, Layout& L, const int* mask, double* gw)
     if (L.path == 5) {
         // (consumes the control-level part of the gradient that ck_cost left in gx: one adjoint sweep per forward sweep)
         WkArgs a = wave_args(h, L, mask, nullptr, gw);
-#ifdef WK_PROF
-        static unsigned long long* d_prof = nullptr;
-        if (!d_prof) cudaMalloc(&d_prof, 8 * 16 * 8);
-        cudaMemsetAsync(d_prof, 0, 8 * 16 * 8, h->stream);
-        a.J = reinterpret_cast<double*>(d_prof);
-#endif
         if (L.wp.K == 2) wk_adjoint<2><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
         else wk_adjoint<3><<<L.wp.grid, WK_NT, L.wp.smem_adj, h->stream>>>(a);
         ++h->launches;
-#ifdef WK_PROF
-        {
-            unsigned long long hp[8 * 16];
-            cudaStreamSynchronize(h->stream);
-            cudaMemcpy(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost);
-            static int nprint = 0;
-            if (nprint++ < 1)
-                for (int w = 0; w < 8; ++w) {
-                    fprintf(stderr, "[wkprof adj] warp %d:", w);
-                    for (int q = 0; q < 8; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
-                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, prep-wait, loads+row1, A+scatter, elected, obs, stores, gap)\n");
-                }
-        }
-#endif
         if (gw) LAUNCH(ck_scale_grad, dim3(std::min(32, (3 * L.maxncell + 255) / 256), L.nsub), 256, L.dsubs, mask, h->cp, L.gx, gw);
         return;
     }
@@ -578,21 +558,6 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
         if (L.wp.K == 2) wk_forward<2><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         else wk_forward<3><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         ++h->launches;
-#ifdef WK_PROF
-        {
-            unsigned long long hp[8 * 16];
-            cudaStreamSynchronize(h->stream);
-            cudaMemcpy(hp, d_prof, sizeof(hp), cudaMemcpyDeviceToHost);
-            static int nprint = 0;
-            if (nprint++ < 2)
-                for (int w = 0; w < 8; ++w) {
-                    fprintf(stderr, "[wkprof fwd] warp %d:", w);
-                    for (int q = 0; q < 8; ++q) fprintf(stderr, " %.3f", hp[w * 16 + q] * 1e-6 / L.wp.grid);
-                    fprintf(stderr, "  (Mcycles per CTA: wait_leader, chunk+ghostcopy, loads+A+h1+u1, v1+STS+fence, obs, lane0 block, -, loop-gap)\n");
-                }
-            a.gw = gw;
-        }
-#endif
         ck_cost<<<L.nsub, CK_NT, 0, h->stream>>>(a);
         ++h->launches;
         if (with_adjoint) adjoint_only(h, L, mask, gw);
@@ -1272,6 +1237,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
         sweep(h, L, false, nullptr, L.st.J, nullptr);
         if (l == 1 && n_gn == 0 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
         if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
+    if (h->overlap_levels) return fail(h, -2, "gn_hessvec: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
         exchange(h, L);
         CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
         if ((rc = sync_check(h))) return rc;
@@ -1288,6 +1254,7 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
 {
     if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
     h->cp.bgw = w_later;
+    if (h->overlap_levels) return fail(h, -2, "run_gn: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
     return 0;
 }
 

@@ -40,9 +40,7 @@ struct FusedPlan {
     int* counter = nullptr;
 };
 #define FK_SMS 148                  // B200
-#ifndef FK_ADJ_CTAS
 #define FK_ADJ_CTAS 3                // resident adjoint CTAs per SM at 128 threads (register budget 168)
-#endif
 typedef void* (*fused_take_fn)(void* arena, size_t bytes);
 
 inline bool fused_fits(const Sub* subs, int nsub)

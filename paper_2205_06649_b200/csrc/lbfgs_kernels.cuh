@@ -9,9 +9,7 @@
 #include "common.cuh"
 namespace cg = cooperative_groups;
 
-#ifndef LK_CL
 #define LK_CL 4      // CTAs per cluster = per subdomain
-#endif
 
 struct LbfgsP {
     int m, max_bt;

@@ -36,9 +36,6 @@
 #pragma once
 #include "wave_common.cuh"
 
-#ifndef WK_APAIR
-#define WK_APAIR 1        // 1: the ticks without a pole-wall event run in pairs (no register moves); 0: one tick body + rotation (smaller code)
-#endif
 
 template <int K> struct WaState {     // every history has depth one: slot [t & 1] is written at tick t and read at tick t + 1
     double zc[2][3][K];             // [slot][field][column]: Z^{n-1} row t-1 (own columns), kept for one tick as row t-2
@@ -70,9 +67,6 @@ template <int K> struct WaCtx {
     long long qcur, qend;
     int p_pk; double p_r;
     unsigned par;                   // bits 0..2: ring slots, bits 3, 4: E/W chunk slots
-#ifdef WK_PROF
-    long long pf[8], pt;
-#endif
 };
 
 // lane 0: padded row r of Z^{n-1} -> ring slot r % 3 (ghost rows whole, tile rows at columns 3 .. 3+ex)
@@ -164,8 +158,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     double zN[3][K];                                // row t (re-read as row t-1 by the next tick: the ring still holds it)
     double (&zC)[3][K] = S.zc[pn];
     double (&zS)[3][K] = S.zc[po];
-    WKP(7)
-
     // ---- (0) the leader has finished row t of lambda^n and u^n; H^T R^-1 (25b) forcing on that row.  First in the tick:
     // the read-modify-write of the forcing and the first step's row copies complete behind stages (1) and (2a), which
     // work on the warp's private ring (4.43 -> 4.33 ms against the poll after stage (2a); one poll per pair of ticks: 4.29 ms)
@@ -178,7 +170,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         wa_issue_lamrow<K>(C, lj + 2);
         __syncwarp();
     }
-    WKP(0)
     if (tile && C.have_obs) {
         const WkArgs& A = *C.A;
         for (;;) {
@@ -193,8 +184,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         }
         __syncwarp();
     }
-    WKP(5)
-
     // ---- (1) Z^{n-1}: own columns of row t, E/W halo and edge u^a of row t-1
     double eL, eR;
     {
@@ -267,8 +256,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         }
         uaW = 0.0; uaE = 0.0;
     }
-    WKP(2)
-
     // ---- (2b) lambda^n: v rows t, t-1, t-2; h, u and u^n row t-1.  UB, HB, P and the row-local parts of A on row t-1
     const uint32_t lrow = C.la0 + (uint32_t)lj * PL8;      // own cell 0 of lambda_h, tile row lj (may lie outside the tile)
     double P1[K];
@@ -328,8 +315,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
             S.HB[pn][i] = 0.0; S.Au[pn][i] = 0.0; S.e[pn][i] = 0.0; S.avp[pn][i] = 0.0;
         }
     }
-    WKP(3)
-
     // ---- (3) row t-2: A_h, A_u, A_v completed; (4) scatter into L0 of rows t-1, t-2, t-3
     double (&Ln)[3][K] = S.mN[pn];                  // L0 of row t-1: northward part of the scatter from row t-2
     double (&La)[3][K] = S.La[pn];                  // L0 of row t-2 (its southward part arrives at the next tick)
@@ -377,8 +362,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     }
 #pragma unroll
     for (int i = 0; i < K; ++i) S.P[pn][i] = P1[i];
-    WKP(6)
-
     // ---- (5) row t-3 of lambda^{n-1} is complete; u^{n-1} of row t-2 replaces u^n
     {
         const bool st3 = (unsigned)(lj - 3) < (unsigned)g.ey;
@@ -408,7 +391,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
     // the next row of Z^{n-1} must have landed; its ghost cells go in place
     if (t + 1 < g.py) wa_prep_row<K>(C, sm, t + 1);
     __syncwarp();
-    WKP(1)
     // ---- (6) one lane: progress word, the row after next, next E/W chunk
     if (wk_elect()) {
         wk_publish(C.a_mine, C.gs10 + (unsigned)t + 1u);
@@ -417,7 +399,6 @@ __device__ __forceinline__ void wa_tick(const int t, WaState<K>& S, WaCtx<K>& C,
         if ((unsigned)l1 < (unsigned)g.ey && (l1 % WK_EWCA) == WK_EWCA - 1 && l1 / WK_EWCA + 2 < C.nchunk)
             wa_issue_chunk<K>(C, l1 / WK_EWCA + 2);
     }
-    WKP(4)
 }
 
 // after a single tick run at slot 0: move every history to slot 1, where the next tick at slot 0 reads it
@@ -465,9 +446,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
     C.la0 = sm32 + 8u * (Ly.st + K * lane);
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm; C.c0k = 1.0 - 4.0 * A.m.kap; C.mu2 = 2.0 * A.cp.mu;
     C.A = &A; C.par = 0u;
-#ifdef WK_PROF
-    for (int q = 0; q < 8; ++q) C.pf[q] = 0;
-#endif
 
     // Every warp walks the same list of (subdomain, adjoint step) pairs (see wk_forward).
     int nord = -1;                              // ordinal of the current subdomain in this CTA's list
@@ -551,14 +529,8 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                 wa_issue_lamrow<K>(C, -g.gys);
                 wa_issue_lamrow<K>(C, 1 - g.gys);
             }
-#if WK_STAGGER
-            if (C.has_leader && !C.first) { const int nd = WK_STAGGER < C.TLd + 1 ? WK_STAGGER : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
-#endif
             wa_prep_row<K>(C, sm, 0);           // (the ring is private to this warp: no leader involved)
             __syncwarp();
-#ifdef WK_PROF
-            C.pt = clock64();
-#endif
             // ticks [0, tp0) and [tp1, T): one at a time (pole-wall events, odd remainder); ticks [tp0, tp1): in
             // pairs (a pair returns every history to the register slot it started in: no register moves)
             const int tp0 = g.ws ? 3 : 0;
@@ -574,7 +546,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                     else wa_tick<K, 0, false>(t, S, C, sm, tab);
                     wa_rotate<K>(S);
                 }
-#if WK_APAIR
                 if (ph == 0) {
 #pragma unroll 1
                     for (; t < tp1; t += 2) {
@@ -582,7 +553,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
                         wa_tick<K, 1, false>(t + 1, S, C, sm, tab);
                     }
                 }
-#endif
             }
             if (C.first) wk_cpa_wait<0>();
             if (wk_elect()) wk_publish(C.a_mine, C.gs10 + (unsigned)C.T + 1u);
@@ -590,13 +560,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_adjoint(const __grid_constant__ W
         }
         }
         glast = gnext + (unsigned)g.W - 1u;
-        gnext = glast + 1u + WK_SKIP;
+        gnext = glast + 1u;
         TL = T; gysL = g.gys;
     }
-#ifdef WK_PROF
-    if (lane == 0 && A.J) {
-        unsigned long long* pr = reinterpret_cast<unsigned long long*>(A.J);
-        for (int q = 0; q < 8; ++q) atomicAdd(pr + w * 16 + q, (unsigned long long)C.pf[q]);
-    }
-#endif
 }

@@ -31,12 +31,6 @@
 #define WK_NW 8                 // warps per CTA = time steps in flight per CTA
 #endif
 #define WK_NT (WK_NW * 32)
-#ifndef WK_SKIP
-#define WK_SKIP 0u         // step numbers skipped between two subdomains (1u rotates the warp <-> level assignment: no gain, 4 idle ticks)
-#endif
-#ifndef WK_STAGGER
-#define WK_STAGGER 0            // ticks a step starts behind its leader (0: as soon as the data allows, 4 ticks)
-#endif
 #define WK_EWC 4                // tile rows per staged chunk of east/west ghost cells (forward kernel)
 #define WK_EWCA 2               // the same in the adjoint kernel (its shared memory is full)
 #define WK_HDR 128              // doubles reserved at the start of shared memory (barriers, flags)
@@ -150,16 +144,10 @@ __device__ __forceinline__ void wk_mbar_init32(uint32_t bar, int count)
 }
 __device__ __forceinline__ void wk_mbar_expect32(uint32_t bar, uint32_t bytes)
 {
-#ifdef WK_NODMA
-    return;
-#endif
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void wk_mbar_wait32(uint32_t bar, uint32_t parity)
 {
-#ifdef WK_NODMA
-    return;
-#endif
     uint32_t ok;
     do {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
@@ -168,17 +156,11 @@ __device__ __forceinline__ void wk_mbar_wait32(uint32_t bar, uint32_t parity)
 }
 __device__ __forceinline__ void wk_g2s32(uint32_t dst, const double* src, uint32_t bytes, uint32_t bar)
 {
-#ifdef WK_NODMA
-    return;
-#endif
     asm volatile("cp.async.bulk.shared::cta.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void wk_s2g32(double* dst, uint32_t src, uint32_t bytes)
 {
-#ifdef WK_NODMA
-    return;
-#endif
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void wk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
@@ -190,32 +172,21 @@ template <int N> __device__ __forceinline__ void wk_wait_read()
 __device__ __forceinline__ void wk_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void wk_fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 // Progress words.  Writer: every lane stores its cells of the row (st.shared), __syncwarp, then ONE lane stores
-// the word; reader: polls the word, then loads the row.  Both sides use plain volatile accesses unless
-// WK_FENCED_FLAGS is defined: the data and the word are shared-memory accesses of the same SM, which its
-// shared-memory pipe performs in issue order (a store issued after another by the same warp becomes visible
-// after it; a load issued after the poll that saw the word cannot see older data), so the release / acquire
-// fences (MEMBAR.ALL.CTA in SASS, once per tick on either side) buy nothing here.
+// the word with release semantics; reader: polls the word with acquire semantics, then loads the row.  The pair
+// st.release.cta / ld.acquire.cta is what the PTX memory model asks for between the row data (weak accesses) and the
+// word; it costs one MEMBAR.ALL.CTA per tick on either side (about 1 % of the sweep against plain volatile accesses,
+// DESIGN.md section 5), which is the price of not resting the hot path on the issue order of one SM's shared-memory pipe.
 __device__ __forceinline__ void wk_publish(uint32_t addr, unsigned v)
 {
-#ifdef WK_FENCED_FLAGS
     asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-#else
-    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
-#endif
 }
 __device__ __forceinline__ unsigned wk_peek(uint32_t addr)
 {
     unsigned v;
-#ifdef WK_FENCED_FLAGS
     asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
-#else
-    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
-#endif
     return v;
 }
-#ifndef WK_BACKOFF
 #define WK_BACKOFF __nanosleep(40)
-#endif
 // wait until the progress word at `addr` has reached `need` (monotone counters, wrap-safe compare)
 __device__ __forceinline__ void wk_wait_prog(uint32_t addr, unsigned need)
 {
@@ -255,26 +226,9 @@ __device__ __forceinline__ void wk_copy_tab(double* dst, const double* __restric
 #define WK_BAR_PER_WARP 8       // mbarriers per warp at the start of shared memory
 #define WK_PROG 64              // progress words (one u32 per warp) at double index WK_PROG
 
-// Position of a physical warp in the step order.  Warps p and p + 4 share a scheduler (SM sub-partition);
-// WK_PAIR_DIST is the distance of such a pair in the step order (4: identity).  Consecutive steps run about
-// 0.8 tick apart in phase, so the distance decides how much the compute phases of a pair overlap.
-#ifndef WK_PAIR_DIST
-#define WK_PAIR_DIST 4
-#endif
-__device__ __forceinline__ int wk_logical_warp(int p)
-{
-#if WK_NW == 8 && WK_PAIR_DIST == 3
-    const int a[4] = { 0, 6, 4, 2 }, b[4] = { 3, 1, 7, 5 };
-    return p < 4 ? a[p] : b[p - 4];
-#elif WK_NW == 8 && WK_PAIR_DIST == 2
-    const int a[4] = { 0, 4, 1, 5 }, b[4] = { 2, 6, 3, 7 };
-    return p < 4 ? a[p] : b[p - 4];
-#elif WK_NW == 8 && WK_PAIR_DIST == 1
-    return p < 4 ? 2 * p : 2 * (p - 4) + 1;
-#else
-    return p;
-#endif
-}
+// Position of a physical warp in the step order: the identity.  (Warps p and p + 4 share a scheduler; other distances of
+// such a pair in the step order were measured and bought nothing, profiles/r2_wave_v2.md.)
+__device__ __forceinline__ int wk_logical_warp(int p) { return p; }
 
 // one elected lane of the (converged) warp; tells the compiler the region is single-threaded
 __device__ __forceinline__ bool wk_elect()
@@ -291,7 +245,7 @@ __device__ __forceinline__ int wk_uni(int v) { return __shfl_sync(0xffffffffu, v
 template <int OFF> __device__ __forceinline__ double wk_lds(uint32_t a)
 {
     double v;
-    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF));
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF) : "memory");
     return v;
 }
 template <int OFF> __device__ __forceinline__ void wk_sts(uint32_t a, double v)

@@ -22,14 +22,11 @@
 // trajectory store: 2 % of the points), the level-0 copy of the trajectory store and the successor-window term
 // run in ck_cost (cost_kernels.cuh) after this kernel: with observations every 8th level and 8 steps in flight
 // one of the steps of the pipeline always carried observations and set the pace of all (7 % of the kernel).
-// There is ONE tick body (uniform branches only, the hot loop must stay inside the instruction
-// cache); the tick loop is unrolled by three so that the row histories rotate by renaming.
+// The ticks without a wall event run a steady body, one tick per loop iteration (the hot loop must stay inside the
+// instruction cache: unrolling by 3 or 6 was slower, profiles/r2_wave_v2.md); the others a general body with uniform branches.
 #pragma once
 #include "wave_common.cuh"
 
-#ifndef WK_FUNROLL
-#define WK_FUNROLL 1      // steady ticks per loop iteration: 1 (register moves, but the loop body stays inside the instruction cache: 3.28 ms), 3 (3.63 ms), 6 (6.67 ms); 0: no steady tick (3.87 ms)
-#endif
 #define WK_XD 3         // a first step fetches its control rows this many ticks ahead (4 mbarrier slots: WK_XD <= 3)
 
 
@@ -58,16 +55,7 @@ template <int K> struct WfCtx {
     const double *gz, *ge; double* tout;
     const WkArgs* A;
     unsigned par;
-#ifdef WK_PROF
-    long long pf[8], pt;
-#endif
 };
-#ifdef WK_PROF
-#define WKP(i) { const long long c_ = clock64(); C.pf[i] += c_ - C.pt; C.pt = c_; }
-#else
-#define WKP(i)
-#endif
-
 template <int K>
 __device__ __forceinline__ void wf_issue_chunk(const WfCtx<K>& C, int c)
 {   // lane 0: E/W ghost cells + edge u^a of tile rows [c*EWC, ...) -> staging slot c & 1
@@ -133,11 +121,9 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
     const int lj = t - g.gys;                       // tile row of padded row t (if it is one)
     const bool tile = (unsigned)lj < (unsigned)g.ey;
     // ---- (0) row t becomes readable
-    WKP(7)
     if (C.has_leader && !(t & 1)) {             // (one poll for two ticks: every even tick waits for what the next one needs)
         const int nd = t + 1 + C.dlead < C.TLd + 1 ? t + 1 + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
     }
-    WKP(0)
     int ra = 0, rfs = 0, re = 0;                    // own column 0 of row t, field stride, edge-u^a index
     if (tile) {                                      // (its E/W ghost cells were put in place one tick earlier)
         if (C.first) wf_wait_xrow<K>(C, lj);
@@ -149,8 +135,6 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
         const int rr = north ? lj - g.ey : t;
         ra = C.I_SN + rr * g.px + C.c0; rfs = 3 * g.px; re = C.I_EDS + (north ? 8 : 0) + rr * 2;
     }
-
-    WKP(1)
     // ---- (1) loads: own columns of row t, E/W halo of row t-1
     double z0[3][K], hz[3][2];
     if (t < g.py) {
@@ -230,8 +214,6 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
 #pragma unroll
         for (int i = 0; i < K; ++i) { h12[i] = (t == g.py + 2 && g.wn) ? R.h13[i] : 0.0; u12[i] = 0.0; }
     }
-
-    WKP(2)
     // ---- (4) v^1 on row t-3: row t-3 of Z^{n+1} is complete
     const int l3 = lj - 3;
     const bool out = (unsigned)l3 < (unsigned)g.ey;
@@ -245,13 +227,11 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
         }
     }
     wk_fence_async();
-    WKP(3)
     // E/W ghost cells and edge u^a of the NEXT row go next to its tile row (the leader read them two ticks ago)
     const int l1 = lj + 1;
     const bool prep = (unsigned)l1 < (unsigned)g.ey;
     if (prep) wf_prep_row<K>(C, sm, l1);
     __syncwarp();
-    WKP(1)
     // ---- (5) one lane: progress word, trajectory stores, refills of the staging buffers
     if (wk_elect()) {
         // a follower overwrites row r after my tick r+6 is published: the store issued three ticks ago must have left
@@ -268,9 +248,6 @@ __device__ __forceinline__ void wf_tick(const int t, WfRegs<K>& R, WfCtx<K>& C, 
         if (C.first && (unsigned)(lj + WK_XD) < (unsigned)g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
         if (prep && (l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
     }
-    WKP(4)
-
-    WKP(5)
     // ---- (6) rotate the row histories
 #pragma unroll
     for (int i = 0; i < K; ++i) {
@@ -292,12 +269,10 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
     const WkGeo& g = C.g;
     const int lj = t - g.gys;
     constexpr uint32_t P8 = 8u * WfCtx<K>::P, FS8 = 8u * WfCtx<K>::FS;
-    WKP(7)
     if (C.has_leader && !(t & 1)) {             // (one poll for two ticks: every even tick waits for what the next one needs)
         const int nd = t + 1 + C.dlead < C.TLd + 1 ? t + 1 + C.dlead : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd);
     }
     if (C.first) wf_wait_xrow<K>(C, lj);
-    WKP(0)
     // ---- loads: own columns of row t, E/W halo and edge u^a of row t-1
     const uint32_t urow = C.sm32 + 8u * (C.st + lj * C.P);          // tile row lj, tile column 0, field 0
     const uint32_t a0 = urow + 8u * (C.c0 - 3), a1 = a0 + FS8, a2 = a1 + FS8;
@@ -349,7 +324,6 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
             u12[i] = mm_u1(R.ua2[i], R.va2[i], hE, hW, gdtcz2, dtf2, dtt2);
         }
     }
-    WKP(2)
     // ---- v^1 on row t-3 -> row t-3 of Z^{n+1}
     {
         const double dtf3 = tab[t * 8 - 16 + WK_T_DTF], dtt3 = tab[t * 8 - 16 + WK_T_DTT];
@@ -362,7 +336,6 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
         if (K > 2 && (C.tmask & 4u)) { wk_sts<16>(o0, R.h13[K > 2 ? 2 : 0]); wk_sts<16>(o1, R.u13[K > 2 ? 2 : 0]); wk_sts<16>(o2, v1[K > 2 ? 2 : 0]); }
         wk_fence_async();
     }
-    WKP(3)
     // ---- E/W ghost cells and edge u^a of row t+1 next to its tile row
     const int l1 = lj + 1, l3 = lj - 3;
     {
@@ -374,7 +347,6 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
         }
     }
     __syncwarp();
-    WKP(1)
     // ---- one lane: progress word, trajectory stores, next E/W chunk
     if (wk_elect()) {
         wk_wait_read<2>();
@@ -386,9 +358,6 @@ __device__ __forceinline__ void wf_tick_steady(const int t, WfRegs<K>& R, WfCtx<
         if ((l1 % WK_EWC) == WK_EWC - 1 && l1 / WK_EWC + 2 < C.nchunk) wf_issue_chunk(C, l1 / WK_EWC + 2);
         if (C.first && lj + WK_XD < g.ey) wf_issue_xrow<K>(C, lj + WK_XD);
     }
-    WKP(4)
-
-    WKP(5)
     // ---- rotate the row histories
 #pragma unroll
     for (int i = 0; i < K; ++i) {
@@ -426,9 +395,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
     C.kap = A.m.kap; C.dtcm = A.m.dtcm; C.gdtcm = A.m.gdtcm;
     C.A = &A; C.par = 0u;
     constexpr int FS = WfCtx<K>::FS;
-#ifdef WK_PROF
-    for (int q = 0; q < 8; ++q) C.pf[q] = 0;
-#endif
 
     // Every warp walks the same list of (subdomain, step) pairs; global step number gs (1, 2, ...) belongs
     // to warp (gs - 1) % WK_NW, and the step gs - 1 is its leader whatever subdomain it belongs to.
@@ -489,14 +455,6 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             }
             R.uaL2 = R.uaR2 = 0.0; R.pa = C.I_SN + 1; R.pfs = 0; R.pe = C.I_EDS;
 
-#ifdef WK_PROF
-            C.pt = clock64();
-#endif
-#if WK_STAGGER
-            // start WK_STAGGER ticks (not just the 4 the data needs) behind the leader: the spare ticks absorb the
-            // jitter of the steps ahead; 8 steps x 7 ticks still fit into the ticks of one step
-            if (C.has_leader && !C.first) { const int nd = WK_STAGGER < C.TLd + 1 ? WK_STAGGER : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
-#endif
             if (C.first || g.gys == 0) {
                 // what tick -1 would do: the control rows that ticks 0 and 1 read, the ghost cells of tile row 0
                 if (C.has_leader) { const int nd = C.dlead - 1 < C.TLd + 1 ? C.dlead - 1 : C.TLd + 1; wk_wait_prog(C.a_lead, C.need0 + (unsigned)nd); }
@@ -514,36 +472,10 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
             const int ts1 = g.gys + g.ey - 1;
 #pragma unroll 1
             for (int t = 0; t < C.T;) {
-#if WK_FUNROLL == 6
-                if (t >= ts0 && t + 6 <= ts1) {
-                    wf_tick_steady<K>(t, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 1, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 2, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 3, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 4, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 5, R, C, sm, tab);
-                    t += 6;
-                    const int rowb = C.st + (t - 1 - g.gys) * C.P;
-                    R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
-                } else
-#endif
-#if WK_FUNROLL == 0
-                if (false) {
-                } else
-#elif WK_FUNROLL == 1
                 if (t >= ts0 && t + 1 <= ts1) {
                     wf_tick_steady<K>(t, R, C, sm, tab);
                     t += 1;
                     const int rowb = C.st + (t - 1 - g.gys) * C.P;
-                    R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
-                } else
-#endif
-                if (WK_FUNROLL == 3 && t >= ts0 && t + 3 <= ts1) {
-                    wf_tick_steady<K>(t, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 1, R, C, sm, tab);
-                    wf_tick_steady<K>(t + 2, R, C, sm, tab);
-                    t += 3;
-                    const int rowb = C.st + (t - 1 - g.gys) * C.P;      // row t-1 for the generic tick that may follow
                     R.pa = rowb - 3 + C.c0; R.pfs = C.FS; R.pe = rowb + g.ex + 3;
                 } else {
                     wf_tick<K>(t, R, C, sm, tab);
@@ -556,13 +488,7 @@ __global__ void __launch_bounds__(WK_NT, 1) wk_forward(const __grid_constant__ W
         }
         }
         glast = gnext + (unsigned)g.W - 1u;
-        gnext = glast + 1u + WK_SKIP;
+        gnext = glast + 1u;
         TL = T; gysL = g.gys;
     }
-#ifdef WK_PROF
-    if (lane == 0 && A.gw) {
-        unsigned long long* pr = reinterpret_cast<unsigned long long*>(A.gw);
-        for (int q = 0; q < 8; ++q) atomicAdd(pr + w * 16 + q, (unsigned long long)C.pf[q]);
-    }
-#endif
 }

@@ -59,3 +59,21 @@ def test_option_is_refused_where_it_is_not_served():
     with pytest.raises(Exception) as e:
         g.set_overlap_levels(False)
     assert getattr(e.value, "code", 0) == -3
+
+
+def test_gauss_newton_entry_points_refuse_the_all_level_overlap_penalty():
+    """include/dd4dvar.h: dd4dvar_run_gn and dd4dvar_gn_hessvec return -2 while dd4dvar_set_overlap_levels is on
+    (there is no Gauss-Newton path for the all-level penalty; running it would silently drop the term's curvature)."""
+    from paper_2205_06649_b200.binding import DD4DVarError
+    w = small_workload()
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob, overlap_levels=True, path=1)
+    x = g.get_controls()
+    with pytest.raises(DD4DVarError) as e1:
+        g.gn_hessvec(x, x)
+    with pytest.raises(DD4DVarError) as e2:
+        g.run_gn(1, 1, 1)
+    assert e1.value.code == -2 and e2.value.code == -2
+    assert "overlap_levels" in str(e1.value)
+    g.run(1)                                   # the L-BFGS driver still serves it
+    g.close()

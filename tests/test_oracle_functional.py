@@ -67,6 +67,28 @@ def test_local_gradient_vs_centred_finite_differences(c0):
         fd_check(lambda z: o.eval_local(k, z, want_grad=False)[0][0], x, g, sb, range(200, 204))
 
 
+@pytest.mark.parametrize("bgw", [0.0, 1.0])
+def test_local_gradient_vs_centred_differences_on_tiles_with_ghost_rows_on_both_sides(bgw):
+    """The same pin on a 3 x 3 x 2 layout with overlap 2, AFTER one outer iteration (frozen neighbour data that is not
+    the background any more), for both weights of (25a) in the later window (R7).  The middle tile row has
+    ghost rows north and south, like every interior tile of configs 1-3; config 0's 2 x 2 tiles all touch a pole wall, so
+    the test above never sees the adjoint of a step whose ghost ring is dropped on every side."""
+    from helpers import small_workload
+    w = small_workload(nlon=48, nlat=30, dt=600.0, nsteps=8, p_lon=3, p_lat=3, q_time=2, overlap=2, bg_later=bgw)
+    o, prob = make(w)
+    o.run(1)
+    sb = prob.sigma_b[:, None, None]
+    middle = [k for k in range(o.nsub) if o.subs[k]["b"] == 1]
+    assert len(middle) == 6 and all(o.subs[k]["gys"] > 0 and o.subs[k]["gyn"] > 0 for k in middle)
+    for k in middle + [0, o.nsub - 1]:
+        x = o.get_control(k) + 0.5 * sb * synth.random_fields(o.sub_shape(k), 70 + k)
+        parts, g, _ = o.eval_local(k, x)
+        assert parts[3] > 0
+        if o.subs[k]["jw"] > 0:
+            assert (parts[1] > 0) == (bgw > 0)
+        fd_check(lambda z: o.eval_local(k, z, want_grad=False)[0][0], x, g, sb, range(300, 303))
+
+
 def identity_model(w, **kw):
     """dt = 0 and kappa = 0 make Phi the identity."""
     args = dict(nlon=w.nlon, nlat=w.nlat, dt=0.0, nsteps=w.nsteps, diffusion=0.0)
