@@ -71,6 +71,22 @@ def algorithmic_bytes(subs, q_time, nobs_binned, with_gw=False):
     return fwd, adj, pts
 
 
+def survey_bytes(subs, nobs_binned):
+    """SURVEY.md 8(d)'s accounting, per sweep and kernel: what the METHOD has to move, not what this implementation
+    moves -- 48 B per processed point-step (state read + write), the ghost ring, 0.2 B of observations and 126 B per
+    control cell of fixed traffic (control, u^b, neighbour data, gradient), split evenly between the two sweeps (about
+    61 B per processed point-step on config 3; algorithmic_bytes() above counts 64.5 B because it includes ck_cost's
+    re-reads).  The 0.60 target of north_star is read against THIS count (roofline.frac_survey_bytes)."""
+    fwd = adj = 0
+    for s in subs:
+        nc = s["ex"] * s["ey"]
+        nring = (s["ex"] + 2 * s["gx"]) * (s["ey"] + s["gys"] + s["gyn"]) - nc
+        W = s["e"] - s["s"]
+        fwd += 24 * W * nc + 24 * W * nring + 63 * nc
+        adj += 24 * W * nc + 24 * W * nring + 63 * nc
+    return fwd + 10 * nobs_binned, adj + 10 * nobs_binned
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -401,9 +417,30 @@ def run_sweep(args):
                 "useful_point_steps_per_s": w.nlon * w.nlat * w.nsteps / (ms * 1e-3), "outer_iters": outer,
                 "time_to_analysis_s": tta, "J_first": float(hist[0, 0]), "J_last": float(hist[-1, 0]),
                 "delta_last": float(hist[-1, 2])}
+        g.close()
+        if args.oracle_outer > 0:
+            # the CPU oracle beside it (BASELINE.json configs[4]: "against the oracle"): the same layout and inputs, one
+            # gradient sweep of every subdomain (median of 2 after a warm-up) and `oracle_outer` outer iterations of
+            # Algorithm 1, on this box's host cores; the 20-iteration time is that per-iteration time scaled up
+            from oracle import Oracle
+            o = Oracle.from_workload(w)
+            o.set_background(prob.xb, prob.sigma_b); o.set_observations(prob.obs)
+            o.sweep_range(0, o.nsub)
+            ts = []
+            for _ in range(2):
+                a = time.perf_counter(); o.sweep_range(0, o.nsub); ts.append(time.perf_counter() - a)
+            osw = float(np.median(ts))
+            a = time.perf_counter(); _, oh = o.run(args.oracle_outer); orun = time.perf_counter() - a
+            line.update({"oracle_cores": cpu_cores(), "oracle_sweep_ms": 1e3 * osw,
+                         "oracle_useful_point_steps_per_s": w.nlon * w.nlat * w.nsteps / osw,
+                         "oracle_outer_iters": args.oracle_outer, "oracle_s_per_outer_iteration": orun / args.oracle_outer,
+                         "oracle_time_to_analysis_s_scaled": orun / args.oracle_outer * outer,
+                         "sweep_speedup_vs_oracle": osw / (ms * 1e-3),
+                         "time_to_analysis_speedup_vs_oracle": orun / args.oracle_outer * outer / tta,
+                         "oracle_J_after": float(oh[-1, 0]), "gpu_J_after_same_iters": float(hist[min(args.oracle_outer, outer), 0])})
+            del o
         run_sweep.done = getattr(run_sweep, "done", []) + [line]
         print(json.dumps(line), flush=True)
-        g.close()
 
 
 def main():
@@ -422,6 +459,7 @@ def main():
     ap.add_argument("--n-gn", type=int, default=2)
     ap.add_argument("--n-cg", type=int, default=5)
     ap.add_argument("--sweep", action="store_true", help="config 4: decomposition sweep on the 0.5 deg problem")
+    ap.add_argument("--oracle-outer", type=int, default=0, help="with --sweep: also time the CPU oracle on every layout (one sweep + this many outer iterations)")
     ap.add_argument("--outer", type=int, default=None, help="outer iterations for --sweep (default: the config's)")
     ap.add_argument("--peaks", action="store_true", help="run the library's fp64 / shared-memory / shuffle microbenchmarks")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash of the CUDA sources (for profiles/traffic.json)")
@@ -495,6 +533,7 @@ def main():
     for lev in lv:
         nobs_binned += per_level * sum(1 for (s0, e0) in wins if s0 <= lev <= e0)
     fwd_b, adj_b, pts = algorithmic_bytes(g.subs, w.q_time, nobs_binned)
+    sv_fwd, sv_adj = survey_bytes(g.subs, nobs_binned)
     useful = w.nlon * w.nlat * w.nsteps
 
     stream = torch.cuda.current_stream(dev)
@@ -555,6 +594,11 @@ def main():
     g.run(1)
     outer_ng_s = time.perf_counter() - t0
     g.set_history_global(True)
+    # the same outer iteration split by phase with CUDA events on the library's stream (dd4dvar_set_phase_timing)
+    g.set_phase_timing(True)
+    g.run(1)
+    phase = g.phase_ms()
+    g.set_phase_timing(False)
     ms, e2e_s, outer_s, outer_ng_s = max_over_ranks([ms, e2e_s, outer_s, outer_ng_s], dev)
 
     if rank == 0:
@@ -580,7 +624,12 @@ def main():
                        "l2": "inputs larger than L2 (trajectory store %.1f GB per sweep)" % (24.0 * pts / 1e9),
                        "parallelism": "replicas" if world > 1 else "single GPU",
                        "outer_iteration_ms": 1e3 * outer_s, "outer_iteration_ms_without_global_history": 1e3 * outer_ng_s,
-                       "outer_iteration": "run(1) after one untimed run(1): 5 L-BFGS iterations (a5) + exchange (a6) + J_global, not in the timed region"},
+                       "outer_iteration": "run(1) after one untimed run(1): 5 L-BFGS iterations (a5) + exchange (a6) + J_global, not in the timed region",
+                       "sweeps_ms": phase["sweeps"], "lbfgs_ms": phase["lbfgs"], "exchange_ms": phase["exchange"],
+                       "jglobal_ms": phase["jglobal"], "gather_ms": phase["gather"],
+                       "outer_iteration_split": "CUDA events on the library's stream inside one more run(1): sweeps (a1-a4 of every "
+                                                "trial and accepted point), L-BFGS kernels incl. the host round trip of each line-search "
+                                                "check (a5), exchange (a6), J_global diagnostic, final gather"},
             "clocks": clocks,
             "e2e": {"value": world * useful / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(g.ctot * 8),
                     "d2h_bytes_per_step": int(g.ctot * 8 + g.nsub * 8), "ms_per_step": 1e3 * e2e_s},
@@ -596,7 +645,13 @@ def main():
                                             "achieved": fwd_b / (t_f * 1e-3) / 1e9, "frac": fwd_b / (t_f * 1e-3) / 1e9 / peak,
                                             "traffic": measured_traffic(fname, args.config) if fused else None,
                                             "note": "forward sweep + trajectory store + cost terms (wk_forward and ck_cost, timed together)"},
-                         "bytes_per_processed_point_step": (fwd_b + adj_b) / pts},
+                         "bytes_per_processed_point_step": (fwd_b + adj_b) / pts,
+                         "frac_survey_bytes": (sv_adj if fused else sv_fwd + sv_adj) / (kt * 1e-3) / 1e9 / peak,
+                         "sweep_frac_survey_bytes": (sv_fwd + sv_adj) / (ms_step * 1e-3) / 1e9 / peak,
+                         "forward_frac_survey_bytes": sv_fwd / (t_f * 1e-3) / 1e9 / peak,
+                         "survey_bytes_per_processed_point_step": (sv_fwd + sv_adj) / pts,
+                         "target": "north_star's 0.60 is read against frac_survey_bytes / sweep_frac_survey_bytes (SURVEY.md 8(d): "
+                                   "~61 B per processed point-step); frac uses this implementation's own count"},
         }
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(w)

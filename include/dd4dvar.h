@@ -250,6 +250,16 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later);
  * Algorithm 1).  on = 0: skip it, column 0 is NaN; default on. */
 int dd4dvar_set_history_global(dd4dvar_t h, int on);
 
+/* Where the time of dd4dvar_run goes (the L-BFGS passes and the exchange are timed separately and
+ * reported).  on = 1: dd4dvar_run records CUDA events on its stream at every change of phase; after it returns,
+ * dd4dvar_get_phase_ms gives the device time of that run per phase, in ms: [0] gradient / trial sweeps (a1-a4),
+ * [1] L-BFGS kernels, resets and the host round trips of the line search (a5), [2] exchange (a6), [3] the J_global
+ * diagnostic (dd4dvar_set_history_global), [4] final gather.  Idle time of the stream while the host decides (the
+ * check of the line search, the sums of the history) falls into the phase that was open.  Default off: nothing is
+ * recorded.  The events are created on first use and destroyed with the handle. */
+int dd4dvar_set_phase_timing(dd4dvar_t h, int on);
+int dd4dvar_get_phase_ms(dd4dvar_t h, double h_out[5]);
+
 /* Sharded runs, one process per GPU: within an outer iteration the local problems are independent
  * (eq (37) l.433) and there is one exchange step per outer iteration (Alg 1 l.465).  Every process holds the whole
  * problem and OWNS the subdomains of the time windows [j0, j1): dd4dvar_run moves only those; its exchange freezes the

@@ -52,7 +52,7 @@ EXPORTS = [
     "dd4dvar_get_local_trajectory", "dd4dvar_forecast", "dd4dvar_forecast_static", "dd4dvar_num_subdomains",
     "dd4dvar_subdomain_info", "dd4dvar_control_offset", "dd4dvar_active_path", "dd4dvar_launch_count",
     "dd4dvar_measure_peaks", "dd4dvar_set_bg_weight", "dd4dvar_run_gn", "dd4dvar_gn_hessvec", "dd4dvar_set_history_global", "dd4dvar_set_overlap_levels", "dd4dvar_set_owned_windows", "dd4dvar_exchange_buffer",
-    "dd4dvar_get_local_stats", "dd4dvar_gather_analysis",
+    "dd4dvar_get_local_stats", "dd4dvar_gather_analysis", "dd4dvar_set_phase_timing", "dd4dvar_get_phase_ms",
     "dd4dvar_last_error", "dd4dvar_destroy",
 ]
 
@@ -103,6 +103,8 @@ def load_library():
     lib.dd4dvar_exchange_buffer.argtypes = [vp, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_longlong)]
     lib.dd4dvar_get_local_stats.argtypes = [vp, hd, hd]
     lib.dd4dvar_gather_analysis.argtypes = [vp, dp]
+    lib.dd4dvar_set_phase_timing.argtypes = [vp, C.c_int]
+    lib.dd4dvar_get_phase_ms.argtypes = [vp, hd]
     lib.dd4dvar_last_error.restype = C.c_char_p
     lib.dd4dvar_last_error.argtypes = [vp]
     lib.dd4dvar_destroy.restype = None
@@ -378,6 +380,15 @@ class DD4DVar:
     def set_overlap_levels(self, on):
         """(25c) case 1 on every level of the window (generic kernels only; before set_background)."""
         self._check("dd4dvar_set_overlap_levels", self.lib.dd4dvar_set_overlap_levels(self._h, int(bool(on))))
+
+    def set_phase_timing(self, on):
+        """Record CUDA-event marks inside run(): phase_ms() then gives the device time of the last run per phase."""
+        self._check("dd4dvar_set_phase_timing", self.lib.dd4dvar_set_phase_timing(self._h, int(bool(on))))
+
+    def phase_ms(self):
+        out = np.zeros(5)
+        self._check("dd4dvar_get_phase_ms", self.lib.dd4dvar_get_phase_ms(self._h, _hd(out)))
+        return dict(zip(("sweeps", "lbfgs", "exchange", "jglobal", "gather"), out.tolist()))
 
     def set_history_global(self, on):
         self._check("dd4dvar_set_history_global", self.lib.dd4dvar_set_history_global(self._h, int(bool(on))))

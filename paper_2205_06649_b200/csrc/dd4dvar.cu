@@ -130,6 +130,11 @@ struct dd4dvar_s {
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_in = nullptr, ev_h2d[EH_CHUNKS] = {}, ev_sw[EH_CHUNKS] = {}, ev_out = nullptr;
     int* h_pin = nullptr;               // pinned scratch for small read-backs
+    // dd4dvar_set_phase_timing: CUDA-event marks inside dd4dvar_run (off by default: no event is recorded)
+    bool ph_on = false;
+    std::vector<cudaEvent_t> ph_ev;     // pool, reused by every run
+    std::vector<int> ph_kind;           // ph_kind[i] = phase that starts at mark i (-1: none)
+    double ph_ms[5] = { 0, 0, 0, 0, 0 };
     std::vector<double> h_tmp;
 };
 
@@ -549,12 +554,6 @@ void sweep(dd4dvar_t h, Layout& L, bool with_adjoint, const int* mask, double* J
     if (L.path == 4 || L.path == 5) {
         // forward sweep + trajectory store + H (25b) in the wavefront kernel, then the control-level terms (ck_cost)
         WkArgs a = wave_args(h, L, mask, Jout, gw);
-#ifdef WK_PROF      // profiling build (_work only): per-phase cycle counters of wk_forward on stderr
-        static unsigned long long* d_prof = nullptr;
-        if (!d_prof) cudaMalloc(&d_prof, 8 * 16 * 8);
-        cudaMemsetAsync(d_prof, 0, 8 * 16 * 8, h->stream);
-        a.gw = reinterpret_cast<double*>(d_prof);
-#endif
         if (L.wp.K == 2) wk_forward<2><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         else wk_forward<3><<<L.wp.grid, WK_NT, L.wp.smem_fwd, h->stream>>>(a);
         ++h->launches;
@@ -595,6 +594,33 @@ int sync_check(dd4dvar_t h)
     CU(cudaStreamSynchronize(h->stream));
     CU(cudaGetLastError());
     return 0;
+}
+
+// Phase marks of dd4dvar_run (dd4dvar_set_phase_timing): a mark closes the phase that is open and opens phase `kind`
+// (0 sweeps, 1 L-BFGS kernels and their host round trips, 2 exchange, 3 J_global diagnostic, 4 gather / other; -1 none).
+enum { PH_SWEEP = 0, PH_LBFGS = 1, PH_EXCH = 2, PH_JGLOBAL = 3, PH_OTHER = 4 };
+void ph_mark(dd4dvar_t h, int kind)
+{
+    if (!h->ph_on) return;
+    const size_t i = h->ph_kind.size();
+    if (i == h->ph_ev.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) { h->ph_on = false; return; }
+        h->ph_ev.push_back(e);
+    }
+    cudaEventRecord(h->ph_ev[i], h->stream);
+    h->ph_kind.push_back(kind);
+}
+// after the stream has been synchronised: add the time between consecutive marks to the phase the first one opened
+void ph_collect(dd4dvar_t h)
+{
+    if (!h->ph_on) return;
+    for (size_t i = 0; i + 1 < h->ph_kind.size(); ++i) {
+        float ms = 0.f;
+        if (h->ph_kind[i] >= 0 && cudaEventElapsedTime(&ms, h->ph_ev[i], h->ph_ev[i + 1]) == cudaSuccess)
+            h->ph_ms[h->ph_kind[i]] += ms;
+    }
+    h->ph_kind.clear();
 }
 
 // J of eq (6) at a global state already in G.x
@@ -1077,14 +1103,20 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, G.x);
         return global_cost(h, out);
     };
+    h->ph_kind.clear();
+    for (double& v : h->ph_ms) v = 0.0;
+    ph_mark(h, PH_JGLOBAL);
     if ((rc = gather_and_cost(&h_history[0]))) return rc;
+    ph_mark(h, PH_LBFGS);
     CU(cudaMemsetAsync(L.st.nactive, 0, 2 * sizeof(int), h->stream));
     h_history[1] = 0.0; h_history[2] = 0.0;
     const dim3 vgrid(std::min(64, (3 * L.maxncell + 255) / 256), nsub);
     if (outer_iters == 0) {
         LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        ph_mark(h, PH_SWEEP);
         sweep(h, L, false, own, L.st.J, nullptr);
+        ph_mark(h, PH_LBFGS);
         if ((rc = sumJ(L.st.J, &h_history[1]))) return rc;
     }
     for (int l = 1; l <= outer_iters; ++l) {
@@ -1095,14 +1127,18 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
         else CU(cudaMemsetAsync(L.st.done, 0, sizeof(int) * nsub, h->stream));
         LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        ph_mark(h, PH_SWEEP);
         sweep(h, L, true, own, L.st.J, L.g);
+        ph_mark(h, PH_LBFGS);
         if (l == 1 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
         for (int it = 0; it < h->opt.n_inner; ++it) {
             LAUNCH(lk_direction<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.g, L.S, L.Y, L.d);
             for (int b = 0; b <= lp.max_bt; ++b) {
                 CU(cudaMemsetAsync(L.st.nactive, 0, sizeof(int), h->stream));
                 LAUNCH(lk_trial, vgrid, 256, L.dsubs, L.st.active, h->cp, L.st.t, L.w, L.d, L.xbs, L.wt, L.x);
+                ph_mark(h, PH_SWEEP);
                 sweep(h, L, false, L.st.active, L.st.Jt, nullptr);
+                ph_mark(h, PH_LBFGS);
                 LAUNCH(lk_lscheck, (nsub + 127) / 128, 128, nsub, lp, L.st);
                 int nact[2] = { 0, 0 };
                 CU(cudaMemcpyAsync(nact, L.st.nactive, 2 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
@@ -1111,24 +1147,49 @@ int dd4dvar_run(dd4dvar_t h, int outer_iters, double* d_analysis, double* h_hist
                 if (nact[0] == 0) break;
             }
             // gradient at the accepted points (their trajectories are still in the store)
+            ph_mark(h, PH_SWEEP);
             adjoint_only(h, L, L.st.ok, L.gn);
+            ph_mark(h, PH_LBFGS);
             LAUNCH(lk_update<NT_LB>, nsub * LK_CL, NT_LB, L.dsubs, lp, L.st, L.w, L.wt, L.g, L.gn, L.S, L.Y);
         }
         // one more forward sweep so that the stored trajectory belongs to the accepted iterate
         LAUNCH(lk_trial, vgrid, 256, L.dsubs, own, h->cp, (const double*)nullptr, L.w,
                (const double*)nullptr, L.xbs, (double*)nullptr, L.x);
+        ph_mark(h, PH_SWEEP);
         sweep(h, L, false, own, L.Jev, nullptr);
+        ph_mark(h, PH_LBFGS);
         if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
+        ph_mark(h, PH_EXCH);
         exchange(h, L);
         CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
         if ((rc = sync_check(h))) return rc;
         double dl = 0; for (int k = 0; k < nsub; ++k) dl = std::max(dl, h->h_tmp[k]);
         h_history[3 * l + 2] = dl;
+        ph_mark(h, PH_JGLOBAL);
         if ((rc = gather_and_cost(&h_history[3 * l]))) return rc;
+        ph_mark(h, PH_LBFGS);
         if ((h->history_global && !isfinite(h_history[3 * l])) || !isfinite(h_history[3 * l + 1])) return fail(h, -5, "run: non-finite cost");
     }
+    ph_mark(h, PH_OTHER);
     LAUNCH(xk_gather, (n1 + 255) / 256, 256, L.dsubs, L.geo, 1, 0, L.xfrozen, d_analysis);
-    return sync_check(h);
+    ph_mark(h, -1);
+    rc = sync_check(h);
+    ph_collect(h);
+    return rc;
+}
+
+int dd4dvar_set_phase_timing(dd4dvar_t h, int on)
+{
+    if (!h) return -1;
+    h->ph_on = on != 0;
+    return 0;
+}
+
+int dd4dvar_get_phase_ms(dd4dvar_t h, double h_out[5])
+{
+    if (!h || !h_out) return -1;
+    for (int q = 0; q < 5; ++q) h_out[q] = h->ph_ms[q];
+    return 0;
 }
 
 // ---- Gauss-Newton local minimiser (gn_kernels.cuh): wavefront layouts only ------------------
@@ -1176,6 +1237,7 @@ int dd4dvar_gn_hessvec(dd4dvar_t h, const double* d_controls, const double* d_p,
     if (!h->have_bg) return fail(h, -3, "gn_hessvec before set_background");
     Layout& L = h->L;
     if (L.path == 2 || L.path == 4 || !L.gn_Hp) return fail(h, -2, "gn_hessvec: the Gauss-Newton solver is served by the wavefront (path 5) and the generic kernels (path 1, 3)");
+    if (h->overlap_levels) return fail(h, -2, "gn_hessvec: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
     CU(cudaMemcpyAsync(L.x, d_controls, sizeof(double) * L.ctot, cudaMemcpyDeviceToDevice, h->stream));
     sweep(h, L, false, nullptr, L.Jev, nullptr);
     int rc = gn_apply(h, L, d_p, L.gn_Hp);
@@ -1192,6 +1254,7 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
     Layout& L = h->L; Layout& G = h->G;
     if (L.path == 2 || L.path == 4 || !L.gn_Hp) return fail(h, -2, "run_gn: the Gauss-Newton solver is served by the wavefront (path 5) and the generic kernels (path 1, 3)");
     if (L.sharded) return fail(h, -2, "run_gn: not available in sharded runs (dd4dvar_set_owned_windows)");
+    if (h->overlap_levels) return fail(h, -2, "run_gn: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
     const int n1 = h->grid.nlon * h->grid.nlat;
     const int nsub = L.nsub;
     h->h_tmp.resize(std::max(nsub, 8));
@@ -1237,7 +1300,6 @@ int dd4dvar_run_gn(dd4dvar_t h, int outer_iters, int n_gn, int n_cg, double* d_a
         sweep(h, L, false, nullptr, L.st.J, nullptr);
         if (l == 1 && n_gn == 0 && (rc = sumJ(L.st.J, &h_history[1]))) return rc;
         if ((rc = sumJ(L.st.J, &h_history[3 * l + 1]))) return rc;
-    if (h->overlap_levels) return fail(h, -2, "gn_hessvec: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
         exchange(h, L);
         CU(cudaMemcpyAsync(h->h_tmp.data(), L.dmax, sizeof(double) * nsub, cudaMemcpyDeviceToHost, h->stream));
         if ((rc = sync_check(h))) return rc;
@@ -1254,7 +1316,6 @@ int dd4dvar_set_bg_weight(dd4dvar_t h, double w_later)
 {
     if (!h || !(w_later >= 0.0)) return fail(h, -1, "set_bg_weight: weight must be >= 0");
     h->cp.bgw = w_later;
-    if (h->overlap_levels) return fail(h, -2, "run_gn: not available with dd4dvar_set_overlap_levels (the all-level overlap penalty has no Gauss-Newton path)");
     return 0;
 }
 
@@ -1351,6 +1412,7 @@ void dd4dvar_destroy(dd4dvar_t h)
 {
     if (!h) return;
     fused_teardown(h->stream, h->L.fp);
+    for (cudaEvent_t e : h->ph_ev) cudaEventDestroy(e);
     if (h->s_h2d) {
         cudaStreamSynchronize(h->s_h2d); cudaStreamSynchronize(h->s_d2h);
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);

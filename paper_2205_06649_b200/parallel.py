@@ -83,7 +83,13 @@ class ShardedDD4DVar:
         for l in range(1, outer_iters + 1):
             g.run(1)
             if self.world > 1:
+                # The broadcasts are queued behind torch's CURRENT stream; the library works on g.stream, which need not
+                # be the same one.  Order them explicitly on both sides: the collectives after this iteration's kernels,
+                # the next iteration's kernels after the collectives (not left to the host-blocking reductions below).
+                cur = torch.cuda.current_stream(g.device)
+                cur.wait_stream(g.stream)
                 exchange((g.exchange_view(0), g.exchange_view(1)), self.plan, self.dist)
+                g.stream.wait_stream(cur)
             J, dm = g.local_stats()
             red = torch.tensor([J[self.owned].sum()], dtype=torch.float64, device=g.device)
             mx = torch.tensor([dm[self.owned].max() if self.owned.any() else 0.0], dtype=torch.float64, device=g.device)

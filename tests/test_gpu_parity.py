@@ -310,3 +310,46 @@ def test_eval_local_host_equals_eval_local(cfg):
         g.eval_local_host(h_ctrl, h_cost, h_grad)
         assert np.array_equal(h_cost, costs)
         assert np.array_equal(h_grad.numpy(), grads.cpu().numpy())
+
+
+def test_phase_timing_of_run_adds_up_and_is_off_by_default():
+    """dd4dvar_set_phase_timing: the per-phase device times of one run (L-BFGS and exchange timed
+    separately) are positive where work was done, add up to less than the wall time of the call, and change nothing."""
+    import time
+    w, o, prob, g = make_pair("wave_k2", 0)
+    a1, h1 = g.run(1)
+    assert all(v == 0.0 for v in g.phase_ms().values())
+    g2 = gpu_problem(w, prob)
+    g2.set_phase_timing(True)
+    t0 = time.perf_counter()
+    b1, k1 = g2.run(1)
+    wall = 1e3 * (time.perf_counter() - t0)
+    ph = g2.phase_ms()
+    assert ph["sweeps"] > 0 and ph["lbfgs"] > 0 and ph["exchange"] > 0 and ph["jglobal"] > 0
+    assert sum(ph.values()) <= wall
+    assert np.array_equal(a1.cpu().numpy(), b1.cpu().numpy()) and np.array_equal(h1, k1)
+    g2.set_history_global(False)
+    g2.run(1)
+    assert g2.phase_ms()["jglobal"] < 0.05          # two marks with nothing between them
+    g.close(); g2.close()
+
+
+def test_eval_local_host_chunked_path_with_pageable_buffers():
+    """64 subdomains take the chunked path of dd4dvar_eval_local_host.  With pageable host buffers (plain numpy arrays)
+    the copies block the host and the overlap is lost (include/dd4dvar.h says so), but the results must still be those
+    of dd4dvar_eval_local, bit for bit, as with pinned buffers."""
+    import torch
+    w = small_workload(nlon=64, nlat=32, nsteps=16, p_lon=4, p_lat=4, q_time=4, overlap=1, dt=300.0)
+    o, prob = oracle_problem(w)
+    g = gpu_problem(w, prob)
+    assert g.nsub == 64
+    x = g.pack(perturbed_controls(o, prob, 3))
+    costs, _, grads = g.eval_local(x)
+    h_x = x.cpu().numpy().copy()                        # pageable
+    h_c = np.zeros(g.nsub); h_g = np.zeros(g.ctot)
+    g.eval_local_host(h_x, h_c, h_g)
+    assert np.array_equal(h_c, costs) and np.array_equal(h_g, grads.cpu().numpy())
+    p_x = x.cpu().pin_memory(); p_g = torch.empty_like(p_x).pin_memory(); p_c = np.zeros(g.nsub)
+    g.eval_local_host(p_x, p_c, p_g)
+    assert np.array_equal(p_c, costs) and np.array_equal(p_g.numpy(), h_g)
+    g.close()

@@ -59,3 +59,32 @@ def test_sharded_driver_with_one_rank_is_the_plain_run():
     an, hist = sh.run(2)
     assert np.array_equal(an.cpu().numpy(), an_s.cpu().numpy())
     assert np.allclose(hist[1:, 0], hist_s[1:, 1], rtol=1e-13) and np.array_equal(hist[1:, 1], hist_s[1:, 2])
+
+
+def test_two_ranks_over_nccl_reproduce_the_single_run():
+    """The same statement over NCCL with one process per GPU, the library on a stream that is not torch's current
+    stream (parallel.ShardedDD4DVar orders the broadcasts against it).  Needs two GPUs; skipped on a one-GPU box."""
+    import os
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    worker = os.path.join(os.path.dirname(os.path.abspath(__file__)), "nccl_shard_worker.py")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29547", worker],
+                       capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "nccl shard worker ok" in r.stdout, r.stdout[-3000:] + r.stderr[-3000:]
+
+
+def test_sharded_driver_on_a_side_stream_with_one_rank():
+    """One rank, library on a side stream: the driver and its stream ordering code run (no exchange with one rank)."""
+    import torch
+    w = small_workload(**LAYOUTS["wave_k2"])
+    o, prob = oracle_problem(w)
+    single = gpu_problem(w, prob)
+    an_s, _ = single.run(2)
+    sh = parallel.ShardedDD4DVar(w, stream=torch.cuda.Stream())
+    sh.set_background(prob.xb, prob.sigma_b); sh.set_observations(prob.obs)
+    an, _ = sh.run(2)
+    assert np.array_equal(an.cpu().numpy(), an_s.cpu().numpy())
