@@ -4,9 +4,12 @@ Within an outer iteration the local problems are independent (eq (37)
 iteration (Alg 1) is what crosses processes.  Spatial neighbours of a subdomain lie in its own window,
 so with whole windows per process only two control-shaped arrays cross: the frozen controls (a window's successor
 term (25c) reads the NEXT window's controls) and the predecessor end states (read by the next window).  Every process
-holds the whole problem (22 GB of 180 GB at the 0.25 deg config) and moves only what it owns, so the exchange is one
-broadcast per owner and array (NCCL over NVLink: 2 x 226 MB per outer iteration at the 0.25 deg config against
-~70 ms of sweeps), plus two scalar reductions for the history.  No arithmetic of the method lives here.
+holds the whole problem (22 GB of 180 GB at the 0.25 deg config) and moves only what it owns.  An owned window reads
+from other ranks only the controls of the window after its block and the end states of the window before it, so the
+exchange of an iteration is point-to-point with the ranks r +- 1 (`exchange_neighbours`: 2 x one window's slice per block
+boundary, 2 x 28 MB per rank at the 0.25 deg config on 8 GPUs), plus two scalar reductions for the history and one broadcast
+of window 0's controls at the end of a run for the gather.  `exchange` (every owner broadcasts its whole block) is kept
+as the plain-collective form and for the tests.  No arithmetic of the method lives here.
 """
 from __future__ import annotations
 
@@ -44,6 +47,40 @@ def exchange(buffers, plan, dist=None):
                 dist.broadcast(buf[lo:hi], src=r)
 
 
+def neighbour_plan(offsets, p12: int, q_time: int, world: int):
+    """What an owned window really reads from another rank: its successor term (25c) reads the controls of the NEXT window,
+    its predecessor term the end states of the window BEFORE it.  With contiguous blocks of windows that is one window's
+    slice per block boundary and direction.  -> list of (buffer, lo, hi, src, dst): at the boundary window j between rank a
+    (owns j - 1) and rank b (owns j), the frozen controls of window j go b -> a and the end states of window j - 1, which
+    are stored at the entries of window j, go a -> b."""
+    blocks = window_blocks(q_time, world)
+    owners = [r for r, (j0, j1) in enumerate(blocks) if j1 > j0]
+    ops = []
+    for a, b in zip(owners[:-1], owners[1:]):
+        j = blocks[b][0]
+        lo, hi = offsets[j * p12], offsets[(j + 1) * p12]
+        ops.append((0, lo, hi, b, a))
+        ops.append((1, lo, hi, a, b))
+    return ops
+
+
+def exchange_neighbours(buffers, ops, rank: int, dist=None):
+    """The exchange of one outer iteration as point-to-point transfers between ranks r and r +- 1 (2 x one window per
+    boundary instead of every rank's whole block to everyone; config 3 on 8 GPUs: 2 x 28 MB per rank against 2 x 226 MB).
+    After it a rank holds valid frozen data for the windows it owns and the two windows next to them, nothing else."""
+    if dist is None:
+        import torch.distributed as dist
+    reqs = []
+    for which, lo, hi, src, dst in ops:
+        if rank == src:
+            reqs.append(dist.P2POp(dist.isend, buffers[which][lo:hi], dst))
+        elif rank == dst:
+            reqs.append(dist.P2POp(dist.irecv, buffers[which][lo:hi], src))
+    if reqs:
+        for w in dist.batch_isend_irecv(reqs):
+            w.wait()
+
+
 class ShardedDD4DVar:
     """Algorithm 1 with the windows sharded over the ranks of the default process group."""
 
@@ -65,6 +102,7 @@ class ShardedDD4DVar:
             g.set_owned_windows(self.j0, self.j1)
             g.set_history_global(False)
         self.plan = exchange_plan(g.offsets, self.p12, self.q, self.world)
+        self.nb_ops = neighbour_plan(g.offsets, self.p12, self.q, self.world)
         self.owned = np.zeros(g.nsub, dtype=bool)
         self.owned[self.j0 * self.p12:self.j1 * self.p12] = True
 
@@ -88,7 +126,7 @@ class ShardedDD4DVar:
                 # the next iteration's kernels after the collectives (not left to the host-blocking reductions below).
                 cur = torch.cuda.current_stream(g.device)
                 cur.wait_stream(g.stream)
-                exchange((g.exchange_view(0), g.exchange_view(1)), self.plan, self.dist)
+                exchange_neighbours((g.exchange_view(0), g.exchange_view(1)), self.nb_ops, self.rank, self.dist)
                 g.stream.wait_stream(cur)
             J, dm = g.local_stats()
             red = torch.tensor([J[self.owned].sum()], dtype=torch.float64, device=g.device)
@@ -97,6 +135,13 @@ class ShardedDD4DVar:
                 self.dist.all_reduce(red, op=self.dist.ReduceOp.SUM)
                 self.dist.all_reduce(mx, op=self.dist.ReduceOp.MAX)
             hist[l, 0] = float(red[0]); hist[l, 1] = float(mx[0])
+        if self.world > 1:
+            # the analysis (eq (12)-(13)) is gathered from the frozen controls of window 0, which only its owner and that
+            # owner's neighbour hold after neighbour exchanges: one broadcast of that window's slice at the end of the run
+            cur = torch.cuda.current_stream(g.device)
+            cur.wait_stream(g.stream)
+            self.dist.broadcast(g.exchange_view(0)[g.offsets[0]:g.offsets[self.p12]], src=0)
+            g.stream.wait_stream(cur)
         return g.gather_analysis(), hist
 
     def close(self):
